@@ -1,0 +1,87 @@
+/* mkfo.h — C ABI of the ORACLE (test infrastructure, not the product).
+ *
+ * Plain, slow, float64 CPU restatement of the mkFit-style Kalman-filter hot path described in
+ * /root/reference/PAPER.md (arxiv 2002.06295): propagate a track state layer to layer, update it with a
+ * hit (§1), on a lightweight geometry of barrel layers at average r and forward layers at
+ * average z with 3D hits (§2), combinatorial building with a per-seed cap on cloned
+ * candidates, short-track preservation and duplicate removal (abstract).
+ * The paper prints no formulas (PAPER.md:29 defers to its refs [3-12]); every formula here follows the
+ * readings C1..C10 / U1..U22 listed in DESIGN.md §3, and is pinned by tests/test_oracle_*.py.
+ *
+ * ONLY tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load this
+ * library. It shares no code, header, table or constant with paper_2002_06295_b200/csrc/.
+ *
+ * All pointers are HOST pointers. Inputs are the same fp32 arrays the CUDA library takes, widened exactly
+ * to double; all arithmetic and all outputs are double. Arrays are SoA, plane-major: par[k*n+i],
+ * cov[k*n+i] with k = i*(i+1)/2+j (j<=i) packed lower triangle of the 6x6 covariance.
+ * State u = (x, y, z, ipt, phi, theta): cm, 1/GeV, rad; charge q = +-1 separately. */
+#ifndef MKFO_H
+#define MKFO_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { int kind;            /* 0 barrel cylinder, 1 disk */
+                 float pos;           /* r (barrel) or signed z (disk) */
+                 float lo, hi;        /* barrel: zmin,zmax ; disk: rmin,rmax */
+                 float xx0;           /* thickness in radiation lengths at normal incidence */
+                 float eta_lo, eta_hi;/* hit pseudorapidity range spanned by the eta bins */ } mkfo_layer;
+typedef struct { int n_layers; const mkfo_layer* layers; float bz; int n_phi_bins, n_eta_bins;
+                 int n_plans; const int* plan_off; const int* plan_layers; } mkfo_geometry;
+typedef struct { float chi2_cut; int max_cand; int max_consec_miss; int min_hits_keep;
+                 float score_hit, score_miss; float graze_cos_min; int material_flags; /* 1 MS, 2 dE/dx */
+                 float dup_frac; } mkfo_params;
+typedef struct { int n_events; int n_hits; const int* layer_off; /* [n_events*(n_layers+1)] */
+                 const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */ } mkfo_hits;
+
+enum { MKFO_PROP_UNREACHABLE = 1, MKFO_GRAZING = 2, MKFO_S_NOT_PD = 4, MKFO_NAN = 8,
+       MKFO_STOPPED_ELOSS = 16, MKFO_TRUNCATED = 32 };
+
+/* ---- single-step functions (exported so the pins can reach every formula) ------------------------ */
+/* C1-C4: propagate u (6) with full 6x6 covariance C (36, row-major, may be NULL) to a surface.
+ * kind 0: cylinder r=pos; kind 1: plane z=pos. Outputs u1 (6), F (36, may be NULL), C1 (36, may be NULL),
+ * s (transverse path). Returns 0 or MKFO_PROP_UNREACHABLE. */
+int mkfo_propagate(int kind, double pos, double bz, int q, const double* u, const double* C,
+                   double* u1, double* F, double* C1, double* s);
+/* C1 alone: helix step by transverse path s. */
+void mkfo_helix_step(double bz, int q, const double* u, double s, double* u1);
+/* C5: material at a layer (state already on the surface). In/out u (6), C (36). Returns 0 or STOPPED_ELOSS.
+ * theta0_out / dE_out (may be NULL) receive the Highland angle and the energy loss. */
+int mkfo_material(int kind, double xx0, int flags, double* u, double* C, double* theta0_out, double* dE_out);
+/* Bethe-Bloch -dE/dx [GeV/cm] in silicon for a pion of momentum p [GeV]; Highland theta0 for thickness t. */
+double mkfo_dedx(double p);
+double mkfo_highland(double p, double t);
+/* C6: chi2 of hit m (3) with covariance V (6: xx,xy,yy,xz,yz,zz); returns 0 or S_NOT_PD. */
+int mkfo_chi2(const double* u, const double* C, const double* m, const double* V, double* chi2);
+/* C6: Kalman update (Joseph form). In/out u, C. */
+int mkfo_update(double* u, double* C, const double* m, const double* V, double* chi2);
+/* U11: search window of a propagated state on layer L. Outputs eta-bin range [e0,e1] and phi-bin range
+ * [p0, p0+np) (np<=n_phi, wraps). vmax = (v_xy, v_zz) of the layer's hits. */
+void mkfo_window(const mkfo_geometry* g, const mkfo_params* p, int layer, const double* u, const double* C,
+                 const double* vmax, int* e0, int* e1, int* p0, int* np);
+
+/* ---- the four calls named by BASELINE.json north_star -------------------------------------------- */
+/* C8. bin_off [n_events*n_layers*n_phi*n_eta + 1], sorted_id [n_hits], vmax [n_events*n_layers*2]. */
+int mkfo_build_hit_index(const mkfo_geometry*, const mkfo_hits*, unsigned* bin_off, int* sorted_id, float* vmax);
+/* C7. seeds par[6][n] cov[21][n] (fp32), q[n]; plan[n]; track_hits[max_plan_len][n] (global hit id or <0).
+ * Outputs (double) par_out[6][n], cov_out[21][n], chi2[n], nfit[n], status[n]. */
+int mkfo_fit(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,
+             const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
+             int max_plan_len, double* par_out, double* cov_out, double* chi2, int* nfit, unsigned* status);
+/* C9. brute_force!=0: every hit of the layer is tried (small events); else the binned window search.
+ * hit_ids [max_plan_len][n]: id | -1 miss | -2 not crossed. margin[n]: smallest decision margin met (U20).
+ * n_chi2_evals (may be NULL): number of (candidate,hit) chi2 evaluations done. */
+int mkfo_build_tracks(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, const unsigned* bin_off,
+             const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,
+             const float* cov, const signed char* q, const int* seed_event, const int* seed_hits,
+             const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
+             double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
+             long long* n_chi2_evals);
+/* C10. track_off[n_events+1]; hit_ids[max_plan_len][n]; keep[n], n_kept[n_events]. */
+int mkfo_remove_duplicates(const mkfo_params*, int n_events, const int* track_off, const int* hit_ids,
+             int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept);
+int mkfo_num_threads(void);
+#ifdef __cplusplus
+}
+#endif
+#endif
