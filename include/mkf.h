@@ -1,0 +1,148 @@
+/* mkf.h — C ABI of the B200-native (sm_100a) batched Kalman-filter track fit / track building library.
+ *
+ * Hot path of arxiv 2002.06295 (mkFit, /root/reference/PAPER.md): "propagate a track state from layer N-1 to
+ * layer N, update it with the hit" (§1), on a "lightweight" geometry of barrel layers collapsed at
+ * their average r and forward layers at their average z, relying on 3D hit positions (§2), with
+ * combinatorial building where "only the best ranking [candidates] are cloned at each layer (with a per-seed
+ * cap)", short-track preservation and explicit duplicate removal (PAPER.md:5 abstract), and a
+ * fit that "applies the KF procedure to all hits identified during building". The paper prints
+ * no formulas (PAPER.md:29 defers to its refs); the formulas are the readings C1..C10 / U1..U22 of DESIGN.md §3.
+ *
+ * CONVENTIONS
+ *  - Every data pointer of the mkf_* calls below is a DEVICE pointer into caller-owned memory unless marked
+ *    "host". The *_host entry points take HOST pointers for everything and stage through device memory
+ *    themselves. The library never frees or keeps caller memory after a call returns.
+ *  - Calls enqueue work on `stream` (a cudaStream_t passed as void*, NULL = default stream) and do NOT
+ *    synchronise (the *_host entry points do synchronise before returning). Outputs are valid after the
+ *    caller synchronises the stream.
+ *  - Scratch comes from a caller-provided device workspace `ws` of at least mkf_workspace_bytes(...) bytes,
+ *    256-byte aligned. Its contents are undefined between calls.
+ *  - Arrays are SoA, plane-major: par[k*n + i] (k = 0..5: x, y, z [cm], ipt = 1/pT [1/GeV], phi, theta [rad]);
+ *    cov[k*n + i] with k = a*(a+1)/2 + b (b <= a) the packed lower triangle of the symmetric 6x6 covariance.
+ *    The charge q = +-1 is carried separately. Field: uniform Bz [T]; kappa = 0.0029979246 GeV/(T cm).
+ *  - Return value: MKF_OK or a negative error code. Numerical trouble is never an error code: it is reported
+ *    per track in `status` (bit set below). mkf_last_error(ctx) gives a text for the last failing call.
+ *  - All arithmetic is fp32 (positions carried as an unevaluated sum of two floats inside the kernels; the hit
+ *    bin keys are evaluated in fp64, reading U12). No host fallback exists: without a CUDA device every compute
+ *    call returns MKF_CUDA_ERROR. */
+#ifndef MKF_H
+#define MKF_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { MKF_OK = 0, MKF_INVALID_ARG = -1, MKF_CUDA_ERROR = -2, MKF_WORKSPACE_TOO_SMALL = -3, MKF_UNSUPPORTED = -4 };
+
+/* per-track status bits */
+enum { MKF_PROP_UNREACHABLE = 1, /* next surface not reachable going forward with < half a turn (U5, U6) */
+       MKF_GRAZING = 2,          /* incidence too shallow: cos(alpha) < graze_cos_min (barrel), |cos theta| < 0.05 (disk) (U7) */
+       MKF_S_NOT_PD = 4,         /* residual covariance S = C(0:3,0:3)+V not positive definite (C6) */
+       MKF_NAN = 8,              /* non-finite value after an update */
+       MKF_STOPPED_ELOSS = 16,   /* energy exhausted by dE/dx (C5) */
+       MKF_TRUNCATED = 32 };     /* building: nothing with >= min_hits_keep hits; the seed itself is returned */
+
+enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total over plans */, MKF_MAX_CAND = 8 };
+
+/* workspace query ids */
+enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3 };
+
+typedef struct mkf_ctx mkf_ctx;       /* opaque: geometry, parameters, last error text */
+
+/* One detector layer of the lightweight geometry. */
+typedef struct { int kind;            /* 0 barrel cylinder, 1 disk */
+                 float pos;           /* r (barrel) or signed z (disk) [cm] */
+                 float lo, hi;        /* acceptance: barrel zmin,zmax ; disk rmin,rmax [cm] */
+                 float xx0;           /* thickness in radiation lengths at normal incidence */
+                 float eta_lo, eta_hi;/* hit pseudorapidity range spanned by the eta bins (U16) */ } mkf_layer;
+
+/* Geometry: all pointers HOST, copied by mkf_create. A "plan" is the ordered list of layers a seed is
+ * followed through (U17); plan p = plan_layers[plan_off[p] .. plan_off[p+1]). */
+typedef struct { int n_layers; const mkf_layer* layers; float bz; int n_phi_bins, n_eta_bins;
+                 int n_plans; const int* plan_off; const int* plan_layers; } mkf_geometry;
+
+typedef struct { float chi2_cut;      /* hit accepted iff chi2 < chi2_cut (30) */
+                 int max_cand;        /* live candidates kept per seed per layer, <= MKF_MAX_CAND (6 or 8) */
+                 int max_consec_miss; /* a candidate stops at this many consecutive missed layers (2) */
+                 int min_hits_keep;   /* stopped candidates with at least this many hits are preserved (4) */
+                 float score_hit, score_miss; /* score = score_hit*nhits - score_miss*nmiss - chi2 (U13) */
+                 float graze_cos_min; /* U7 (0.25) */
+                 int material_flags;  /* bit0 multiple scattering, bit1 dE/dx (C5) */
+                 float dup_frac;      /* duplicate if shared/min(nhits) > dup_frac (0.5) */ } mkf_params;
+
+/* Hits of n_events events, grouped by (event, layer): the hits of (ev, l) are the ids
+ * layer_off[ev*(n_layers+1)+l] .. layer_off[ev*(n_layers+1)+l+1]; ids are global (0..n_hits). */
+typedef struct { int n_events; int n_hits; const int* layer_off;
+                 const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */ } mkf_hits;
+
+/* The phi/eta-binned hit index (C8), written by mkf_build_hit_index, read by mkf_build_tracks.
+ * bin_off  [n_events*n_layers*n_phi*n_eta + 1]  exclusive prefix of hits per bin (bin = ie*n_phi + ip inside
+ *          segment (ev*n_layers + l)), last entry = n_hits;
+ * sorted_id[n_hits]  hit ids ordered by (segment, bin, id);
+ * vmax     [n_events*n_layers*2]  per segment: max over hits of the larger eigenvalue of the xy block of V, max V_zz;
+ * packed   [n_hits*12]  the hits in sorted order as 48-byte records {x,y,z,id(bits) | Vxx,Vxy,Vyy,Vxz | Vyz,Vzz,0,0}
+ *          (a derived copy so that a bin scan reads contiguous memory; may be NULL in mkf_build_hit_index, in
+ *          which case mkf_build_tracks gathers from the SoA arrays instead). */
+typedef struct { unsigned* bin_off; int* sorted_id; float* vmax; float* packed; } mkf_hit_index;
+
+typedef struct { int n; float* par; float* cov; signed char* q; } mkf_states;   /* par[6][n], cov[21][n], q[n] */
+
+/* ---- context ----------------------------------------------------------------------------------------- */
+/* Copies geometry and parameters. Errors: INVALID_ARG (null, n_layers<1), UNSUPPORTED (limits above). */
+int mkf_create(mkf_ctx** out, const mkf_geometry* geom, const mkf_params* params);
+void mkf_destroy(mkf_ctx*);
+const char* mkf_last_error(const mkf_ctx*);
+/* Bytes of device workspace the given call needs for these sizes (0 is a valid answer). */
+size_t mkf_workspace_bytes(const mkf_ctx*, int call_id, int n_events, int n_hits, int n_seeds);
+/* Number of kernel launches the library has enqueued through this context so far. */
+long long mkf_launch_count(const mkf_ctx*);
+/* Longest plan of the geometry (the leading dimension callers give track_hits / hit_ids). */
+int mkf_max_plan_len(const mkf_ctx*);
+
+/* ---- the four calls of BASELINE.json north_star -------------------------------------------------------- */
+/* a1 / C8 ("data preparation ... for each event"). Errors: INVALID_ARG, WORKSPACE_TOO_SMALL,
+ * UNSUPPORTED (n_hits >= 2^28), CUDA_ERROR. */
+int mkf_build_hit_index(mkf_ctx*, const mkf_hits*, mkf_hit_index* out, void* ws, size_t ws_bytes, void* stream);
+
+/* a11 / C7 ("Fitting simply applies the KF procedure to all hits identified during building").
+ * seeds: n states; plan[n]: plan id per track; track_hits[max_plan_len][n]: global hit id per plan step or <0.
+ * For every step with a hit: propagate (C2/C3) -> grazing test (U7) -> covariance transport (C4) -> material
+ * (C5) -> chi2 + update (C6). A track stops at the first failing step and keeps its last good state.
+ * out: states after the last fitted hit (phi wrapped to (-pi,pi]); chi2[n] total; nfit[n]; status[n]. */
+int mkf_fit(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed char* plan, const int* track_hits,
+            int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
+            void* ws, size_t ws_bytes, void* stream);
+
+/* a12 / C9. seeds: n states at their first hit; seed_event[n]; seed_hits[3][n] global hit ids;
+ * plan[n]. Each seed is first fitted through its own three hits, then followed through the rest of its plan.
+ * out: state of the winning candidate; chi2, score, nhits (incl. seed hits), nmiss;
+ * hit_ids[max_plan_len][n]: hit id | -1 missed layer | -2 layer not crossed; status. */
+int mkf_build_tracks(mkf_ctx*, const mkf_hits*, const mkf_hit_index*, const mkf_states* seeds,
+            const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
+            mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status,
+            void* ws, size_t ws_bytes, void* stream);
+
+/* a10 / C10 ("duplicate tracks ... explicitly removed in an additional processing step").
+ * track_off[n_events+1] (device): tracks of event ev are track_off[ev]..track_off[ev+1]; n = total tracks (the
+ * plane stride of hit_ids); n_hits = size of the hit-id space. keep[n] = 0/1, n_kept[n_events]. */
+int mkf_remove_duplicates(mkf_ctx*, int n_events, int n, int n_hits, const int* track_off, const int* hit_ids,
+            int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept,
+            void* ws, size_t ws_bytes, void* stream);
+
+/* ---- host-buffer entry points (end-to-end use: all pointers HOST; synchronous) ------------------------- */
+/* Same semantics as mkf_fit, every pointer (hits arrays included) in host memory. Device memory is taken from
+ * the CUDA stream-ordered pool and released before returning. h2d_bytes/d2h_bytes (may be NULL) receive the
+ * bytes copied each way. */
+int mkf_fit_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_host, const signed char* plan,
+            const int* track_hits, int max_plan_len, mkf_states* out_host, float* chi2, int* nfit, unsigned* status,
+            long long* h2d_bytes, long long* d2h_bytes);
+/* mkf_build_hit_index + mkf_build_tracks (+ mkf_remove_duplicates if keep != NULL; seeds must then be grouped
+ * by event in ascending order) on host buffers. */
+int mkf_build_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_host, const int* seed_event,
+            const int* seed_hits, const signed char* plan, int max_plan_len, mkf_states* out_host, float* chi2,
+            float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, unsigned char* keep,
+            long long* h2d_bytes, long long* d2h_bytes);
+#ifdef __cplusplus
+}
+#endif
+#endif

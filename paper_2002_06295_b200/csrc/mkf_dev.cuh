@@ -1,0 +1,93 @@
+// mkf_dev.cuh — device-side tables passed by value as kernel parameters, and SoA load/store helpers.
+#pragma once
+#include "kf_math.cuh"
+
+namespace mkf {
+
+constexpr int MAX_LAYERS = 64, MAX_PLANS = 8, MAX_PLAN_STEPS = 192, MAX_CAND = 8;
+
+// Geometry + parameters: ~2.1 KB, lives in the kernel parameter (constant) bank.
+struct GeomDev {
+  int n_layers, n_plans, n_phi, n_eta;
+  float bz;
+  int plan_off[MAX_PLANS + 1];
+  unsigned char plan_layers[MAX_PLAN_STEPS];
+  LayerDev layers[MAX_LAYERS];
+};
+
+struct ParamsDev {
+  float chi2_cut; int max_cand, max_consec_miss, min_hits_keep;
+  float score_hit, score_miss, graze_cos_min; int material_flags; float dup_frac;
+};
+
+struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; };
+
+MKF_HD void load_state(KState& S, const float* par, const float* cov, size_t n, size_t i) {
+  S.x = par[i]; S.y = par[n + i]; S.z = par[2 * n + i];
+  S.xl = 0.f; S.yl = 0.f; S.zl = 0.f;
+  S.ipt = par[3 * n + i]; S.phi = par[4 * n + i]; S.th = par[5 * n + i];
+#pragma unroll
+  for (int k = 0; k < 21; k++) S.c[k] = cov[(size_t)k * n + i];
+}
+
+MKF_HD void store_state(const KState& S, float* par, float* cov, size_t n, size_t i) {
+  par[i] = S.x + S.xl; par[n + i] = S.y + S.yl; par[2 * n + i] = S.z + S.zl;
+  par[3 * n + i] = S.ipt; par[4 * n + i] = wrap_phi(S.phi); par[5 * n + i] = S.th;
+#pragma unroll
+  for (int k = 0; k < 21; k++) cov[(size_t)k * n + i] = S.c[k];
+}
+
+MKF_HD void load_hit(Hit& H, const HitsDev& h, int id) {
+  const size_t nh = (size_t)h.n_hits;
+  H.x = h.x[id]; H.y = h.y[id]; H.z = h.z[id];
+#pragma unroll
+  for (int k = 0; k < 6; k++) H.v[k] = h.V[(size_t)k * nh + id];
+}
+
+// ---- fit of one track (C7) ------------------------------------------------------------------------------
+struct FitArgs {
+  HitsDev hits;
+  int n; const float* par; const float* cov; const signed char* q; const signed char* plan;
+  const int* track_hits; int max_plan_len;
+  float* par_out; float* cov_out; float* chi2; int* nfit; unsigned* status;
+};
+
+// The track keeps its last good state when a step fails. Failures found before the covariance is touched
+// (unreachable, grazing, energy exhausted) leave the state as it was; the two that can only be seen after the
+// update (S not positive definite, non-finite result) re-run the track from its seed up to the failing step.
+MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
+  const size_t n = (size_t)a.n;
+  const int pl = a.plan[i];
+  const int p0 = g.plan_off[pl];
+  int plen = g.plan_off[pl + 1] - p0;
+  if (plen > a.max_plan_len) plen = a.max_plan_len;
+  const float aq = -(float)a.q[i] * KAPPA * g.bz;
+  unsigned stat = 0;
+  int stop_at = plen;
+  KState S;
+  float c2tot; int nf;
+  for (int pass = 0; pass < 2; pass++) {
+    load_state(S, a.par, a.cov, n, (size_t)i);
+    c2tot = 0.f; nf = 0;
+    bool redo = false;
+    for (int s = 0; s < stop_at; s++) {
+      const int hid = a.track_hits[(size_t)s * n + i];
+      if (hid < 0) continue;
+      const LayerDev L = g.layers[g.plan_layers[p0 + s]];
+      Hit H; load_hit(H, a.hits, hid);
+      const unsigned rc = step_to_layer(S, L, aq, p.graze_cos_min, p.material_flags, false);
+      if (rc) { stat |= rc; break; }
+      SInv o; float c2;
+      const Frame f = frame_of(S, L.kind);
+      if (!chi2_of(S, f, H, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
+      kalman_update(S, f, o);
+      if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; stop_at = s; redo = true; break; }
+      c2tot += c2; nf++;
+    }
+    if (!redo) break;
+  }
+  store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+  a.chi2[i] = c2tot; a.nfit[i] = nf; a.status[i] = stat;
+}
+
+}  // namespace mkf
