@@ -1,0 +1,357 @@
+"""bench.py — KF layer-steps/s of mkf_fit on BASELINE.json configs[1] (4 M helices x 17 barrel layers), or built
+events/s of the building path on configs[2..4] (--workload build2|build3|build4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mkf|reference] [--workload fit|build2|build3|build4]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...
+
+One JSON line on rank 0 (contract in DESIGN.md §8). A "step" is one pass of the whole path over the workload with
+inputs resident in HBM; `e2e` is the same pass through the host-buffer C-ABI call (pinned host memory, copies
+timed). Events/tracks are independent, so N > 1 shards them with no collective (weak scaling: every rank owns a
+full-size workload generated from seed+rank).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+ALGO_FLOP_PER_LAYER_STEP = 1000.0        # DESIGN.md §6 (SURVEY.md §8 d): propagate 150 + transport 420 + material 90 + update 340
+ALGO_BYTES_PER_LAYER_STEP = 54.0         # hit 36 B + index 4 B + state in/out amortised 14 B
+FP32_LANES_PER_SM, N_SM = 128, 148
+
+
+def peaks():
+    p = dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+    try:
+        m = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        p.update(hbm_gbs=float(m["hbm_gbs"]), sm_max_mhz=float(m.get("sm_max_mhz", 1965.0)), source="measured")
+    except Exception:
+        pass
+    p["fp32_tflops"] = N_SM * FP32_LANES_PER_SM * 2 * p["sm_max_mhz"] * 1e6 / 1e12
+    return p
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------------------------------------------
+def make_fit_workload(seed, scale):
+    """configs[1]: generated as chunks of 1 M helices (bounded host memory), hits concatenated, ids offset."""
+    from paper_2002_06295_b200 import datagen
+    total = max(1, int(round(4000000 * scale)))
+    chunk = 1000000
+    parts, nh0 = [], 0
+    geom = prm = None
+    done = 0
+    k = 0
+    while done < total:
+        m = min(chunk, total - done)
+        ev, prm = datagen.config(1, scale=m / 4000000.0, seed=seed * 16 + k)
+        geom = ev["geom"]
+        s = ev["seeds"]
+        th = s["track_hits"].copy()
+        th[th >= 0] += nh0
+        parts.append((ev["hits"], dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], track_hits=th)))
+        nh0 += ev["hits"]["x"].shape[0]
+        done += m
+        k += 1
+    hits = dict(n_events=1, layer_off=np.zeros(len(geom["layers"]) + 1, np.int32),
+                x=np.concatenate([p[0]["x"] for p in parts]), y=np.concatenate([p[0]["y"] for p in parts]),
+                z=np.concatenate([p[0]["z"] for p in parts]), V=np.concatenate([p[0]["V"] for p in parts], axis=1))
+    seeds = {k2: np.ascontiguousarray(np.concatenate([p[1][k2] for p in parts], axis=-1)) for k2 in ("par", "cov", "q", "plan", "track_hits")}
+    return geom, prm, hits, seeds, parts[0]
+
+
+def make_build_workload(which, seed, scale):
+    from paper_2002_06295_b200 import datagen
+    ev, prm = datagen.config(which, scale=scale, seed=seed)
+    return ev, prm
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.samples, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc:
+            self.proc.terminate()
+        inside = [s for t, s in self.samples if t0 <= t <= t1] or [s for _, s in self.samples[-3:]]
+        mhz, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in inside:
+            f = [x.strip() for x in s.split(",")]
+            try:
+                mhz.append(float(f[0])); mx = max(mx, float(f[1]))
+            except Exception:
+                continue
+            for nme, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return dict(sm_mhz=float(np.median(mhz)) if mhz else None, sm_max_mhz=mx or None, reasons=sorted(reasons),
+                    samples=len(mhz))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline of the mkf arm, and the whole --impl reference arm)
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_fit_rate(geom, prm, hits, seeds, n_tracks, repeat=1):
+    from oracle import mkfo
+    o = mkfo.Oracle(geom, prm)
+    sl = slice(0, n_tracks)
+    args = (hits, seeds["par"][:, sl], seeds["cov"][:, sl], seeds["q"][sl], seeds["plan"][sl], np.ascontiguousarray(seeds["track_hits"][:, sl]))
+    t = time.perf_counter()
+    for _ in range(repeat):
+        r = o.fit(*args)
+    dt = (time.perf_counter() - t) / repeat
+    return float(r["nfit"].sum()) / dt, dt, o.num_threads(), int(r["nfit"].sum())
+
+
+def oracle_build_rate(ev, prm, n_events, dedup):
+    from oracle import mkfo
+    s = ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], prm)
+    nl = len(ev["geom"]["layers"])
+    h = ev["hits"]
+    lo = h["layer_off"].reshape(-1, nl + 1)
+    nh = int(lo[n_events - 1, nl])
+    sub = dict(n_events=n_events, layer_off=np.ascontiguousarray(lo[:n_events]).reshape(-1), x=h["x"][:nh], y=h["y"][:nh], z=h["z"][:nh],
+               V=np.ascontiguousarray(h["V"][:, :nh]))
+    m = s["event"] < n_events
+    t = time.perf_counter()
+    idx = o.build_hit_index(sub)
+    r = o.build_tracks(sub, idx, s["par"][:, m], s["cov"][:, m], s["q"][m], s["event"][m], np.ascontiguousarray(s["hits"][:, m]), s["plan"][m])
+    if dedup:
+        counts = np.bincount(s["event"][m], minlength=n_events)
+        o.remove_duplicates(np.concatenate([[0], np.cumsum(counts)]).astype(np.int32), r["hit_ids"], r["nhits"], r["score"].astype(np.float32))
+    dt = time.perf_counter() - t
+    return n_events / dt, dt, o.num_threads()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="mkf", choices=["mkf", "reference"])
+    ap.add_argument("--workload", default="fit", choices=["fit", "build2", "build3", "build4"])
+    ap.add_argument("--scale", type=float, default=1.0, help="shrinks the workload (testing only; the JSON says so)")
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    a = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    warm = max(a.warmup, 3)
+    is_fit = a.workload == "fit"
+    metric = "KF layer-steps/s (propagate+update)" if is_fit else "built events/s"
+    unit = "layer-steps/s" if is_fit else "events/s"
+    names = dict(fit="configs[1]: track fit, 4M helices x 17 barrel layers, MS + dE/dx, seeds from 3 hits, cov x100",
+                 build2="configs[2]: building, barrel, 100 events x 1000 tracks + 20k noise hits, top 6",
+                 build3="configs[3]: building, barrel+endcap, 200 events x 1500 seeds, ~80k hits/event",
+                 build4="configs[4]: batched building + duplicate removal, 64 events x 6000 seeds, ~300k hits/event, top 8")
+    cfg = dict(workload=names[a.workload], scale=a.scale, l2="inputs larger than L2 (no flush needed)", seed=a.seed)
+
+    # ---- reference arm: the oracle on host cores, bounded sample ------------------------------------------------
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        if is_fit:
+            n_s = max(1, int(round(200000 * min(1.0, a.scale * 20))))
+            geom, prm, hits, seeds, _ = make_fit_workload(a.seed, n_s / 4000000.0)
+            rates = []
+            for k in range(warm + a.steps):
+                rate, dt, cores, steps = oracle_fit_rate(geom, prm, hits, seeds, n_s)
+                if k >= warm:
+                    rates.append((rate, dt))
+            sample = "first %d helices of the workload per step (%d layer-steps)" % (n_s, steps)
+        else:
+            which = int(a.workload[-1])
+            nev_full = {2: 100, 3: 200, 4: 64}[which]
+            n_ev = max(1, min(4, int(round(nev_full * a.scale))))
+            ev, prm = make_build_workload(which, a.seed, n_ev / nev_full)
+            rates = []
+            for k in range(warm + a.steps):
+                rate, dt, cores = oracle_build_rate(ev, prm, n_ev, which == 4)
+                if k >= warm:
+                    rates.append((rate, dt))
+            sample = "%d events of the workload per step" % n_ev
+        ms = 1e3 * float(np.mean([d for _, d in rates]))
+        v = float(np.mean([r for r, _ in rates]))
+        print(json.dumps(dict(metric=metric, value=v, unit=unit, n_gpus=a.gpus, steps=a.steps, warmup=warm, ms_per_step=ms,
+                              higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", config=cfg,
+                              impl="reference", cpu_baseline=dict(value=v, unit=unit, cores=cores, kind="oracle", sample=sample),
+                              e2e=dict(value=v, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)))
+        return
+
+    # ---- mkf arm ------------------------------------------------------------------------------------------------
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl mkf needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    from paper_2002_06295_b200 import binding as B
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pk = peaks()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if is_fit:
+        geom, prm, hits, seeds, _ = make_fit_workload(a.seed + rank, a.scale)
+        ctx = B.Context(geom, prm)
+        dh = B.hits_to_device(hits)
+        ds = B.to_device(seeds, ["par", "cov", "q", "plan", "track_hits"])
+        n = seeds["par"].shape[1]
+        out = B.alloc_fit_out(n)
+
+        def step():
+            ctx.fit(dh, ds, ds["plan"], ds["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+
+        def units():
+            return float(out["nfit"].sum().item())
+
+        def e2e_step():
+            r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"])
+            return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
+    else:
+        which = int(a.workload[-1])
+        ev, prm = make_build_workload(which, a.seed + rank, a.scale)
+        geom, hits, s = ev["geom"], ev["hits"], ev["seeds"]
+        seeds = dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"])
+        ctx = B.Context(geom, prm)
+        dh = B.hits_to_device(hits)
+        nh, nev, n = hits["x"].shape[0], hits["n_events"], s["par"].shape[1]
+        idx, ws = B.alloc_hit_index(ctx, nev, nh)
+        ds = B.to_device(seeds, ["par", "cov", "q", "plan", "event", "hits"])
+        out = B.alloc_build_out(n, ctx.max_plan_len)
+        dedup = which == 4
+        if dedup:
+            counts = np.bincount(s["event"], minlength=nev)
+            toff = torch.from_numpy(np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)).cuda()
+            keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+            nk = torch.empty(nev, dtype=torch.int32, device="cuda")
+            ws2 = torch.empty(max(ctx.workspace_bytes(B.CALL_REMOVE_DUPLICATES, nev, nh, n), 256), dtype=torch.uint8, device="cuda")
+
+        def step():
+            ctx.build_hit_index(dh, idx, ws)
+            ctx.build_tracks(dh, idx, ds, ds["event"], ds["hits"], ds["plan"], out, out["chi2"], out["score"], out["nhits"],
+                             out["nmiss"], out["hit_ids"], out["status"])
+            if dedup:
+                ctx.remove_duplicates(nh, toff, out["hit_ids"], out["nhits"], out["score"], keep, nk, ws2)
+
+        def units():
+            return float(nev)
+
+        def e2e_step():
+            r = ctx.build_host(hits_p, seeds_p, seeds_p["event"], seeds_p["hits"], seeds_p["plan"], dedup=dedup)
+            return float(nev), r["h2d_bytes"], r["d2h_bytes"]
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    for _ in range(warm):
+        step()
+    barrier()
+    l0 = ctx.launch_count()
+    t0 = time.time()
+    ev0.record()
+    for _ in range(a.steps):
+        step()
+    ev1.record()
+    barrier()
+    t1 = time.time()
+    launches = ctx.launch_count() - l0
+    ms_total = ev0.elapsed_time(ev1)
+    u = units()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    tot = torch.tensor([ms_total, u], dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = tot.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = tot.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms_total, u_all = float(mx[0]), float(sm[1])
+    else:
+        u_all = u
+    ms_step = ms_total / a.steps
+    value = u_all / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer C-ABI call (pinned host memory) --------------------------------------
+    def pin(d, keys):
+        return {k: torch.from_numpy(np.ascontiguousarray(d[k])).pin_memory().numpy() for k in keys}
+    hits_p = pin(hits, ["layer_off", "x", "y", "z", "V"]); hits_p["n_events"] = hits["n_events"]
+    seeds_p = pin(seeds, list(seeds.keys()))
+    e2e_step()                                            # warm the stream-ordered pool
+    barrier()
+    te = time.perf_counter()
+    for _ in range(a.e2e_steps):
+        eu, h2d, d2h = e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - te) / a.e2e_steps
+    ee = torch.tensor([e2e_s, eu], dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = ee.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = ee.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        e2e_s, eu = float(mx[0]), float(sm[1])
+    e2e = dict(value=eu / e2e_s, unit=unit, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h), steps=a.e2e_steps,
+               ms_per_step=1e3 * e2e_s, host_memory="pinned")
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel ----------------------------------------------------------------------------
+    if is_fit:
+        steps_per_launch = u                                  # one launch = one step = all layer-steps of this rank
+        t_launch = ms_total / a.steps * 1e-3
+        ach = ALGO_FLOP_PER_LAYER_STEP * steps_per_launch / t_launch / 1e12
+        roof = dict(bound="alu", kernel="mkf_fit_kernel", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
+                    traffic=None, peak_source="148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (%s max clock)" % (pk["sm_max_mhz"], pk["source"]),
+                    algorithmic_flop_per_layer_step=ALGO_FLOP_PER_LAYER_STEP,
+                    hbm=dict(achieved=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
+                             frac=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9 / pk["hbm_gbs"]))
+    else:
+        roof = dict(bound="hbm", kernel="mkf_build_kernel", achieved=None, peak=pk["hbm_gbs"], unit="GB/s", frac=None, traffic=None,
+                    note="building is reported, not held to the 50% bar (BASELINE.json north_star); see DESIGN.md §6")
+    # ---- cpu baseline: the oracle as it stands on a bounded sample ---------------------------------------------------
+    cpu = None
+    if not a.no_cpu_baseline:
+        if is_fit:
+            n_s = min(n, 1000000)
+            rate, dt, cores, st = oracle_fit_rate(geom, prm, hits, seeds, n_s)
+            cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d helices of the workload (%d layer-steps, %.1f s)" % (n_s, st, dt))
+        else:
+            n_ev = min(nev, 4)
+            rate, dt, cores = oracle_build_rate(ev, prm, n_ev, dedup)
+            cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d events of the workload (%.1f s)" % (n_ev, dt))
+    print(json.dumps(dict(metric=metric, value=value, unit=unit, n_gpus=world, steps=a.steps, warmup=warm, ms_per_step=ms_step,
+                          higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic", config=cfg,
+                          clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, cpu_baseline=cpu, impl="mkf",
+                          units_per_step=u_all)))
+
+
+if __name__ == "__main__":
+    main()

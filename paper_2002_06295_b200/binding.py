@@ -1,0 +1,281 @@
+"""Thin ctypes binding of libmkf.so (include/mkf.h): argument marshalling only — every step runs in the CUDA kernels.
+
+Device calls take torch CUDA tensors (caller-owned; PyTorch is used for device memory and streams only) and enqueue
+on torch's current stream without synchronising. Host calls (`fit_host`, `build_host`) take numpy arrays or CPU
+tensors. There is no CPU fallback: a missing library or a missing CUDA device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+OK, INVALID_ARG, CUDA_ERROR, WORKSPACE_TOO_SMALL, UNSUPPORTED = 0, -1, -2, -3, -4
+PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8, 16, 32
+CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
+
+EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
+           "mkf_build_hit_index", "mkf_fit", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host"]
+
+
+class Layer(C.Structure):
+    _fields_ = [("kind", C.c_int), ("pos", C.c_float), ("lo", C.c_float), ("hi", C.c_float), ("xx0", C.c_float),
+                ("eta_lo", C.c_float), ("eta_hi", C.c_float)]
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("layers", C.POINTER(Layer)), ("bz", C.c_float), ("n_phi_bins", C.c_int),
+                ("n_eta_bins", C.c_int), ("n_plans", C.c_int), ("plan_off", C.POINTER(C.c_int)),
+                ("plan_layers", C.POINTER(C.c_int))]
+
+
+class Params(C.Structure):
+    _fields_ = [("chi2_cut", C.c_float), ("max_cand", C.c_int), ("max_consec_miss", C.c_int), ("min_hits_keep", C.c_int),
+                ("score_hit", C.c_float), ("score_miss", C.c_float), ("graze_cos_min", C.c_float),
+                ("material_flags", C.c_int), ("dup_frac", C.c_float)]
+
+
+class Hits(C.Structure):
+    _fields_ = [("n_events", C.c_int), ("n_hits", C.c_int), ("layer_off", C.c_void_p), ("x", C.c_void_p),
+                ("y", C.c_void_p), ("z", C.c_void_p), ("V", C.c_void_p)]
+
+
+class HitIndex(C.Structure):
+    _fields_ = [("bin_off", C.c_void_p), ("sorted_id", C.c_void_p), ("vmax", C.c_void_p), ("packed", C.c_void_p)]
+
+
+class States(C.Structure):
+    _fields_ = [("n", C.c_int), ("par", C.c_void_p), ("cov", C.c_void_p), ("q", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads (building first if needed) libmkf.so. Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB if os.path.exists(_build.LIB) and os.environ.get("MKF_NO_REBUILD") else _build.build()
+        L = C.CDLL(path)
+        L.mkf_last_error.restype = C.c_char_p
+        L.mkf_last_error.argtypes = [C.c_void_p]
+        L.mkf_workspace_bytes.restype = C.c_size_t
+        L.mkf_workspace_bytes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.mkf_launch_count.restype = C.c_longlong
+        L.mkf_launch_count.argtypes = [C.c_void_p]
+        L.mkf_max_plan_len.argtypes = [C.c_void_p]
+        L.mkf_destroy.restype = None
+        L.mkf_destroy.argtypes = [C.c_void_p]
+        L.mkf_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(Geometry), C.POINTER(Params)]
+        vp, sz, i = C.c_void_p, C.c_size_t, C.c_int
+        L.mkf_build_hit_index.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), vp, sz, vp]
+        L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
+        L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
+                                       C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.mkf_remove_duplicates.argtypes = [vp, i, i, i, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
+        ll = C.POINTER(C.c_longlong)
+        L.mkf_fit_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, ll, ll]
+        L.mkf_build_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, vp, i, C.POINTER(States), vp, vp,
+                                     vp, vp, vp, vp, vp, ll, ll]
+        _lib = L
+    return _lib
+
+
+class MkfError(RuntimeError):
+    pass
+
+
+def _dev(t, dtype):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    return t.data_ptr()
+
+
+def _host(a, dtype):
+    if isinstance(a, torch.Tensor):
+        a = a.numpy()
+    if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags["C_CONTIGUOUS"]):
+        raise TypeError("expected a C-contiguous numpy array of dtype %s" % dtype)
+    return a.ctypes.data
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Context:
+    """mkf_ctx: geometry + parameters (dicts as made by datagen). Methods carry the names of the C calls."""
+
+    def __init__(self, geom, params):
+        self.L = lib()
+        lay = geom["layers"]
+        self._layers = (Layer * len(lay))(*[Layer(int(l["kind"]), float(l["pos"]), float(l["lo"]), float(l["hi"]),
+                                                 float(l["xx0"]), float(l["eta_lo"]), float(l["eta_hi"])) for l in lay])
+        self._plan_off = np.ascontiguousarray(geom["plan_off"], np.int32)
+        self._plan_layers = np.ascontiguousarray(geom["plan_layers"], np.int32)
+        g = Geometry(len(lay), self._layers, float(geom["bz"]), int(geom["n_phi_bins"]), int(geom["n_eta_bins"]),
+                     len(self._plan_off) - 1, self._plan_off.ctypes.data_as(C.POINTER(C.c_int)),
+                     self._plan_layers.ctypes.data_as(C.POINTER(C.c_int)))
+        p = Params(float(params["chi2_cut"]), int(params["max_cand"]), int(params["max_consec_miss"]),
+                   int(params["min_hits_keep"]), float(params["score_hit"]), float(params["score_miss"]),
+                   float(params["graze_cos_min"]), int(params["material_flags"]), float(params["dup_frac"]))
+        h = C.c_void_p()
+        rc = self.L.mkf_create(C.byref(h), C.byref(g), C.byref(p))
+        if rc != OK:
+            raise MkfError("mkf_create failed: %d" % rc)
+        self.h = h
+        self.n_layers = len(lay)
+        self.n_bins = int(geom["n_phi_bins"]) * int(geom["n_eta_bins"])
+        self.max_plan_len = int(self.L.mkf_max_plan_len(self.h))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.mkf_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != OK:
+            raise MkfError("%s failed (%d): %s" % (what, rc, self.L.mkf_last_error(self.h).decode()))
+
+    def launch_count(self):
+        return int(self.L.mkf_launch_count(self.h))
+
+    def workspace_bytes(self, call_id, n_events, n_hits, n_seeds):
+        return int(self.L.mkf_workspace_bytes(self.h, call_id, n_events, n_hits, n_seeds))
+
+    # ---- marshalling helpers ------------------------------------------------------------------------------
+    @staticmethod
+    def hits_struct(h, ptr, i32=torch.int32, f32=torch.float32):
+        return Hits(int(h["n_events"]), int(h["x"].shape[0]), ptr(h["layer_off"], i32), ptr(h["x"], f32), ptr(h["y"], f32),
+                    ptr(h["z"], f32), ptr(h["V"], f32))
+
+    # ---- the four calls -----------------------------------------------------------------------------------
+    def build_hit_index(self, hits, out, ws):
+        """hits: dict of CUDA tensors (layer_off int32, x,y,z float32 [n], V float32 [6,n]); out: dict(bin_off int32
+        [n_events*n_layers*n_bins+1] (unsigned offsets), sorted_id int32 [n], vmax float32 [n_events*n_layers*2],
+        packed float32 [n*12] or None); ws: uint8 CUDA tensor."""
+        hs = self.hits_struct(hits, _dev)
+        packed = out.get("packed")
+        idx = HitIndex(_dev(out["bin_off"], torch.int32), _dev(out["sorted_id"], torch.int32), _dev(out["vmax"], torch.float32),
+                       _dev(packed, torch.float32) if packed is not None else None)
+        rc = self.L.mkf_build_hit_index(self.h, C.byref(hs), C.byref(idx), ws.data_ptr() if ws is not None else None,
+                                        ws.numel() if ws is not None else 0, _stream())
+        self._check(rc, "mkf_build_hit_index")
+
+    def fit(self, hits, seeds, plan, track_hits, out, chi2, nfit, status):
+        """seeds/out: dict(par float32 [6,n], cov float32 [21,n], q int8 [n]); plan int8 [n]; track_hits int32 [mpl,n]."""
+        hs = self.hits_struct(hits, _dev)
+        n = int(seeds["par"].shape[1])
+        s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
+        o = States(n, _dev(out["par"], torch.float32), _dev(out["cov"], torch.float32), _dev(seeds["q"], torch.int8))
+        rc = self.L.mkf_fit(self.h, C.byref(hs), C.byref(s), _dev(plan, torch.int8), _dev(track_hits, torch.int32),
+                            int(track_hits.shape[0]), C.byref(o), _dev(chi2, torch.float32), _dev(nfit, torch.int32),
+                            _dev(status, torch.int32), None, 0, _stream())
+        self._check(rc, "mkf_fit")
+
+    def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status):
+        hs = self.hits_struct(hits, _dev)
+        packed = idx.get("packed")
+        ix = HitIndex(_dev(idx["bin_off"], torch.int32), _dev(idx["sorted_id"], torch.int32), _dev(idx["vmax"], torch.float32),
+                      _dev(packed, torch.float32) if packed is not None else None)
+        n = int(seeds["par"].shape[1])
+        s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
+        o = States(n, _dev(out["par"], torch.float32), _dev(out["cov"], torch.float32), _dev(seeds["q"], torch.int8))
+        rc = self.L.mkf_build_tracks(self.h, C.byref(hs), C.byref(ix), C.byref(s), _dev(seed_event, torch.int32),
+                                     _dev(seed_hits, torch.int32), _dev(plan, torch.int8), int(hit_ids.shape[0]), C.byref(o),
+                                     _dev(chi2, torch.float32), _dev(score, torch.float32), _dev(nhits, torch.int32),
+                                     _dev(nmiss, torch.int32), _dev(hit_ids, torch.int32), _dev(status, torch.int32),
+                                     None, 0, _stream())
+        self._check(rc, "mkf_build_tracks")
+
+    def remove_duplicates(self, n_hits, track_off, hit_ids, nhits, score, keep, n_kept, ws):
+        n_events = int(track_off.shape[0]) - 1
+        rc = self.L.mkf_remove_duplicates(self.h, n_events, int(hit_ids.shape[1]), int(n_hits), _dev(track_off, torch.int32),
+                                          _dev(hit_ids, torch.int32), int(hit_ids.shape[0]), _dev(nhits, torch.int32),
+                                          _dev(score, torch.float32), _dev(keep, torch.uint8), _dev(n_kept, torch.int32),
+                                          ws.data_ptr(), ws.numel(), _stream())
+        self._check(rc, "mkf_remove_duplicates")
+
+    # ---- host-buffer entry points -------------------------------------------------------------------------
+    def fit_host(self, hits, seeds, plan, track_hits):
+        """All arguments numpy / CPU tensors; returns dict of numpy arrays plus the bytes copied each way."""
+        f32, i32, i8 = np.float32, np.int32, np.int8
+        hs = self.hits_struct(hits, _host, i32, f32)
+        n = int(seeds["par"].shape[1])
+        out = dict(par=np.empty((6, n), f32), cov=np.empty((21, n), f32), chi2=np.empty(n, f32), nfit=np.empty(n, i32),
+                   status=np.empty(n, np.uint32))
+        s = States(n, _host(seeds["par"], f32), _host(seeds["cov"], f32), _host(seeds["q"], i8))
+        o = States(n, out["par"].ctypes.data, out["cov"].ctypes.data, _host(seeds["q"], i8))
+        h2d, d2h = C.c_longlong(0), C.c_longlong(0)
+        rc = self.L.mkf_fit_host(self.h, C.byref(hs), C.byref(s), _host(plan, i8), _host(track_hits, i32),
+                                 int(track_hits.shape[0]), C.byref(o), out["chi2"].ctypes.data, out["nfit"].ctypes.data,
+                                 out["status"].ctypes.data, C.byref(h2d), C.byref(d2h))
+        self._check(rc, "mkf_fit_host")
+        out["h2d_bytes"], out["d2h_bytes"] = h2d.value, d2h.value
+        return out
+
+    def build_host(self, hits, seeds, seed_event, seed_hits, plan, dedup=False):
+        f32, i32, i8 = np.float32, np.int32, np.int8
+        hs = self.hits_struct(hits, _host, i32, f32)
+        n = int(seeds["par"].shape[1])
+        mpl = self.max_plan_len
+        out = dict(par=np.empty((6, n), f32), cov=np.empty((21, n), f32), chi2=np.empty(n, f32), score=np.empty(n, f32),
+                   nhits=np.empty(n, i32), nmiss=np.empty(n, i32), hit_ids=np.empty((mpl, n), i32),
+                   status=np.empty(n, np.uint32))
+        keep = np.empty(n, np.uint8) if dedup else None
+        s = States(n, _host(seeds["par"], f32), _host(seeds["cov"], f32), _host(seeds["q"], i8))
+        o = States(n, out["par"].ctypes.data, out["cov"].ctypes.data, _host(seeds["q"], i8))
+        h2d, d2h = C.c_longlong(0), C.c_longlong(0)
+        rc = self.L.mkf_build_host(self.h, C.byref(hs), C.byref(s), _host(seed_event, i32), _host(seed_hits, i32),
+                                   _host(plan, i8), mpl, C.byref(o), out["chi2"].ctypes.data, out["score"].ctypes.data,
+                                   out["nhits"].ctypes.data, out["nmiss"].ctypes.data, out["hit_ids"].ctypes.data,
+                                   out["status"].ctypes.data, keep.ctypes.data if dedup else None, C.byref(h2d), C.byref(d2h))
+        self._check(rc, "mkf_build_host")
+        if dedup:
+            out["keep"] = keep
+        out["h2d_bytes"], out["d2h_bytes"] = h2d.value, d2h.value
+        return out
+
+
+# ---- convenience: allocate outputs on the device (still marshalling only) ---------------------------------------
+def to_device(d, keys, device="cuda"):
+    """Copies the named numpy arrays of dict d to CUDA tensors (int32/float32/int8 kept)."""
+    return {k: torch.from_numpy(np.ascontiguousarray(d[k])).to(device) for k in keys}
+
+
+def hits_to_device(hits, device="cuda"):
+    h = to_device(hits, ["layer_off", "x", "y", "z", "V"], device)
+    h["n_events"] = int(hits["n_events"])
+    return h
+
+
+def alloc_hit_index(ctx, n_events, n_hits, packed=True, device="cuda"):
+    nseg = n_events * ctx.n_layers
+    out = dict(bin_off=torch.empty(nseg * ctx.n_bins + 1, dtype=torch.int32, device=device),
+               sorted_id=torch.empty(n_hits, dtype=torch.int32, device=device),
+               vmax=torch.empty(nseg * 2, dtype=torch.float32, device=device),
+               packed=torch.empty(n_hits * 12, dtype=torch.float32, device=device) if packed else None)
+    ws = torch.empty(max(ctx.workspace_bytes(CALL_BUILD_HIT_INDEX, n_events, n_hits, 0), 256), dtype=torch.uint8, device=device)
+    return out, ws
+
+
+def alloc_fit_out(n, device="cuda"):
+    return dict(par=torch.empty((6, n), dtype=torch.float32, device=device), cov=torch.empty((21, n), dtype=torch.float32, device=device),
+                chi2=torch.empty(n, dtype=torch.float32, device=device), nfit=torch.empty(n, dtype=torch.int32, device=device),
+                status=torch.empty(n, dtype=torch.int32, device=device))
+
+
+def alloc_build_out(n, mpl, device="cuda"):
+    f32, i32 = torch.float32, torch.int32
+    return dict(par=torch.empty((6, n), dtype=f32, device=device), cov=torch.empty((21, n), dtype=f32, device=device),
+                chi2=torch.empty(n, dtype=f32, device=device), score=torch.empty(n, dtype=f32, device=device),
+                nhits=torch.empty(n, dtype=i32, device=device), nmiss=torch.empty(n, dtype=i32, device=device),
+                hit_ids=torch.empty((mpl, n), dtype=i32, device=device), status=torch.empty(n, dtype=i32, device=device))

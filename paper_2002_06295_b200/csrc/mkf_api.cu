@@ -1,0 +1,76 @@
+// mkf_api.cu — context management and the fit entry point of libmkf.so (see include/mkf.h).
+#include "mkf_ctx.h"
+
+using namespace mkf;
+
+extern "C" int mkf_create(mkf_ctx** out, const mkf_geometry* geom, const mkf_params* prm) {
+  if (!out || !geom || !prm || !geom->layers || !geom->plan_off || !geom->plan_layers) return MKF_INVALID_ARG;
+  if (geom->n_layers < 1 || geom->n_plans < 1 || geom->n_phi_bins < 1 || geom->n_eta_bins < 1) return MKF_INVALID_ARG;
+  if (geom->n_layers > MAX_LAYERS || geom->n_plans > MAX_PLANS) return MKF_UNSUPPORTED;
+  if (geom->plan_off[0] != 0 || geom->plan_off[geom->n_plans] > MAX_PLAN_STEPS) return MKF_UNSUPPORTED;
+  if (prm->max_cand < 1 || prm->max_cand > MAX_CAND) return MKF_UNSUPPORTED;
+  mkf_ctx* c = new mkf_ctx();
+  memset(c, 0, sizeof(*c));
+  c->g.n_layers = geom->n_layers; c->g.n_plans = geom->n_plans;
+  c->g.n_phi = geom->n_phi_bins; c->g.n_eta = geom->n_eta_bins; c->g.bz = geom->bz;
+  for (int l = 0; l < geom->n_layers; l++) {
+    const mkf_layer& s = geom->layers[l];
+    LayerDev& d = c->g.layers[l];
+    d.kind = s.kind; d.pos = s.pos; d.lo = s.lo; d.hi = s.hi; d.xx0 = s.xx0; d.eta_lo = s.eta_lo; d.eta_hi = s.eta_hi;
+    if ((s.kind != 0 && s.kind != 1) || !(s.eta_hi > s.eta_lo) || (s.kind == 0 && !(s.pos > 0.f))) { delete c; return MKF_INVALID_ARG; }
+  }
+  int mpl = 0;
+  for (int p = 0; p <= geom->n_plans; p++) c->g.plan_off[p] = geom->plan_off[p];
+  for (int p = 0; p < geom->n_plans; p++) {
+    const int len = geom->plan_off[p + 1] - geom->plan_off[p];
+    if (len < 0) { delete c; return MKF_INVALID_ARG; }
+    if (len > mpl) mpl = len;
+  }
+  for (int k = 0; k < geom->plan_off[geom->n_plans]; k++) {
+    const int l = geom->plan_layers[k];
+    if (l < 0 || l >= geom->n_layers) { delete c; return MKF_INVALID_ARG; }
+    c->g.plan_layers[k] = (unsigned char)l;
+  }
+  c->max_plan_len = mpl;
+  c->p.chi2_cut = prm->chi2_cut; c->p.max_cand = prm->max_cand; c->p.max_consec_miss = prm->max_consec_miss;
+  c->p.min_hits_keep = prm->min_hits_keep; c->p.score_hit = prm->score_hit; c->p.score_miss = prm->score_miss;
+  c->p.graze_cos_min = prm->graze_cos_min; c->p.material_flags = prm->material_flags; c->p.dup_frac = prm->dup_frac;
+  *out = c;
+  return MKF_OK;
+}
+
+extern "C" void mkf_destroy(mkf_ctx* c) { delete c; }
+extern "C" const char* mkf_last_error(const mkf_ctx* c) { return c ? c->err : "null context"; }
+extern "C" long long mkf_launch_count(const mkf_ctx* c) { return c ? c->launches : 0; }
+extern "C" int mkf_max_plan_len(const mkf_ctx* c) { return c ? c->max_plan_len : 0; }
+
+// ---- fit (a11 / C7): one thread per track, state and covariance in registers for the whole layer loop ----
+constexpr int FIT_BLOCK = 128;
+
+__global__ void __launch_bounds__(FIT_BLOCK) mkf_fit_kernel(const __grid_constant__ GeomDev g,
+                                                            const __grid_constant__ ParamsDev p,
+                                                            const __grid_constant__ FitArgs a) {
+  const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
+  if (i < a.n) fit_one(g, p, a, i);
+}
+
+extern "C" int mkf_fit(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
+                       const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit,
+                       unsigned* status, void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || !seeds || !out || !plan || !track_hits || !chi2 || !nfit || !status) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
+  if (seeds->n < 0 || out->n != seeds->n || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_fit: bad sizes");
+  if (seeds->n == 0) return MKF_OK;
+  if (!h->x || !h->y || !h->z || !h->V || !seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov)
+    return fail(c, MKF_INVALID_ARG, "mkf_fit: null array");
+  FitArgs a;
+  a.hits = hits_dev(h);
+  a.n = seeds->n; a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.plan = plan;
+  a.track_hits = track_hits; a.max_plan_len = max_plan_len;
+  a.par_out = out->par; a.cov_out = out->cov; a.chi2 = chi2; a.nfit = nfit; a.status = status;
+  const int grid = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
+  mkf_fit_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
+  MKF_LAUNCHED(c, "mkf_fit_kernel");
+  return MKF_OK;
+}

@@ -1,0 +1,175 @@
+// mkf_hit_index.cu — a1 / C8: per (event, layer) phi/eta-binned hit index ("data preparation").
+//
+// Counting sort over the global bin space (segment = event*n_layers + layer, bin = ie*n_phi + ip):
+//   1. hi_key_count : one CTA per segment; bin key per hit in fp64 (U12), count per bin (global atomics on a
+//                     mostly empty table), per-segment max hit variances (block reduction, no atomics);
+//   2. hi_scan_*    : exclusive prefix sum of the counts (reduce / scan-of-partials / downsweep);
+//   3. hi_place     : scatter hit ids to their bins (atomic cursor);
+//   4. hi_sort_bins : each bin's ids sorted ascending -> the order is the unique stable order (C8) whatever
+//                     order the atomics ran in;
+//   5. hi_pack      : 48-byte records of the hits in sorted order, so that a bin scan reads contiguous memory.
+// HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
+#include "mkf_ctx.h"
+#include "mkf_scan.cuh"
+
+using namespace mkf;
+
+namespace {
+
+constexpr int HI_BLOCK = 256;
+
+struct HiArgs {
+  HitsDev hits; int n_layers, n_phi, n_eta;
+  int* key;            // [n_hits] bin inside the segment
+  unsigned* cnt;       // [n_bins_total] counts, later the scatter cursors
+  unsigned* bin_off; int* sorted_id; float* vmax; float4* packed;
+};
+
+__device__ __forceinline__ int phi_bin_d(double phi, int nphi) {
+  const double PI = 3.14159265358979323846;
+  int ip = (int)floor((phi + PI) * (double)nphi / (2.0 * PI));
+  if (ip >= nphi) ip -= nphi;
+  if (ip < 0) ip = 0;
+  return ip;
+}
+__device__ __forceinline__ int eta_bin_d(double eta, double lo, double hi, int neta) {
+  int ie = (int)floor((eta - lo) * (double)neta / (hi - lo));
+  if (ie < 0) ie = 0;
+  if (ie > neta - 1) ie = neta - 1;
+  return ie;
+}
+
+__global__ void __launch_bounds__(HI_BLOCK) hi_key_count(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
+  const int seg = blockIdx.x;
+  const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
+  const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
+  const double elo = (double)g.layers[l].eta_lo, ehi = (double)g.layers[l].eta_hi;
+  const size_t nh = (size_t)a.hits.n_hits;
+  const size_t bin0 = (size_t)seg * (size_t)(a.n_phi * a.n_eta);
+  float vxy = 0.f, vzz = 0.f;
+  for (int i = b + threadIdx.x; i < e; i += HI_BLOCK) {
+    const double x = (double)a.hits.x[i], y = (double)a.hits.y[i], z = (double)a.hits.z[i];
+    const int ip = phi_bin_d(atan2(y, x), a.n_phi);
+    const int ie = eta_bin_d(asinh(z / sqrt(x * x + y * y)), elo, ehi, a.n_eta);
+    const int key = ie * a.n_phi + ip;
+    a.key[i] = key;
+    atomicAdd(&a.cnt[bin0 + key], 1u);
+    // larger eigenvalue of the xy block of V in round-to-nearest fp32 without contraction (bit-exact with C8)
+    const float vxx = a.hits.V[i], vxyv = a.hits.V[nh + i], vyy = a.hits.V[2 * nh + i];
+    const float hs = __fmul_rn(0.5f, __fadd_rn(vxx, vyy)), hd = __fmul_rn(0.5f, __fsub_rn(vxx, vyy));
+    const float ev1 = __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(vxyv, vxyv))));
+    vxy = fmaxf(vxy, ev1);
+    vzz = fmaxf(vzz, a.hits.V[5 * nh + i]);
+  }
+  __shared__ float s_xy[HI_BLOCK / 32], s_zz[HI_BLOCK / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    vxy = fmaxf(vxy, __shfl_xor_sync(0xffffffffu, vxy, o));
+    vzz = fmaxf(vzz, __shfl_xor_sync(0xffffffffu, vzz, o));
+  }
+  if ((threadIdx.x & 31) == 0) { s_xy[threadIdx.x >> 5] = vxy; s_zz[threadIdx.x >> 5] = vzz; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < HI_BLOCK / 32; w++) { vxy = fmaxf(vxy, s_xy[w]); vzz = fmaxf(vzz, s_zz[w]); }
+    a.vmax[2 * (size_t)seg] = vxy; a.vmax[2 * (size_t)seg + 1] = vzz;
+  }
+}
+
+__global__ void __launch_bounds__(HI_BLOCK) hi_place(const __grid_constant__ HiArgs a) {
+  const int seg = blockIdx.x;
+  const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
+  const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
+  const size_t bin0 = (size_t)seg * (size_t)(a.n_phi * a.n_eta);
+  for (int i = b + threadIdx.x; i < e; i += HI_BLOCK) {
+    const unsigned pos = atomicAdd(&a.cnt[bin0 + a.key[i]], 1u);
+    a.sorted_id[pos] = i;
+  }
+}
+
+// one thread per bin: ascending ids (insertion sort for the usual handful, heap sort for crowded edge bins)
+__global__ void __launch_bounds__(HI_BLOCK) hi_sort_bins(const unsigned* __restrict__ bin_off, size_t n_bins, int* sorted_id) {
+  const size_t bin = (size_t)blockIdx.x * HI_BLOCK + threadIdx.x;
+  if (bin >= n_bins) return;
+  const unsigned b = bin_off[bin], e = bin_off[bin + 1];
+  const int len = (int)(e - b);
+  if (len < 2) return;
+  int* v = sorted_id + b;
+  if (len <= 24) {
+    for (int i = 1; i < len; i++) {
+      const int x = v[i];
+      int j = i - 1;
+      while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; j--; }
+      v[j + 1] = x;
+    }
+    return;
+  }
+  auto sift = [&](int start, int end) {
+    int root = start;
+    while (2 * root + 1 <= end) {
+      int child = 2 * root + 1;
+      if (child + 1 <= end && v[child] < v[child + 1]) child++;
+      if (v[root] < v[child]) { const int t = v[root]; v[root] = v[child]; v[child] = t; root = child; }
+      else return;
+    }
+  };
+  for (int s = (len - 2) / 2; s >= 0; s--) sift(s, len - 1);
+  for (int end = len - 1; end > 0; end--) { const int t = v[0]; v[0] = v[end]; v[end] = t; sift(0, end - 1); }
+}
+
+__global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiArgs a) {
+  const int t = blockIdx.x * HI_BLOCK + threadIdx.x;
+  if (t >= a.hits.n_hits) return;
+  const int id = a.sorted_id[t];
+  const size_t nh = (size_t)a.hits.n_hits;
+  const float* V = a.hits.V;
+  float4* o = a.packed + (size_t)3 * t;
+  o[0] = make_float4(a.hits.x[id], a.hits.y[id], a.hits.z[id], __int_as_float(id));
+  o[1] = make_float4(V[id], V[nh + id], V[2 * nh + id], V[3 * nh + id]);
+  o[2] = make_float4(V[4 * nh + id], V[5 * nh + id], 0.f, 0.f);
+}
+
+}  // namespace
+
+namespace mkf {
+size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits) {
+  const size_t nbins = (size_t)n_events * c->g.n_layers * c->g.n_phi * c->g.n_eta;
+  return align256((size_t)n_hits * 4) + align256(nbins * 4) + scan_partial_bytes(nbins);
+}
+}  // namespace mkf
+
+extern "C" int mkf_build_hit_index(mkf_ctx* c, const mkf_hits* h, mkf_hit_index* out, void* ws, size_t ws_bytes, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || !out || !out->bin_off || !out->sorted_id || !out->vmax || !h->layer_off)
+    return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index: null argument");
+  if (h->n_events < 1 || h->n_hits < 0) return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index: bad sizes");
+  if (h->n_hits >= (1 << 28)) return fail(c, MKF_UNSUPPORTED, "mkf_build_hit_index: n_hits >= 2^28");
+  if (h->n_hits > 0 && (!h->x || !h->y || !h->z || !h->V)) return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index: null hit array");
+  const size_t need = hit_index_ws_bytes(c, h->n_events, h->n_hits);
+  if (ws_bytes < need || (need && !ws)) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_build_hit_index: workspace too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nseg = h->n_events * c->g.n_layers;
+  const size_t nbins = (size_t)nseg * c->g.n_phi * c->g.n_eta;
+  char* w = (char*)ws;
+  HiArgs a;
+  a.hits = hits_dev(h); a.n_layers = c->g.n_layers; a.n_phi = c->g.n_phi; a.n_eta = c->g.n_eta;
+  a.key = (int*)w; w += align256((size_t)h->n_hits * 4);
+  a.cnt = (unsigned*)w; w += align256(nbins * 4);
+  unsigned* partial = (unsigned*)w;
+  a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
+  cudaError_t e = cudaMemsetAsync(a.cnt, 0, nbins * 4, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_hit_index: memset");
+  hi_key_count<<<nseg, HI_BLOCK, 0, st>>>(c->g, a);
+  MKF_LAUNCHED(c, "hi_key_count");
+  { const int rc = exclusive_scan_u32(c, a.cnt, nbins, partial, a.bin_off, (unsigned)h->n_hits, st); if (rc) return rc; }
+  if (h->n_hits > 0) {
+    hi_place<<<nseg, HI_BLOCK, 0, st>>>(a);
+    MKF_LAUNCHED(c, "hi_place");
+    hi_sort_bins<<<(unsigned)((nbins + HI_BLOCK - 1) / HI_BLOCK), HI_BLOCK, 0, st>>>(a.bin_off, nbins, a.sorted_id);
+    MKF_LAUNCHED(c, "hi_sort_bins");
+    if (a.packed) {
+      hi_pack<<<(h->n_hits + HI_BLOCK - 1) / HI_BLOCK, HI_BLOCK, 0, st>>>(a);
+      MKF_LAUNCHED(c, "hi_pack");
+    }
+  }
+  return MKF_OK;
+}

@@ -1,0 +1,65 @@
+"""Helpers for the -m gpu parity tests: run the CUDA path through the binding on datagen events."""
+import numpy as np
+import torch
+
+from paper_2002_06295_b200 import binding as B
+
+
+def gpu_fit(ev, prm, seeds=None):
+    s = seeds if seeds is not None else ev["seeds"]
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    sd = B.to_device(s, ["par", "cov", "q", "plan", "track_hits"])
+    n = s["par"].shape[1]
+    out = B.alloc_fit_out(n)
+    ctx.fit(hits, sd, sd["plan"], sd["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+    torch.cuda.synchronize()
+    r = {k: v.cpu().numpy() for k, v in out.items()}
+    r["status"] = r["status"].view(np.uint32)
+    ctx.close()
+    return r
+
+
+def gpu_hit_index(ev, prm, packed=True):
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    out, ws = B.alloc_hit_index(ctx, hits["n_events"], hits["x"].shape[0], packed=packed)
+    ctx.build_hit_index(hits, out, ws)
+    torch.cuda.synchronize()
+    r = dict(bin_off=out["bin_off"].cpu().numpy().view(np.uint32), sorted_id=out["sorted_id"].cpu().numpy(),
+             vmax=out["vmax"].cpu().numpy())
+    if packed:
+        r["packed"] = out["packed"].cpu().numpy()
+    ctx.close()
+    return r
+
+
+def gpu_build(ev, prm, packed=True, dedup=False):
+    s = ev["seeds"]
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    nh = hits["x"].shape[0]
+    idx, ws = B.alloc_hit_index(ctx, hits["n_events"], nh, packed=packed)
+    ctx.build_hit_index(hits, idx, ws)
+    sd = B.to_device(dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"]),
+                     ["par", "cov", "q", "plan", "event", "hits"])
+    n = s["par"].shape[1]
+    out = B.alloc_build_out(n, ctx.max_plan_len)
+    ctx.build_tracks(hits, idx, sd, sd["event"], sd["hits"], sd["plan"], out, out["chi2"], out["score"], out["nhits"],
+                     out["nmiss"], out["hit_ids"], out["status"])
+    r = None
+    if dedup:
+        counts = np.bincount(s["event"], minlength=hits["n_events"])
+        toff = torch.from_numpy(np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)).cuda()
+        keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+        nk = torch.empty(hits["n_events"], dtype=torch.int32, device="cuda")
+        ws2 = torch.empty(max(ctx.workspace_bytes(B.CALL_REMOVE_DUPLICATES, hits["n_events"], nh, n), 256), dtype=torch.uint8, device="cuda")
+        ctx.remove_duplicates(nh, toff, out["hit_ids"], out["nhits"], out["score"], keep, nk, ws2)
+    torch.cuda.synchronize()
+    r = {k: v.cpu().numpy() for k, v in out.items()}
+    r["status"] = r["status"].view(np.uint32)
+    if dedup:
+        r["keep"] = keep.cpu().numpy(); r["n_kept"] = nk.cpu().numpy(); r["track_off"] = toff.cpu().numpy()
+    r["launches"] = ctx.launch_count()
+    ctx.close()
+    return r

@@ -1,0 +1,184 @@
+"""-m gpu: hit index (bit-exact), track building (hit lists identical up to small oracle margins) and duplicate
+removal (exact) against the oracle."""
+import numpy as np
+import pytest
+
+from oracle import mkfo
+from paper_2002_06295_b200 import datagen
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+def check_index(ev, prm):
+    from gpu_helpers import gpu_hit_index
+    o = mkfo.Oracle(ev["geom"], prm)
+    ref = o.build_hit_index(ev["hits"])
+    got = gpu_hit_index(ev, prm)
+    assert np.array_equal(got["bin_off"], ref["bin_off"])
+    assert np.array_equal(got["sorted_id"], ref["sorted_id"])
+    assert np.array_equal(got["vmax"].view(np.uint32), ref["vmax"].view(np.uint32))     # bit-exact floats
+    # packed records are the hits in sorted order
+    pk = got["packed"].reshape(-1, 12)
+    sid = ref["sorted_id"]
+    h = ev["hits"]
+    assert np.array_equal(pk[:, 3].copy().view(np.int32), sid)
+    assert np.array_equal(pk[:, 0], h["x"][sid]) and np.array_equal(pk[:, 2], h["z"][sid])
+    assert np.array_equal(pk[:, 4:10], h["V"][:, sid].T)
+    return ref
+
+
+def test_hit_index_barrel_bit_exact():
+    ev, prm = datagen.config(2, scale=0.05)           # 5 events x 17 layers
+    check_index(ev, prm)
+
+
+def test_hit_index_endcap_bit_exact():
+    ev, prm = datagen.config(3, scale=0.015)          # 3 events x 38 layers, ~80k hits each
+    check_index(ev, prm)
+
+
+def test_hit_index_empty_layers_and_crowded_bins():
+    """Layers without hits, and all hits of a layer in one bin (exercises the heap-sort branch)."""
+    g = datagen.geometry_barrel(3, 10.0, 30.0, 50.0, 0.02)
+    n1 = 700
+    rng = np.random.default_rng(3)
+    # layer 0: empty; layer 1: n1 hits at (nearly) the same place; layer 2: 5 hits spread out
+    ph2 = np.linspace(-3, 3, 5)
+    x = np.concatenate([20 * np.cos(0.3 + 1e-6 * rng.random(n1)), 30 * np.cos(ph2)])
+    y = np.concatenate([20 * np.sin(0.3 + 1e-6 * rng.random(n1)), 30 * np.sin(ph2)])
+    z = np.concatenate([np.full(n1, 1.0), np.linspace(-40, 40, 5)])
+    V = np.zeros((6, n1 + 5), np.float32); V[0] = V[2] = 1e-5; V[5] = 1e-4; V[1] = 3e-6
+    hits = dict(n_events=1, layer_off=np.array([0, 0, n1, n1 + 5], np.int32), x=x.astype(np.float32), y=y.astype(np.float32),
+                z=z.astype(np.float32), V=V)
+    check_index(dict(geom=g, hits=hits), datagen.default_params())
+
+
+def compare_build(ev, prm, r, h, min_same=0.999):
+    n = r["nhits"].shape[0]
+    same = np.all(h["hit_ids"] == r["hit_ids"], axis=0)
+    frac = same.mean()
+    # mismatches only where the oracle itself was within 1e-3 of a decision boundary (U20)
+    assert np.all(r["margin"][~same] < 1e-3), (np.sort(r["margin"][~same])[-5:], frac)
+    assert frac >= min_same, frac
+    assert np.array_equal(h["nhits"][same], r["nhits"][same])
+    assert np.array_equal(h["nmiss"][same], r["nmiss"][same])
+    assert np.array_equal(h["status"][same], r["status"][same])
+    ok = same & ((r["status"] & 32) == 0)
+    # the state sits on the layer of the last found hit
+    geom = ev["geom"]
+    plan_off, plan_layers = np.asarray(geom["plan_off"]), np.asarray(geom["plan_layers"])
+    hid = r["hit_ids"]
+    has = hid >= 0
+    last = hid.shape[0] - 1 - np.argmax(has[::-1], axis=0)
+    lay = plan_layers[plan_off[ev["seeds"]["plan"].astype(int)] + last]
+    kinds = np.array([l["kind"] for l in geom["layers"]])[lay]
+    pos = np.array([abs(l["pos"]) for l in geom["layers"]])[lay]
+    # a candidate that ended on missed layers has been propagated beyond its last hit: find the surface it is on
+    # from the state itself (barrel if its radius matches a barrel layer better than its z matches a disk)
+    pe = parity.param_errors(h["par"], r["par"], np.maximum(pos, 1.0))[ok]
+    xe = parity.chi2_errors(h["chi2"], r["chi2"])[ok]
+    se = np.abs(h["score"] - r["score"])[ok] / np.maximum(np.abs(r["score"][ok]), 1.0)
+    assert pe.max() <= parity.TOL_PAR, pe.max()
+    assert xe.max() <= parity.TOL_CHI2, xe.max()
+    assert se.max() <= parity.TOL_CHI2, se.max()
+    # covariance: on the surface the state sits on (the last crossed layer, hit or miss)
+    crossed = hid >= -1
+    lastc = hid.shape[0] - 1 - np.argmax(crossed[::-1], axis=0)
+    layc = plan_layers[plan_off[ev["seeds"]["plan"].astype(int)] + lastc]
+    kindc = np.array([l["kind"] for l in geom["layers"]])[layc]
+    ce = parity.cov_errors(h["cov"], r["cov"], r["par"], kindc)[ok]
+    assert np.quantile(ce, 0.999) <= parity.TOL_COV and ce.max() <= 3 * parity.TOL_COV, (np.quantile(ce, 0.999), ce.max())
+    return frac
+
+
+def run_build(ev, prm, brute=False, packed=True):
+    from gpu_helpers import gpu_build
+    s = ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], prm)
+    idx = o.build_hit_index(ev["hits"])
+    r = o.build_tracks(ev["hits"], idx, s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"], brute_force=brute)
+    h = gpu_build(ev, prm, packed=packed)
+    return r, h
+
+
+def test_build_barrel_config2_sample():
+    ev, prm = datagen.config(2, scale=0.05)           # 5 events x 1000 seeds, 20k noise hits each
+    r, h = run_build(ev, prm)
+    frac = compare_build(ev, prm, r, h)
+    assert (r["nhits"] >= 10).mean() > 0.8
+
+
+def test_build_barrel_unpacked_gather_path_and_brute_force_oracle():
+    ev, prm = datagen.config(2, scale=0.01)
+    r, h = run_build(ev, prm, brute=True, packed=False)       # oracle tries every hit of the layer
+    compare_build(ev, prm, r, h)
+
+
+def test_build_barrel_endcap_config3_sample():
+    ev, prm = datagen.config(3, scale=0.015)          # 3 events x ~1500 seeds, 38 layers, propagateToZ, 5 % inefficiency
+    r, h = run_build(ev, prm)
+    compare_build(ev, prm, r, h)
+    assert (r["nmiss"] > 0).mean() > 0.1 and ((r["status"] & 32) != 0).sum() >= 0
+
+
+def test_build_config4_like_eight_candidates_and_duplicate_removal():
+    from gpu_helpers import gpu_build
+    ev, prm = datagen.config(4, scale=1 / 64.0)       # one high-occupancy event, 6000 seeds, max_cand 8
+    s = ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], prm)
+    idx = o.build_hit_index(ev["hits"])
+    r = o.build_tracks(ev["hits"], idx, s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    h = gpu_build(ev, prm, dedup=True)
+    compare_build(ev, prm, r, h)
+    # duplicate removal is integer-only: the oracle on the GPU's own built tracks must agree exactly
+    d = o.remove_duplicates(h["track_off"], h["hit_ids"], h["nhits"], h["score"])
+    assert np.array_equal(h["keep"], d["keep"]) and np.array_equal(h["n_kept"], d["n_kept"])
+
+
+def test_remove_duplicates_exact_on_synthetic_overlaps():
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    rng = np.random.default_rng(11)
+    g = datagen.geometry_barrel(12, 4.0, 48.0, 100.0, 0.02)
+    prm = datagen.default_params()
+    n_events, per_ev, mpl, hits_per_ev = 3, 400, 12, 3000
+    n = n_events * per_ev
+    hit_ids = np.full((mpl, n), -1, np.int32)
+    for i in range(n):
+        ev = i // per_ev
+        if i % 3 and i > ev * per_ev:                                  # derive from the previous track: heavy overlap
+            hit_ids[:, i] = hit_ids[:, i - 1]
+            k = rng.integers(0, mpl, rng.integers(1, 9))
+            hit_ids[k, i] = ev * hits_per_ev + rng.integers(0, hits_per_ev, k.size)
+        else:
+            hit_ids[:, i] = ev * hits_per_ev + rng.integers(0, hits_per_ev, mpl)
+        hit_ids[rng.random(mpl) < 0.2, i] = -1
+    nhits = (hit_ids >= 0).sum(0).astype(np.int32)
+    score = np.round(rng.normal(200, 30, n)).astype(np.float32)         # rounded: many exact ties
+    toff = (np.arange(n_events + 1) * per_ev).astype(np.int32)
+    ref = mkfo.Oracle(g, prm).remove_duplicates(toff, hit_ids, nhits, score)
+    ctx = B.Context(g, prm)
+    nh = n_events * hits_per_ev
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda"); nk = torch.empty(n_events, dtype=torch.int32, device="cuda")
+    ws = torch.empty(ctx.workspace_bytes(B.CALL_REMOVE_DUPLICATES, n_events, nh, n), dtype=torch.uint8, device="cuda")
+    ctx.remove_duplicates(nh, torch.from_numpy(toff).cuda(), torch.from_numpy(hit_ids).cuda(), torch.from_numpy(nhits).cuda(),
+                          torch.from_numpy(score).cuda(), keep, nk, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(keep.cpu().numpy(), ref["keep"]) and np.array_equal(nk.cpu().numpy(), ref["n_kept"])
+    assert 0.2 < ref["keep"].mean() < 0.95
+    ctx.close()
+
+
+def test_build_host_entry_point_matches_device_path():
+    from gpu_helpers import gpu_build
+    from paper_2002_06295_b200 import binding as B
+    ev, prm = datagen.config(2, scale=0.02)
+    h = gpu_build(ev, prm, dedup=True)
+    ctx = B.Context(ev["geom"], prm)
+    s = ev["seeds"]
+    r = ctx.build_host(ev["hits"], s, np.ascontiguousarray(s["event"]), np.ascontiguousarray(s["hits"]),
+                       np.ascontiguousarray(s["plan"]), dedup=True)
+    for k in ("hit_ids", "nhits", "nmiss", "chi2", "score", "par", "cov", "keep"):
+        assert np.array_equal(r[k], h[k]), k
+    ctx.close()

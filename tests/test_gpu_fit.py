@@ -1,0 +1,116 @@
+"""-m gpu: mkf_fit (CUDA, fp32) against the fp64 oracle on the same seeded inputs (tolerances: BASELINE.json
+north_star; U19 of DESIGN.md §3 says how 'relative' is read)."""
+import numpy as np
+import pytest
+
+from oracle import mkfo
+from paper_2002_06295_b200 import datagen
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+def check_fit(ev, prm, seeds=None, min_good=0.99):
+    from gpu_helpers import gpu_fit
+    s = seeds if seeds is not None else ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], prm)
+    r = o.fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], s["track_hits"])
+    h = gpu_fit(ev, prm, s)
+    # integer outputs: identical
+    assert np.array_equal(h["nfit"], r["nfit"])
+    assert np.array_equal(h["status"], r["status"])
+    ok = r["nfit"] > 0
+    assert ok.mean() >= min_good
+    lay, kinds, pos = parity.last_layer_of_fit(ev["geom"], s["plan"], s["track_hits"], r["nfit"])
+    pe = parity.param_errors(h["par"], r["par"], pos)[ok]
+    ce = parity.cov_errors(h["cov"], r["cov"], r["par"], kinds)[ok]
+    xe = parity.chi2_errors(h["chi2"], r["chi2"])[ok]
+    assert pe.max() <= parity.TOL_PAR, pe.max()
+    assert xe.max() <= parity.TOL_CHI2, xe.max()
+    assert ce.max() <= parity.TOL_COV, ce.max()
+    return r, h
+
+
+def test_fit_config0_full():
+    ev, prm = datagen.config(0)                       # 10 000 helices, 10 layers: 79 CTAs, ragged last CTA
+    r, h = check_fit(ev, prm)
+    assert r["nfit"].sum() == 100000
+
+
+def test_fit_config1_sample():
+    ev, prm = datagen.config(1, scale=0.0125)          # 50 000 helices, 17 layers incl. low-pT tracks that stop early
+    r, h = check_fit(ev, prm)
+    assert (r["nfit"] < 17).mean() > 0.03              # the short (near-grazing) tracks are in the sample
+
+
+def test_fit_barrel_endcap_truth_hits():
+    ev, prm = datagen.config(3, scale=0.01)            # 2 events of the 38-layer geometry: propagateToZ on disks
+    r, h = check_fit(ev, prm, min_good=0.9)
+    kinds = np.array([l["kind"] for l in ev["geom"]["layers"]])
+    lay, k, pos = parity.last_layer_of_fit(ev["geom"], ev["seeds"]["plan"], ev["seeds"]["track_hits"], r["nfit"])
+    assert (k == 1).sum() > 100 and (k == 0).sum() > 100
+
+
+def test_fit_material_flags_and_status_paths():
+    ev, prm = datagen.config(0, scale=0.05)
+    for flags in (0, 1, 2):
+        check_fit(ev, dict(prm, material_flags=flags))
+    # unreachable: a 0.2 GeV track cannot reach r = 40 cm (radius of curvature 17.5 cm)
+    s = {k: np.array(v[..., :64]) for k, v in ev["seeds"].items() if k in ("par", "cov", "q", "plan", "track_hits")}
+    s["par"][3, :32] = 5.0
+    # grazing / energy exhausted: very soft tracks
+    s["par"][3, 32:48] = 1.0 / 0.27
+    s["par"][3, 48:] = 1.0 / 0.05
+    from gpu_helpers import gpu_fit
+    o = mkfo.Oracle(ev["geom"], prm)
+    r = o.fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], s["track_hits"])
+    h = gpu_fit(ev, prm, s)
+    assert np.array_equal(h["nfit"], r["nfit"]) and np.array_equal(h["status"], r["status"])
+    assert (r["status"] & 1).any() and (r["status"] != 0).sum() >= 48
+    ok = r["nfit"] > 0
+    lay, kinds, pos = parity.last_layer_of_fit(ev["geom"], s["plan"], s["track_hits"], r["nfit"])
+    assert parity.param_errors(h["par"], r["par"], pos)[ok].max() <= parity.TOL_PAR
+    # tracks that never fitted a hit return their seed unchanged
+    z = r["nfit"] == 0
+    if z.any():
+        assert np.allclose(h["par"][:3, z], s["par"][:3, z], atol=0, rtol=0)
+
+
+def test_fit_empty_and_no_hits():
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    ev, prm = datagen.config(0, scale=0.01)
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    s = ev["seeds"]
+    sd = B.to_device(s, ["par", "cov", "q", "plan", "track_hits"])
+    # n = 0: nothing launched, OK
+    e = {k: v[..., :0].contiguous() for k, v in sd.items()}
+    out = B.alloc_fit_out(0)
+    before = ctx.launch_count()
+    ctx.fit(hits, e, e["plan"], e["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+    assert ctx.launch_count() == before
+    # tracks without any hit: state returned unchanged, nfit 0, chi2 0
+    sd["track_hits"].fill_(-1)
+    n = s["par"].shape[1]
+    out = B.alloc_fit_out(n)
+    ctx.fit(hits, sd, sd["plan"], sd["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+    torch.cuda.synchronize()
+    assert int(out["nfit"].sum()) == 0 and float(out["chi2"].abs().sum()) == 0.0
+    assert torch.equal(out["par"][:4], sd["par"][:4]) and torch.equal(out["cov"], sd["cov"])
+    ctx.close()
+
+
+def test_fit_host_entry_point_matches_device_path():
+    from gpu_helpers import gpu_fit
+    from paper_2002_06295_b200 import binding as B
+    ev, prm = datagen.config(0, scale=0.1)
+    h = gpu_fit(ev, prm)
+    ctx = B.Context(ev["geom"], prm)
+    s = ev["seeds"]
+    r = ctx.fit_host(ev["hits"], s, np.ascontiguousarray(s["plan"]), np.ascontiguousarray(s["track_hits"]))
+    for k in ("par", "cov", "chi2", "nfit"):
+        assert np.array_equal(r[k], h[k]), k
+    n = s["par"].shape[1]
+    assert r["d2h_bytes"] == n * (27 * 4 + 12) and r["h2d_bytes"] > n * 27 * 4
+    ctx.close()
