@@ -48,7 +48,7 @@ __device__ __forceinline__ void load_packed(Hit& H, int& id, const float4* __res
 }
 
 // U11: window of bins that contains every hit with chi2 < cut (fp32, one extra bin of padding on every side).
-__device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, float cut, const KState& S, const Frame& f,
+__device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, float cut, const KState& S,
                                        float tt, float zz_or_yy, float vxy, float vzz, int& e0, int& e1, int& p0, int& np) {
   const float x = S.x + S.xl, y = S.y + S.yl, z = S.z + S.zl;
   const float php = atan2f(y, x);
@@ -88,7 +88,9 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
     S.x = __shfl_sync(gm, S.x, src); S.y = __shfl_sync(gm, S.y, src); S.z = __shfl_sync(gm, S.z, src);       \
     S.xl = __shfl_sync(gm, S.xl, src); S.yl = __shfl_sync(gm, S.yl, src); S.zl = __shfl_sync(gm, S.zl, src); \
     S.ipt = __shfl_sync(gm, S.ipt, src); S.phi = __shfl_sync(gm, S.phi, src); S.th = __shfl_sync(gm, S.th, src); \
-    _Pragma("unroll") for (int k_ = 0; k_ < 21; k_++) S.c[k_] = __shfl_sync(gm, S.c[k_], src);             \
+    S.f.kind = __shfl_sync(gm, S.f.kind, src); S.f.cb = __shfl_sync(gm, S.f.cb, src); S.f.sb = __shfl_sync(gm, S.f.sb, src); \
+    _Pragma("unroll") for (int k_ = 0; k_ < 10; k_++) S.u[k_] = __shfl_sync(gm, S.u[k_], src);             \
+    _Pragma("unroll") for (int k_ = 0; k_ < 5; k_++) S.d[k_] = __shfl_sync(gm, S.d[k_], src);              \
   } while (0)
 
 __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_constant__ GeomDev g,
@@ -124,7 +126,8 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
   }
   __syncwarp(gm);
   if (have_seed && sub == 0) {
-    load_state(S, a.par, a.cov, n, (size_t)i);
+    load_params(S, a.par, n, (size_t)i);
+    bool has_ud = false;
     const int* loff = a.hits.layer_off + (size_t)ev * (g.n_layers + 1);
     seed_ok = true;
     for (int k = 0; k < 3 && seed_ok; k++) {
@@ -135,18 +138,19 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
       for (int s = last_step + 1; s < plen; s++) if ((int)g.plan_layers[p0 + s] == lay) { step = s; break; }
       if (step < 0) { stat |= ST_TRUNC; seed_ok = false; break; }
       const LayerDev L = g.layers[lay];
-      const unsigned rc = step_to_layer(S, L, aq, p.graze_cos_min, p.material_flags, false);
+      const unsigned rc = step_to_layer(S, !has_ud, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
       if (rc) { stat |= rc; seed_ok = false; break; }
+      has_ud = true;
       Hit H; load_hit(H, a.hits, hid);
-      const Frame f = frame_of(S, L.kind);
       SInv o; float c2;
-      if (!chi2_of(S, f, H, o, c2)) { stat |= ST_S_NOT_PD; seed_ok = false; break; }
-      kalman_update(S, f, o);
+      if (!chi2_of(S, H, o, c2)) { stat |= ST_S_NOT_PD; seed_ok = false; break; }
+      kalman_update(S, o);
       chi2 += c2; nh++; last_step = step;
       trellis[step * G + 0] = (unsigned)(hid + 2);
     }
     // fallback output: the seed candidate itself (C9 last line); overwritten by best_short / the final winner
-    store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+    if (has_ud) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+    else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
     live = seed_ok;
   }
   seed_ok = __shfl_sync(gm, (int)seed_ok, gbase) != 0;
@@ -176,22 +180,17 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
     bool miss_avail = false, pass_avail = false;
     bool offer = false; int offer_phase = 0; float offer_score = 0.f; int offer_nm = 0;
     if (live) {
-      const unsigned rc = step_to_layer(S, L, aq, p.graze_cos_min, p.material_flags, true);
+      const unsigned rc = step_to_layer(S, false, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, true);
       if (rc & (ST_UNREACH | ST_SKIP_ACC)) {
         pass_avail = true;                                   // silent skip: competes unchanged (C9.1)
       } else if (rc) {                                       // grazing / energy exhausted: the candidate stops
         stat |= rc;
         if (nh >= p.min_hits_keep) { offer = true; offer_phase = 0; offer_nm = nm; offer_score = score_of(p, nh, nm, chi2); }
       } else {
-        const Frame f = frame_of(S, L.kind);
         float tt, tz, zz;
-        if (L.kind == 0) {
-          tt = f.sb * f.sb * S.c[CI(0, 0)] - 2.f * f.sb * f.cb * S.c[CI(1, 0)] + f.cb * f.cb * S.c[CI(1, 1)];
-          tz = f.cb * S.c[CI(2, 1)] - f.sb * S.c[CI(2, 0)];
-          zz = S.c[CI(2, 2)];
-        } else { tt = S.c[CI(0, 0)]; tz = S.c[CI(1, 0)]; zz = S.c[CI(1, 1)]; }
+        cov_aa(S, tt, tz, zz);
         int e0, e1, w0, wn;
-        window(g, L, p.chi2_cut, S, f, tt, zz, a.vmax[2 * seg], a.vmax[2 * seg + 1], e0, e1, w0, wn);
+        window(g, L, p.chi2_cut, S, tt, zz, a.vmax[2 * seg], a.vmax[2 * seg + 1], e0, e1, w0, wn);
         const unsigned* boff = a.bin_off + seg * (size_t)nb;
         for (int ie = e0; ie <= e1; ie++) {
           const unsigned* row = boff + ie * g.n_phi;
@@ -205,7 +204,7 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
               if (a.packed) load_packed(H, id, a.packed + (size_t)3 * t);
               else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
               SInv o; float c2;
-              if (!chi2_local(S, f, tt, tz, zz, H, o, c2)) continue;
+              if (!chi2_local(S, tt, tz, zz, H, o, c2)) continue;
               if (c2 < p.chi2_cut) {
                 n_hitc = min(n_hitc + 1, G);
                 float v = c2; int vid = id;
@@ -291,10 +290,9 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
       if (my_kind == 1) { nm++; consec++; }
       else if (my_kind == 0) {
         Hit H; load_hit(H, a.hits, my_hit);
-        const Frame f = frame_of(S, L.kind);
         SInv o; float c2;
-        if (chi2_of(S, f, H, o, c2)) {
-          kalman_update(S, f, o);
+        if (chi2_of(S, H, o, c2)) {
+          kalman_update(S, o);
           chi2 += c2; nh++; consec = 0;
           if (!state_finite(S)) live = false;                 // dropped (C9: NaN child)
         } else live = false;

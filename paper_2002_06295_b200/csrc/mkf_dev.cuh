@@ -22,19 +22,52 @@ struct ParamsDev {
 
 struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; };
 
-MKF_HD void load_state(KState& S, const float* par, const float* cov, size_t n, size_t i) {
+// Parameters of a caller's state; the covariance is read separately by the first propagation (commit_first).
+MKF_HD void load_params(KState& S, const float* par, size_t n, size_t i) {
   S.x = par[i]; S.y = par[n + i]; S.z = par[2 * n + i];
   S.xl = 0.f; S.yl = 0.f; S.zl = 0.f;
   S.ipt = par[3 * n + i]; S.phi = par[4 * n + i]; S.th = par[5 * n + i];
+  S.f.kind = 0; S.f.cb = 1.f; S.f.sb = 0.f;
 #pragma unroll
-  for (int k = 0; k < 21; k++) S.c[k] = cov[(size_t)k * n + i];
+  for (int k = 0; k < 10; k++) S.u[k] = 0.f;
+#pragma unroll
+  for (int k = 0; k < 5; k++) S.d[k] = 0.f;
 }
 
+MKF_HD void load_cov(float* c, const float* cov, size_t n, size_t i) {
+#pragma unroll
+  for (int k = 0; k < 21; k++) c[k] = cov[(size_t)k * n + i];
+}
+
+// State with factors -> the caller's layout (global packed 6x6).
 MKF_HD void store_state(const KState& S, float* par, float* cov, size_t n, size_t i) {
   par[i] = S.x + S.xl; par[n + i] = S.y + S.yl; par[2 * n + i] = S.z + S.zl;
   par[3 * n + i] = S.ipt; par[4 * n + i] = wrap_phi(S.phi); par[5 * n + i] = S.th;
+  float l[15], c[21];
+  ud_to_cov(S.u, S.d, l);
+  cov_from_local(l, S.f, c);
 #pragma unroll
-  for (int k = 0; k < 21; k++) cov[(size_t)k * n + i] = S.c[k];
+  for (int k = 0; k < 21; k++) cov[(size_t)k * n + i] = c[k];
+}
+
+// A state that never completed a propagation: the caller's seed goes out as it came in.
+MKF_HD void copy_seed(const float* par, const float* cov, float* par_out, float* cov_out, size_t n, size_t i) {
+#pragma unroll
+  for (int k = 0; k < 6; k++) par_out[(size_t)k * n + i] = par[(size_t)k * n + i];
+#pragma unroll
+  for (int k = 0; k < 21; k++) cov_out[(size_t)k * n + i] = cov[(size_t)k * n + i];
+}
+
+// One filter step up to (not including) the update. `first`: the state has no factors yet (they are made from the
+// caller's covariance). Returns 0 and the advanced state, or a status bit with the state unchanged.
+MKF_HD unsigned step_to_layer(KState& S, bool first, const float* cov, size_t n, size_t i, const LayerDev& L, float aq,
+                              float graze_cos_min, int mflags, bool check_acc) {
+  Prop P;
+  const unsigned rc = propagate_geom(S, L, aq, graze_cos_min, mflags, check_acc, P);
+  if (rc) return rc;
+  if (first) { float c[21]; load_cov(c, cov, n, i); commit_first(S, c, P, mflags); }
+  else commit_step(S, P, mflags);
+  return 0;
 }
 
 MKF_HD void load_hit(Hit& H, const HitsDev& h, int id) {
@@ -67,7 +100,7 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
   KState S;
   float c2tot; int nf;
   for (int pass = 0; pass < 2; pass++) {
-    load_state(S, a.par, a.cov, n, (size_t)i);
+    load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0;
     bool redo = false;
     for (int s = 0; s < stop_at; s++) {
@@ -75,18 +108,18 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
       if (hid < 0) continue;
       const LayerDev L = g.layers[g.plan_layers[p0 + s]];
       Hit H; load_hit(H, a.hits, hid);
-      const unsigned rc = step_to_layer(S, L, aq, p.graze_cos_min, p.material_flags, false);
+      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
       if (rc) { stat |= rc; break; }
       SInv o; float c2;
-      const Frame f = frame_of(S, L.kind);
-      if (!chi2_of(S, f, H, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
-      kalman_update(S, f, o);
+      if (!chi2_of(S, H, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
+      kalman_update(S, o);
       if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; stop_at = s; redo = true; break; }
       c2tot += c2; nf++;
     }
     if (!redo) break;
   }
-  store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+  if (nf > 0) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+  else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
   a.chi2[i] = c2tot; a.nfit[i] = nf; a.status[i] = stat;
 }
 
