@@ -59,9 +59,10 @@ extern "C" int mkf_fit(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, c
                        unsigned* status, void* ws, size_t ws_bytes, void* stream) {
   (void)ws; (void)ws_bytes;
   if (!c) return MKF_INVALID_ARG;
-  if (!h || !seeds || !out || !plan || !track_hits || !chi2 || !nfit || !status) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
+  if (!h || !seeds || !out) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
   if (seeds->n < 0 || out->n != seeds->n || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_fit: bad sizes");
-  if (seeds->n == 0) return MKF_OK;
+  if (seeds->n == 0) return MKF_OK;                      // nothing to do; array pointers may be null
+  if (!plan || !track_hits || !chi2 || !nfit || !status) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
   if (!h->x || !h->y || !h->z || !h->V || !seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov)
     return fail(c, MKF_INVALID_ARG, "mkf_fit: null array");
   FitArgs a;

@@ -367,11 +367,12 @@ extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_ind
                                 unsigned* status, void* ws, size_t ws_bytes, void* stream) {
   (void)ws; (void)ws_bytes;
   if (!c) return MKF_INVALID_ARG;
-  if (!h || !idx || !seeds || !out || !seed_event || !seed_hits || !plan || !chi2 || !score || !nhits || !nmiss || !hit_ids || !status)
-    return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
+  if (!h || !idx || !seeds || !out) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
   if (seeds->n < 0 || out->n != seeds->n || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: bad sizes");
   if (h->n_hits >= (1 << 28)) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: n_hits >= 2^28");
-  if (seeds->n == 0) return MKF_OK;
+  if (seeds->n == 0) return MKF_OK;                      // nothing to do; array pointers may be null
+  if (!seed_event || !seed_hits || !plan || !chi2 || !score || !nhits || !nmiss || !hit_ids || !status)
+    return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
   if (!idx->bin_off || !idx->sorted_id || !idx->vmax || !h->layer_off || !h->x || !h->y || !h->z || !h->V ||
       !seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov)
     return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null array");

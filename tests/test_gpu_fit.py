@@ -55,25 +55,28 @@ def test_fit_material_flags_and_status_paths():
     ev, prm = datagen.config(0, scale=0.05)
     for flags in (0, 1, 2):
         check_fit(ev, dict(prm, material_flags=flags))
-    # unreachable: a 0.2 GeV track cannot reach r = 40 cm (radius of curvature 17.5 cm)
-    s = {k: np.array(v[..., :64]) for k, v in ev["seeds"].items() if k in ("par", "cov", "q", "plan", "track_hits")}
-    s["par"][3, :32] = 5.0
-    # grazing / energy exhausted: very soft tracks
-    s["par"][3, 32:48] = 1.0 / 0.27
-    s["par"][3, 48:] = 1.0 / 0.05
+    # status paths, with the states frozen (covariance x1e-8, no scattering noise) so that the hits cannot pull
+    # them back: 0.2 GeV cannot reach r = 36 cm (radius of curvature 17.5 cm) -> PROP_UNREACHABLE; 0.05 GeV loses
+    # all its energy -> STOPPED_ELOSS; 0.226..0.24 GeV straddles the grazing threshold at r = 40 cm -> GRAZING
     from gpu_helpers import gpu_fit
-    o = mkfo.Oracle(ev["geom"], prm)
-    r = o.fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], s["track_hits"])
-    h = gpu_fit(ev, prm, s)
-    assert np.array_equal(h["nfit"], r["nfit"]) and np.array_equal(h["status"], r["status"])
-    assert (r["status"] & 1).any() and (r["status"] != 0).sum() >= 48
-    ok = r["nfit"] > 0
-    lay, kinds, pos = parity.last_layer_of_fit(ev["geom"], s["plan"], s["track_hits"], r["nfit"])
-    assert parity.param_errors(h["par"], r["par"], pos)[ok].max() <= parity.TOL_PAR
-    # tracks that never fitted a hit return their seed unchanged
-    z = r["nfit"] == 0
-    if z.any():
-        assert np.allclose(h["par"][:3, z], s["par"][:3, z], atol=0, rtol=0)
+    s = {k: np.array(v[..., :64]) for k, v in ev["seeds"].items() if k in ("par", "cov", "q", "plan", "track_hits")}
+    s["cov"] *= 1e-8
+    for flags, ipt, want in ((2, np.r_[np.full(32, 5.0), np.full(32, 20.0)], (1, 16)),
+                             (0, 1.0 / np.linspace(0.226, 0.24, 64), (2,))):
+        s["par"][3] = ipt
+        p2 = dict(prm, material_flags=flags)
+        r = mkfo.Oracle(ev["geom"], p2).fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], s["track_hits"])
+        h = gpu_fit(ev, p2, s)
+        assert np.array_equal(h["nfit"], r["nfit"]) and np.array_equal(h["status"], r["status"])
+        for bit in want:
+            assert (r["status"] & bit).any(), bit
+        assert (r["status"] == 0).any() or flags == 2
+        ok = r["nfit"] > 0
+        lay, kinds, pos = parity.last_layer_of_fit(ev["geom"], s["plan"], s["track_hits"], r["nfit"])
+        assert parity.param_errors(h["par"], r["par"], pos)[ok].max() <= parity.TOL_PAR
+        z = r["nfit"] == 0                           # tracks that never fitted a hit return their seed unchanged
+        if z.any():
+            assert np.array_equal(h["par"][:, z], s["par"][:, z]) and np.array_equal(h["cov"][:, z], s["cov"][:, z])
 
 
 def test_fit_empty_and_no_hits():
