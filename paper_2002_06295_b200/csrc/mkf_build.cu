@@ -143,8 +143,8 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
       has_ud = true;
       Hit H; load_hit(H, a.hits, hid);
       SInv o; float c2;
-      if (!chi2_of(S, H, o, c2)) { stat |= ST_S_NOT_PD; seed_ok = false; break; }
-      kalman_update(S, o);
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; seed_ok = false; break; }
       chi2 += c2; nh++; last_step = step;
       trellis[step * G + 0] = (unsigned)(hid + 2);
     }
@@ -291,8 +291,8 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
       else if (my_kind == 0) {
         Hit H; load_hit(H, a.hits, my_hit);
         SInv o; float c2;
-        if (chi2_of(S, H, o, c2)) {
-          kalman_update(S, o);
+        hit_to_local(S, H, o);
+        if (kalman_update(S, o, c2)) {
           chi2 += c2; nh++; consec = 0;
           if (!state_finite(S)) live = false;                 // dropped (C9: NaN child)
         } else live = false;

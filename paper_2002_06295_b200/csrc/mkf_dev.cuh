@@ -99,7 +99,10 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
   int stop_at = plen;
   KState S;
   float c2tot; int nf;
-  for (int pass = 0; pass < 2; pass++) {
+  // pass 0 runs without per-step finiteness checks; only if its result is not finite, pass 1 finds the step
+  // and pass 2 stops before it
+  for (int pass = 0; pass < 3; pass++) {
+    const bool check = pass == 1;
     load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0;
     bool redo = false;
@@ -111,12 +114,16 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
       const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
       if (rc) { stat |= rc; break; }
       SInv o; float c2;
-      if (!chi2_of(S, H, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
-      kalman_update(S, o);
-      if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; stop_at = s; redo = true; break; }
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) {                          // state untouched by the failed update, but already
+        stat |= ST_S_NOT_PD; stop_at = s; redo = true; break;  // propagated: re-run up to the step before
+      }
+      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; break; }
       c2tot += c2; nf++;
     }
-    if (!redo) break;
+    if (redo) continue;
+    if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
+    break;
   }
   if (nf > 0) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
   else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
