@@ -88,6 +88,8 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
     S.x = __shfl_sync(gm, S.x, src); S.y = __shfl_sync(gm, S.y, src); S.z = __shfl_sync(gm, S.z, src);       \
     S.xl = __shfl_sync(gm, S.xl, src); S.yl = __shfl_sync(gm, S.yl, src); S.zl = __shfl_sync(gm, S.zl, src); \
     S.ipt = __shfl_sync(gm, S.ipt, src); S.phi = __shfl_sync(gm, S.phi, src); S.th = __shfl_sync(gm, S.th, src); \
+    S.cph = __shfl_sync(gm, S.cph, src); S.sph = __shfl_sync(gm, S.sph, src);                                 \
+    S.cth = __shfl_sync(gm, S.cth, src); S.sth = __shfl_sync(gm, S.sth, src);                                 \
     S.f.kind = __shfl_sync(gm, S.f.kind, src); S.f.cb = __shfl_sync(gm, S.f.cb, src); S.f.sb = __shfl_sync(gm, S.f.sb, src); \
     _Pragma("unroll") for (int k_ = 0; k_ < 10; k_++) S.u[k_] = __shfl_sync(gm, S.u[k_], src);             \
     _Pragma("unroll") for (int k_ = 0; k_ < 5; k_++) S.d[k_] = __shfl_sync(gm, S.d[k_], src);              \

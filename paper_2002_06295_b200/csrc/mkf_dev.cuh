@@ -27,6 +27,8 @@ MKF_HD void load_params(KState& S, const float* par, size_t n, size_t i) {
   S.x = par[i]; S.y = par[n + i]; S.z = par[2 * n + i];
   S.xl = 0.f; S.yl = 0.f; S.zl = 0.f;
   S.ipt = par[3 * n + i]; S.phi = par[4 * n + i]; S.th = par[5 * n + i];
+  sincos_f(S.phi, &S.sph, &S.cph);
+  sincos_f(S.th, &S.sth, &S.cth);
   S.f.kind = 0; S.f.cb = 1.f; S.f.sb = 0.f;
 #pragma unroll
   for (int k = 0; k < 10; k++) S.u[k] = 0.f;
@@ -106,8 +108,11 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
     load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0;
     bool redo = false;
+    const int* th = a.track_hits + i;
+    int hid_next = stop_at > 0 ? th[0] : -1;                     // the hit id is fetched one step ahead
     for (int s = 0; s < stop_at; s++) {
-      const int hid = a.track_hits[(size_t)s * n + i];
+      const int hid = hid_next;
+      hid_next = s + 1 < stop_at ? th[(size_t)(s + 1) * n] : -1;
       if (hid < 0) continue;
       const LayerDev L = g.layers[g.plan_layers[p0 + s]];
       Hit H; load_hit(H, a.hits, hid);
