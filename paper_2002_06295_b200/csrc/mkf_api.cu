@@ -46,8 +46,11 @@ extern "C" int mkf_max_plan_len(const mkf_ctx* c) { return c ? c->max_plan_len :
 
 // ---- fit (a11 / C7): one thread per track, state and covariance in registers for the whole layer loop ----
 constexpr int FIT_BLOCK = 128;
+#ifndef MKF_FIT_MIN_BLOCKS
+#define MKF_FIT_MIN_BLOCKS 5
+#endif
 
-__global__ void __launch_bounds__(FIT_BLOCK) mkf_fit_kernel(const __grid_constant__ GeomDev g,
+__global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_kernel(const __grid_constant__ GeomDev g,
                                                             const __grid_constant__ ParamsDev p,
                                                             const __grid_constant__ FitArgs a) {
   const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
