@@ -75,6 +75,27 @@ def make_build_workload(which, seed, scale):
 
 
 # ---------------------------------------------------------------------------------------------------------------
+# ranks: events / tracks are independent, so a rank owns its own workload and nothing but timings is exchanged
+# ---------------------------------------------------------------------------------------------------------------
+def rank_seed(seed, rank):
+    """Seed of the workload a rank owns (weak scaling: every rank generates a full-size workload of its own)."""
+    return seed + rank
+
+
+def aggregate(ms_total, units, world, device):
+    """(max over ranks of the time, sum over ranks of the units). One all-reduce each; identity for world == 1."""
+    if world == 1:
+        return float(ms_total), float(units)
+    import torch
+    import torch.distributed as dist
+    mx = torch.tensor([ms_total], dtype=torch.float64, device=device)
+    sm = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+    dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+    return float(mx[0]), float(sm[0])
+
+
+# ---------------------------------------------------------------------------------------------------------------
 # clocks
 # ---------------------------------------------------------------------------------------------------------------
 class ClockSampler:
@@ -126,7 +147,7 @@ def oracle_fit_rate(geom, prm, hits, seeds, n_tracks, repeat=1):
     for _ in range(repeat):
         r = o.fit(*args)
     dt = (time.perf_counter() - t) / repeat
-    return float(r["nfit"].sum()) / dt, dt, o.num_threads(), int(r["nfit"].sum())
+    return float(r["nfit"].sum()) / dt, dt, o.num_threads(), int(r["nfit"].sum()), r
 
 
 def oracle_build_rate(ev, prm, n_events, dedup):
@@ -147,7 +168,7 @@ def oracle_build_rate(ev, prm, n_events, dedup):
         counts = np.bincount(s["event"][m], minlength=n_events)
         o.remove_duplicates(np.concatenate([[0], np.cumsum(counts)]).astype(np.int32), r["hit_ids"], r["nhits"], r["score"].astype(np.float32))
     dt = time.perf_counter() - t
-    return n_events / dt, dt, o.num_threads()
+    return n_events / dt, dt, o.num_threads(), r, m
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -185,7 +206,7 @@ def main():
             geom, prm, hits, seeds, _ = make_fit_workload(a.seed, n_s / 4000000.0)
             rates = []
             for k in range(warm + a.steps):
-                rate, dt, cores, steps = oracle_fit_rate(geom, prm, hits, seeds, n_s)
+                rate, dt, cores, steps, _ = oracle_fit_rate(geom, prm, hits, seeds, n_s)
                 if k >= warm:
                     rates.append((rate, dt))
             sample = "first %d helices of the workload per step (%d layer-steps)" % (n_s, steps)
@@ -196,7 +217,7 @@ def main():
             ev, prm = make_build_workload(which, a.seed, n_ev / nev_full)
             rates = []
             for k in range(warm + a.steps):
-                rate, dt, cores = oracle_build_rate(ev, prm, n_ev, which == 4)
+                rate, dt, cores, _, _ = oracle_build_rate(ev, prm, n_ev, which == 4)
                 if k >= warm:
                     rates.append((rate, dt))
             sample = "%d events of the workload per step" % n_ev
@@ -226,7 +247,7 @@ def main():
     pk = peaks()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if is_fit:
-        geom, prm, hits, seeds, _ = make_fit_workload(a.seed + rank, a.scale)
+        geom, prm, hits, seeds, _ = make_fit_workload(rank_seed(a.seed, rank), a.scale)
         ctx = B.Context(geom, prm)
         dh = B.hits_to_device(hits)
         ds = B.to_device(seeds, ["par", "cov", "q", "plan", "track_hits"])
@@ -244,7 +265,7 @@ def main():
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
     else:
         which = int(a.workload[-1])
-        ev, prm = make_build_workload(which, a.seed + rank, a.scale)
+        ev, prm = make_build_workload(which, rank_seed(a.seed, rank), a.scale)
         geom, hits, s = ev["geom"], ev["hits"], ev["seeds"]
         seeds = dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"])
         ctx = B.Context(geom, prm)
@@ -291,13 +312,7 @@ def main():
     ms_total = ev0.elapsed_time(ev1)
     u = units()
     clocks = sampler.stop(t0, t1) if sampler else None
-    tot = torch.tensor([ms_total, u], dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = tot.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = tot.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms_total, u_all = float(mx[0]), float(sm[1])
-    else:
-        u_all = u
+    ms_total, u_all = aggregate(ms_total, u, world, "cuda")
     ms_step = ms_total / a.steps
     value = u_all / (ms_step * 1e-3)
 
@@ -313,11 +328,7 @@ def main():
         eu, h2d, d2h = e2e_step()
     barrier()
     e2e_s = (time.perf_counter() - te) / a.e2e_steps
-    ee = torch.tensor([e2e_s, eu], dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = ee.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = ee.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        e2e_s, eu = float(mx[0]), float(sm[1])
+    e2e_s, eu = aggregate(e2e_s, eu, world, "cuda")
     e2e = dict(value=eu / e2e_s, unit=unit, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h), steps=a.e2e_steps,
                ms_per_step=1e3 * e2e_s, host_memory="pinned")
 
@@ -341,12 +352,28 @@ def main():
     if not a.no_cpu_baseline:
         if is_fit:
             n_s = min(n, 1000000)
-            rate, dt, cores, st = oracle_fit_rate(geom, prm, hits, seeds, n_s)
+            rate, dt, cores, st, r = oracle_fit_rate(geom, prm, hits, seeds, n_s)
             cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d helices of the workload (%d layer-steps, %.1f s)" % (n_s, st, dt))
+            # parity of the timed launch configuration on that same sample (the oracle results are already here)
+            from paper_2002_06295_b200 import parity
+            g = {k: out[k][..., :n_s].cpu().numpy() for k in ("par", "cov", "chi2", "nfit", "status")}
+            ok = r["nfit"] > 0
+            lay, kinds, pos = parity.last_layer_of_fit(geom, seeds["plan"][:n_s], seeds["track_hits"][:, :n_s], r["nfit"])
+            cpu["parity"] = dict(n=int(n_s), nfit_identical=bool(np.array_equal(g["nfit"], r["nfit"])),
+                                 status_identical=bool(np.array_equal(g["status"].view(np.uint32), r["status"])),
+                                 par_max=float(parity.param_errors(g["par"], r["par"], pos)[ok].max()),
+                                 cov_max=float(parity.cov_errors(g["cov"], r["cov"], r["par"], kinds)[ok].max()),
+                                 chi2_max=float(parity.chi2_errors(g["chi2"], r["chi2"])[ok].max()),
+                                 tol=dict(par=parity.TOL_PAR, cov=parity.TOL_COV, chi2=parity.TOL_CHI2))
         else:
             n_ev = min(nev, 4)
-            rate, dt, cores = oracle_build_rate(ev, prm, n_ev, dedup)
+            rate, dt, cores, r, m = oracle_build_rate(ev, prm, n_ev, dedup)
             cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d events of the workload (%.1f s)" % (n_ev, dt))
+            hid = out["hit_ids"].cpu().numpy()[:, m]
+            same = np.all(hid == r["hit_ids"], axis=0)
+            cpu["parity"] = dict(n=int(m.sum()), hit_lists_identical=float(same.mean()),
+                                 mismatches_with_margin_above_1e_3=int((r["margin"][~same] >= 1e-3).sum()),
+                                 chi2_max=float((np.abs(out["chi2"].cpu().numpy()[m] - r["chi2"]) / np.maximum(r["chi2"], 1.0))[same].max()))
     print(json.dumps(dict(metric=metric, value=value, unit=unit, n_gpus=world, steps=a.steps, warmup=warm, ms_per_step=ms_step,
                           higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic", config=cfg,
                           clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, cpu_baseline=cpu, impl="mkf",

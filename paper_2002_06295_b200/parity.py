@@ -1,4 +1,4 @@
-"""Parity metrics between a float32 result and the float64 oracle result (tolerances of BASELINE.json north_star,
+"""Parity metrics between a float32 result and a float64 reference result (tolerances of BASELINE.json north_star,
 made precise by readings U19/U20 of DESIGN.md §3). Pure numpy; used by the -m gpu tests and by bench.py's checks."""
 import numpy as np
 

@@ -5,7 +5,7 @@ import pytest
 
 from oracle import mkfo
 from paper_2002_06295_b200 import datagen
-import parity
+from paper_2002_06295_b200 import parity
 
 pytestmark = pytest.mark.gpu
 
