@@ -193,6 +193,8 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
         cov_aa(S, tt, tz, zz);
         int e0, e1, w0, wn;
         window(g, L, p.chi2_cut, S, tt, zz, a.vmax[2 * seg], a.vmax[2 * seg + 1], e0, e1, w0, wn);
+        const float lim1 = p.chi2_cut * (tt + a.vmax[2 * seg]) * 1.0001f;
+        const float lim2 = p.chi2_cut * (zz + (L.kind == 0 ? a.vmax[2 * seg + 1] : a.vmax[2 * seg])) * 1.0001f;
         const unsigned* boff = a.bin_off + seg * (size_t)nb;
         for (int ie = e0; ie <= e1; ie++) {
           const unsigned* row = boff + ie * g.n_phi;
@@ -203,8 +205,15 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
             else { if (w0 + wn <= g.n_phi) break; tb = row[0]; te = row[w0 + wn - g.n_phi]; }
             for (unsigned t = tb; t < te; t++) {
               Hit H; int id;
-              if (a.packed) load_packed(H, id, a.packed + (size_t)3 * t);
-              else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
+              if (a.packed) {
+                // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11),
+                // so most hits of the padded bins are rejected before their covariance is read
+                const float4 q0 = __ldg(a.packed + (size_t)3 * t);
+                const float rx = (q0.x - S.x) - S.xl, ry = (q0.y - S.y) - S.yl, rz = (q0.z - S.z) - S.zl;
+                const float r1 = S.f.kind == 0 ? S.f.cb * ry - S.f.sb * rx : rx, r2 = S.f.kind == 0 ? rz : ry;
+                if (r1 * r1 > lim1 || r2 * r2 > lim2) continue;
+                load_packed(H, id, a.packed + (size_t)3 * t);
+              } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
               SInv o; float c2;
               if (!chi2_local(S, tt, tz, zz, H, o, c2)) continue;
               if (c2 < p.chi2_cut) {
