@@ -95,7 +95,10 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
     _Pragma("unroll") for (int k_ = 0; k_ < 5; k_++) S.d[k_] = __shfl_sync(gm, S.d[k_], src);              \
   } while (0)
 
-__global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_constant__ GeomDev g,
+#ifndef MKF_BUILD_MIN_BLOCKS
+#define MKF_BUILD_MIN_BLOCKS 8
+#endif
+__global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
                                                                 const __grid_constant__ ParamsDev p,
                                                                 const __grid_constant__ BuildArgs a) {
   extern __shared__ unsigned trellis_all[];                  // [seed in CTA][step][slot]
@@ -203,12 +206,16 @@ __global__ void __launch_bounds__(BUILD_BLOCK) mkf_build_kernel(const __grid_con
             unsigned tb, te;
             if (part == 0) { tb = row[w0]; te = row[min(w0 + wn, g.n_phi)]; }
             else { if (w0 + wn <= g.n_phi) break; tb = row[0]; te = row[w0 + wn - g.n_phi]; }
+            float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (a.packed && tb < te) qn = __ldg(a.packed + (size_t)3 * tb);
             for (unsigned t = tb; t < te; t++) {
               Hit H; int id;
               if (a.packed) {
                 // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11),
-                // so most hits of the padded bins are rejected before their covariance is read
-                const float4 q0 = __ldg(a.packed + (size_t)3 * t);
+                // so most hits of the padded bins are rejected before their covariance is read; the next record's
+                // position is already in flight
+                const float4 q0 = qn;
+                if (t + 1 < te) qn = __ldg(a.packed + (size_t)3 * (t + 1));
                 const float rx = (q0.x - S.x) - S.xl, ry = (q0.y - S.y) - S.yl, rz = (q0.z - S.z) - S.zl;
                 const float r1 = S.f.kind == 0 ? S.f.cb * ry - S.f.sb * rx : rx, r2 = S.f.kind == 0 ? rz : ry;
                 if (r1 * r1 > lim1 || r2 * r2 > lim2) continue;
