@@ -45,7 +45,10 @@ extern "C" long long mkf_launch_count(const mkf_ctx* c) { return c ? c->launches
 extern "C" int mkf_max_plan_len(const mkf_ctx* c) { return c ? c->max_plan_len : 0; }
 
 // ---- fit (a11 / C7): one thread per track, state and covariance in registers for the whole layer loop ----
-constexpr int FIT_BLOCK = 128;
+#ifndef MKF_FIT_BLOCK
+#define MKF_FIT_BLOCK 128
+#endif
+constexpr int FIT_BLOCK = MKF_FIT_BLOCK;
 #ifndef MKF_FIT_MIN_BLOCKS
 #define MKF_FIT_MIN_BLOCKS 5
 #endif

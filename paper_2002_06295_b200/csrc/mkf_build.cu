@@ -47,7 +47,7 @@ __device__ __forceinline__ void load_packed(Hit& H, int& id, const float4* __res
   H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = c.x; H.v[5] = c.y;
 }
 
-// U11: window of bins that contains every hit with chi2 < cut (fp32, one extra bin of padding on every side).
+// U11: window of bins that contains every hit with chi2 < cut.
 __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, float cut, const KState& S,
                                        float tt, float zz_or_yy, float vxy, float vzz, int& e0, int& e1, int& p0, int& np) {
   const float x = S.x + S.xl, y = S.y + S.yl, z = S.z + S.zl;
@@ -69,15 +69,17 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
     const float ea = asinhf(L.pos / rlo), eb = asinhf(L.pos / rhi);
     eta_a = fminf(ea, eb); eta_b = fmaxf(ea, eb);
   }
-  dphi = dphi * (1.f + 1e-5f) + 1e-5f;
+  // The (dphi, eta) box is already a proven superset of {chi2 < cut} (U11); it only needs margins for the fp32
+  // evaluation of its edges against the fp64 bin keys of the hits (C8), not whole extra bins.
+  dphi = dphi * (1.f + 1e-4f) + 2e-5f;
   const float esc = (float)g.n_eta / (L.eta_hi - L.eta_lo);
-  int ia = (int)floorf((eta_a - L.eta_lo) * esc), ib = (int)floorf((eta_b - L.eta_lo) * esc);
-  ia = min(max(ia, 0), g.n_eta - 1); ib = min(max(ib, 0), g.n_eta - 1);
-  e0 = max(0, ia - 1); e1 = min(g.n_eta - 1, ib + 1);
+  const float em = 2e-5f + 1e-5f * fmaxf(fabsf(eta_a), fabsf(eta_b));
+  int ia = (int)floorf((eta_a - em - L.eta_lo) * esc), ib = (int)floorf((eta_b + em - L.eta_lo) * esc);
+  e0 = min(max(ia, 0), g.n_eta - 1); e1 = min(max(ib, 0), g.n_eta - 1);
   if (!(dphi < PI_F)) { p0 = 0; np = g.n_phi; return; }
   const float ibw = (float)g.n_phi * (1.f / (2.f * PI_F));
-  const int a = (int)floorf((php - dphi + PI_F) * ibw) - 1;
-  const int b = (int)floorf((php + dphi + PI_F) * ibw) + 1;
+  const int a = (int)floorf((php - dphi + PI_F) * ibw);
+  const int b = (int)floorf((php + dphi + PI_F) * ibw);
   const int cnt = b - a + 1;
   if (cnt >= g.n_phi) { p0 = 0; np = g.n_phi; return; }
   p0 = ((a % g.n_phi) + g.n_phi) % g.n_phi; np = cnt;
