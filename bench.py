@@ -25,6 +25,9 @@ sys.path.insert(0, ROOT)
 ALGO_FLOP_PER_LAYER_STEP = 1000.0        # DESIGN.md §6 (SURVEY.md §8 d): propagate 150 + transport 420 + material 90 + update 340
 ALGO_BYTES_PER_LAYER_STEP = 54.0         # hit 36 B + index 4 B + state in/out amortised 14 B
 FP32_LANES_PER_SM, N_SM = 128, 148
+# dram__bytes_read.sum + dram__bytes_write.sum of one mkf_fit_kernel launch on the full configs[1] workload, from
+# the `ncu --set full` capture summarised in profiles/r1_fit_kernel_ncu.md (3.1226 GB + 0.5044 GB)
+NCU_TRAFFIC_BYTES_FIT_FULL = 3.627e9
 
 
 def peaks():
@@ -340,7 +343,8 @@ def main():
         t_launch = ms_total / a.steps * 1e-3
         ach = ALGO_FLOP_PER_LAYER_STEP * steps_per_launch / t_launch / 1e12
         roof = dict(bound="alu", kernel="mkf_fit_kernel", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
-                    traffic=None, peak_source="148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (%s max clock)" % (pk["sm_max_mhz"], pk["source"]),
+                    traffic=NCU_TRAFFIC_BYTES_FIT_FULL if a.scale == 1.0 else None,
+                    algorithmic_bytes=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch, peak_source="148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (%s max clock)" % (pk["sm_max_mhz"], pk["source"]),
                     algorithmic_flop_per_layer_step=ALGO_FLOP_PER_LAYER_STEP,
                     hbm=dict(achieved=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
                              frac=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9 / pk["hbm_gbs"]))
