@@ -4,8 +4,8 @@
 //
 // Mapping: 8 lanes of a warp own one seed (4 seeds per warp); lane k holds live candidate k (rank order) with its
 // state and covariance in registers. Per layer: every live lane propagates its candidate (a2-a4), scans the
-// phi/eta bins of its window (a5) reading the 48-byte packed hit records, keeps its own best MAX_CAND hits by
-// chi2 in a register-resident sorted list (a6); the group then picks the top max_cand children of the whole seed
+// phi/eta bins of its window (a5) reading the 48-byte packed hit records (position first: most are rejected before
+// their covariance is read), keeps its own best MAX_CAND hits by chi2 in a sorted list in shared memory (a6); the group then picks the top max_cand children of the whole seed
 // with 8-lane shuffle tournaments under the total order U14 (a8), the winners fetch their parent's state with
 // shuffles and update it (a7). The hit lists are a trellis in shared memory (per step and slot: hit id and
 // parent slot), so cloning a candidate costs one 4-byte entry; the winner's list is read back at the end.
@@ -114,6 +114,9 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
   const size_t n = (size_t)a.n;
   const int mpl = a.max_plan_len;
   unsigned* trellis = trellis_all + (size_t)seed_in_cta * mpl * G;
+  // per-thread list of accepted hits of the current layer, [k][thread] (bank-conflict free): chi2, hit id
+  float* hc2 = reinterpret_cast<float*>(trellis_all + (size_t)(BUILD_BLOCK / G) * mpl * G) + threadIdx.x;
+  int* hid = reinterpret_cast<int*>(hc2 - threadIdx.x + G * BUILD_BLOCK) + threadIdx.x;
   const int nb = g.n_phi * g.n_eta;
 
   // ---- seed phase: slot 0 fits the seed through its own three hits (U18b) --------------------------------
@@ -180,10 +183,7 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
     const size_t seg = (size_t)ev * g.n_layers + lay;
 
     // ---- each live lane: propagate, scan its window, keep its own best hits ------------------------------
-    float lc2[G]; int lid[G];
-#pragma unroll
-    for (int k = 0; k < G; k++) { lc2[k] = INFINITY; lid[k] = HIT_NONE; }
-    int n_hitc = 0;                       // hit children available in lc2/lid
+    int n_hitc = 0, head = 0;             // accepted hits in hc2/hid (sorted), next one to offer
     bool miss_avail = false, pass_avail = false;
     bool offer = false; int offer_phase = 0; float offer_score = 0.f; int offer_nm = 0;
     if (live) {
@@ -226,13 +226,20 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
               SInv o; float c2;
               if (!chi2_local(S, tt, tz, zz, H, o, c2)) continue;
               if (c2 < p.chi2_cut) {
-                n_hitc = min(n_hitc + 1, G);
-                float v = c2; int vid = id;
-#pragma unroll
-                for (int k = 0; k < G; k++) {
-                  const bool sw = v < lc2[k] || (v == lc2[k] && vid < lid[k]);
-                  const float tv = lc2[k]; const int ti = lid[k];
-                  if (sw) { lc2[k] = v; lid[k] = vid; v = tv; vid = ti; }
+                // kept sorted by (chi2, id) in shared memory: lists are short (1-2 entries on average), so the
+                // insertion is a handful of divergent instructions and no register array is needed
+                int k = n_hitc;
+                if (n_hitc == G) {
+                  const float wv = hc2[(G - 1) * BUILD_BLOCK]; const int wi = hid[(G - 1) * BUILD_BLOCK];
+                  k = (c2 < wv || (c2 == wv && id < wi)) ? G - 1 : -1;
+                } else n_hitc++;
+                if (k >= 0) {
+                  while (k > 0) {
+                    const float pv = hc2[(k - 1) * BUILD_BLOCK]; const int pi = hid[(k - 1) * BUILD_BLOCK];
+                    if (!(c2 < pv || (c2 == pv && id < pi))) break;
+                    hc2[k * BUILD_BLOCK] = pv; hid[k * BUILD_BLOCK] = pi; k--;
+                  }
+                  hc2[k * BUILD_BLOCK] = c2; hid[k * BUILD_BLOCK] = id;
                 }
               }
             }
@@ -273,7 +280,7 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
     int n_new = 0;
     for (int r = 0; r < p.max_cand; r++) {
       float hs, hc; int hh, hk;                               // head child of this lane
-      if (n_hitc > 0) { hs = base_hit - lc2[0]; hc = chi2 + lc2[0]; hh = lid[0]; hk = 0; }
+      if (head < n_hitc) { const float c2h = hc2[head * BUILD_BLOCK]; hs = base_hit - c2h; hc = chi2 + c2h; hh = hid[head * BUILD_BLOCK]; hk = 0; }
       else if (miss_avail) { hs = sc_miss; hc = chi2; hh = HIT_NONE; hk = 1; }
       else if (pass_avail) { hs = sc_pass; hc = chi2; hh = HIT_NONE; hk = 2; }
       else { hs = -INFINITY; hc = INFINITY; hh = HIT_NONE; hk = 3; }
@@ -287,9 +294,7 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
       if (!(ws > -INFINITY)) break;                           // pool exhausted (uniform in the group)
       if (sub == wp) {                                        // the winner lane pops its head
         if (wk == 0) {
-#pragma unroll
-          for (int k = 0; k < G - 1; k++) { lc2[k] = lc2[k + 1]; lid[k] = lid[k + 1]; }
-          lc2[G - 1] = INFINITY; lid[G - 1] = HIT_NONE; n_hitc--;
+          head++;
         } else if (wk == 1) miss_avail = false;
         else pass_avail = false;
       }
@@ -378,7 +383,9 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
 }  // namespace
 
 namespace mkf {
-size_t build_smem_bytes(int max_plan_len) { return (size_t)(BUILD_BLOCK / G) * max_plan_len * G * sizeof(unsigned); }
+size_t build_smem_bytes(int max_plan_len) {
+  return (size_t)(BUILD_BLOCK / G) * max_plan_len * G * sizeof(unsigned) + (size_t)2 * G * BUILD_BLOCK * sizeof(float);
+}
 }
 
 extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
