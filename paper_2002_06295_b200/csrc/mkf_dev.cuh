@@ -109,10 +109,11 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
     c2tot = 0.f; nf = 0;
     bool redo = false;
     const int* th = a.track_hits + i;
-    int hid_next = stop_at > 0 ? th[0] : -1;                     // the hit id is fetched one step ahead
+    int hid_next = stop_at > 0 ? *th : -1;                       // the hit id is fetched one step ahead
     for (int s = 0; s < stop_at; s++) {
       const int hid = hid_next;
-      hid_next = s + 1 < stop_at ? th[(size_t)(s + 1) * n] : -1;
+      th += n;
+      hid_next = s + 1 < stop_at ? *th : -1;
       if (hid < 0) continue;
       const LayerDev L = g.layers[g.plan_layers[p0 + s]];
       Hit H; load_hit(H, a.hits, hid);
