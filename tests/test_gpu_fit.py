@@ -117,3 +117,33 @@ def test_fit_host_entry_point_matches_device_path():
     n = s["par"].shape[1]
     assert r["d2h_bytes"] == n * (27 * 4 + 12) and r["h2d_bytes"] > n * 27 * 4
     ctx.close()
+
+
+def test_fit_quarter_of_configs1_in_bench_launch_configuration_sampled():
+    """1 M helices (a quarter of configs[1], generated exactly as bench.py does, same launch configuration: 7813 CTAs
+    of 128 threads); the oracle checks a sample of 60 000 tracks taken across the whole range."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    from gpu_helpers import gpu_fit
+    geom, prm, hits, seeds, _ = bench.make_fit_workload(3, 0.25)
+    n = seeds["par"].shape[1]
+    assert n == 1000000
+    h = gpu_fit(dict(geom=geom, hits=hits), prm, seeds)
+    sel = np.sort(np.random.default_rng(0).choice(n, 60000, replace=False))
+    sub = {k: np.ascontiguousarray(v[..., sel]) for k, v in seeds.items()}
+    r = mkfo.Oracle(geom, prm).fit(hits, sub["par"], sub["cov"], sub["q"], sub["plan"], sub["track_hits"])
+    assert np.array_equal(h["nfit"][sel], r["nfit"]) and np.array_equal(h["status"][sel], r["status"])
+    ok = r["nfit"] > 0
+    lay, kinds, pos = parity.last_layer_of_fit(geom, sub["plan"], sub["track_hits"], r["nfit"])
+    assert parity.param_errors(h["par"][:, sel], r["par"], pos)[ok].max() <= parity.TOL_PAR
+    assert parity.cov_errors(h["cov"][:, sel], r["cov"], r["par"], kinds)[ok].max() <= parity.TOL_COV
+    assert parity.chi2_errors(h["chi2"][sel], r["chi2"])[ok].max() <= parity.TOL_CHI2
+    # property that holds at any size: every track ends on the layer of its last fitted hit (the update moves the
+    # point along the tangent plane, so the radius may exceed the layer's by shift^2 / 2R)
+    R = np.hypot(h["par"][0], h["par"][1])
+    radii = np.array([l["pos"] for l in geom["layers"]])
+    fitted = h["nfit"] > 0
+    dR = R[fitted] - radii[h["nfit"][fitted] - 1]
+    assert dR.min() > -2e-5 * 110 and dR.max() < 0.1 and np.quantile(np.abs(dR), 0.99) < 1e-3
+    assert np.isfinite(h["chi2"]).all() and np.isfinite(h["cov"]).all()
