@@ -4,7 +4,7 @@
 //
 // Mapping: 8 lanes of a warp own one seed (4 seeds per warp); lane k holds live candidate k (rank order) with its
 // state and covariance in registers. Per layer: every live lane propagates its candidate (a2-a4), scans the
-// phi/eta bins of its window (a5) reading the 48-byte packed hit records (position first: most are rejected before
+// phi/eta bins of its window (a5) reading the packed hit records (16-byte positions first: most are rejected before
 // their covariance is read), keeps its own best MAX_CAND hits by chi2 in a sorted list in shared memory (a6); the group then picks the top max_cand children of the whole seed
 // with 8-lane shuffle tournaments under the total order U14 (a8), the winners fetch their parent's state with
 // shuffles and update it (a7). The hit lists are a trellis in shared memory (per step and slot: hit id and
@@ -41,8 +41,8 @@ __device__ __forceinline__ bool before(float sa, float ca, int pa, int ha, float
   return ha < hb;
 }
 
-__device__ __forceinline__ void load_packed(Hit& H, int& id, const float4* __restrict__ rec) {
-  const float4 a = __ldg(rec), b = __ldg(rec + 1), c = __ldg(rec + 2);
+__device__ __forceinline__ void load_packed(Hit& H, int& id, const float4 a, const float4* __restrict__ cov) {
+  const float4 b = __ldg(cov), c = __ldg(cov + 1);
   H.x = a.x; H.y = a.y; H.z = a.z; id = __float_as_int(a.w);
   H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = c.x; H.v[5] = c.y;
 }
@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
             if (part == 0) { tb = row[w0]; te = row[min(w0 + wn, g.n_phi)]; }
             else { if (w0 + wn <= g.n_phi) break; tb = row[0]; te = row[w0 + wn - g.n_phi]; }
             float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (a.packed && tb < te) qn = __ldg(a.packed + (size_t)3 * tb);
+            if (a.packed && tb < te) qn = __ldg(a.packed + tb);
             for (unsigned t = tb; t < te; t++) {
               Hit H; int id;
               if (a.packed) {
@@ -217,11 +217,11 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
                 // so most hits of the padded bins are rejected before their covariance is read; the next record's
                 // position is already in flight
                 const float4 q0 = qn;
-                if (t + 1 < te) qn = __ldg(a.packed + (size_t)3 * (t + 1));
+                if (t + 1 < te) qn = __ldg(a.packed + t + 1);
                 const float rx = (q0.x - S.x) - S.xl, ry = (q0.y - S.y) - S.yl, rz = (q0.z - S.z) - S.zl;
                 const float r1 = S.f.kind == 0 ? S.f.cb * ry - S.f.sb * rx : rx, r2 = S.f.kind == 0 ? rz : ry;
                 if (r1 * r1 > lim1 || r2 * r2 > lim2) continue;
-                load_packed(H, id, a.packed + (size_t)3 * t);
+                load_packed(H, id, q0, a.packed + (size_t)a.hits.n_hits + (size_t)2 * t);
               } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
               SInv o; float c2;
               if (!chi2_local(S, tt, tz, zz, H, o, c2)) continue;

@@ -7,7 +7,8 @@
 //   3. hi_place     : scatter hit ids to their bins (atomic cursor);
 //   4. hi_sort_bins : each bin's ids sorted ascending -> the order is the unique stable order (C8) whatever
 //                     order the atomics ran in;
-//   5. hi_pack      : 48-byte records of the hits in sorted order, so that a bin scan reads contiguous memory.
+//   5. hi_pack      : the hits in sorted order, positions (16 B) and covariances (32 B) in two contiguous blocks,
+//                     so that a bin scan reads contiguous memory.
 // HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
 #include "mkf_ctx.h"
 #include "mkf_scan.cuh"
@@ -122,10 +123,12 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
   const int id = a.sorted_id[t];
   const size_t nh = (size_t)a.hits.n_hits;
   const float* V = a.hits.V;
-  float4* o = a.packed + (size_t)3 * t;
-  o[0] = make_float4(a.hits.x[id], a.hits.y[id], a.hits.z[id], __int_as_float(id));
-  o[1] = make_float4(V[id], V[nh + id], V[2 * nh + id], V[3 * nh + id]);
-  o[2] = make_float4(V[4 * nh + id], V[5 * nh + id], 0.f, 0.f);
+  // positions first (16 B per hit, what the window scan reads for every hit), covariances behind them (32 B per
+  // hit, read only for the hits that survive the position test)
+  a.packed[t] = make_float4(a.hits.x[id], a.hits.y[id], a.hits.z[id], __int_as_float(id));
+  float4* o = a.packed + nh + (size_t)2 * t;
+  o[0] = make_float4(V[id], V[nh + id], V[2 * nh + id], V[3 * nh + id]);
+  o[1] = make_float4(V[4 * nh + id], V[5 * nh + id], 0.f, 0.f);
 }
 
 }  // namespace

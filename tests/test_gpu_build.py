@@ -18,13 +18,14 @@ def check_index(ev, prm):
     assert np.array_equal(got["bin_off"], ref["bin_off"])
     assert np.array_equal(got["sorted_id"], ref["sorted_id"])
     assert np.array_equal(got["vmax"].view(np.uint32), ref["vmax"].view(np.uint32))     # bit-exact floats
-    # packed records are the hits in sorted order
-    pk = got["packed"].reshape(-1, 12)
+    # packed copy: the hits in sorted order, positions then covariances
     sid = ref["sorted_id"]
     h = ev["hits"]
-    assert np.array_equal(pk[:, 3].copy().view(np.int32), sid)
-    assert np.array_equal(pk[:, 0], h["x"][sid]) and np.array_equal(pk[:, 2], h["z"][sid])
-    assert np.array_equal(pk[:, 4:10], h["V"][:, sid].T)
+    nh = len(sid)
+    pos, cv = got["packed"][:4 * nh].reshape(nh, 4), got["packed"][4 * nh:].reshape(nh, 8)
+    assert np.array_equal(pos[:, 3].copy().view(np.int32), sid)
+    assert np.array_equal(pos[:, 0], h["x"][sid]) and np.array_equal(pos[:, 1], h["y"][sid]) and np.array_equal(pos[:, 2], h["z"][sid])
+    assert np.array_equal(cv[:, :6], h["V"][:, sid].T)
     return ref
 
 
