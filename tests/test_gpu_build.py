@@ -183,3 +183,99 @@ def test_build_host_entry_point_matches_device_path():
     for k in ("hit_ids", "nhits", "nmiss", "chi2", "score", "par", "cov", "keep"):
         assert np.array_equal(r[k], h[k]), k
     ctx.close()
+
+
+def test_fit_of_built_tracks_chained_from_build_output():
+    """PAPER.md:25 'Fitting simply applies the KF procedure to all hits identified during building': the hit_ids
+    array written by mkf_build_tracks is the track_hits input of mkf_fit as it is (-1 / -2 entries are skipped)."""
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    from gpu_helpers import gpu_build
+    ev, prm = datagen.config(3, scale=0.01)
+    s = ev["seeds"]
+    hb = gpu_build(ev, prm)
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    sd = B.to_device(dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"]), ["par", "cov", "q", "plan"])
+    th = torch.from_numpy(hb["hit_ids"]).cuda()
+    n = s["par"].shape[1]
+    out = B.alloc_fit_out(n)
+    ctx.fit(hits, sd, sd["plan"], th, out, out["chi2"], out["nfit"], out["status"])
+    torch.cuda.synchronize()
+    g = {k: v.cpu().numpy() for k, v in out.items()}
+    r = mkfo.Oracle(ev["geom"], prm).fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], hb["hit_ids"])
+    assert np.array_equal(g["nfit"], r["nfit"]) and np.array_equal(g["status"].view(np.uint32), r["status"])
+    ok = (r["nfit"] > 0)
+    # a built track without missed layers is fitted through exactly the same sequence of steps, so the total chi2
+    # agrees with the build's (with a miss the build also applied the material of the missed layer; the fit,
+    # which goes from hit to hit, does not)
+    full = ok & (g["nfit"] == hb["nhits"]) & ((hb["status"] & 32) == 0) & (hb["nmiss"] == 0)
+    assert full.mean() > 0.3
+    lay, kinds, pos = parity.last_layer_of_fit(ev["geom"], s["plan"], hb["hit_ids"], r["nfit"])
+    assert parity.param_errors(g["par"], r["par"], pos)[ok].max() <= parity.TOL_PAR
+    assert parity.cov_errors(g["cov"], r["cov"], r["par"], kinds)[ok].max() <= parity.TOL_COV
+    assert parity.chi2_errors(g["chi2"], r["chi2"])[ok].max() <= parity.TOL_CHI2
+    assert (np.abs(g["chi2"][full] - hb["chi2"][full]) <= 1e-3 * np.maximum(hb["chi2"][full], 1.0)).all()
+    ctx.close()
+
+
+def test_degenerate_inputs():
+    """No seeds, events without hits, seeds whose hits are not on their plan, no tracks for duplicate removal."""
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    g = datagen.geometry_barrel(6, 4.0, 24.0, 50.0, 0.02)
+    prm = datagen.default_params()
+    ev = datagen.make_events(g, 5, 2, 40, n_noise=600)
+    o = mkfo.Oracle(g, prm)
+    # event 1 emptied: all its hits removed
+    h = ev["hits"]
+    lo = h["layer_off"].reshape(2, 7)
+    n0 = int(lo[0, 6])
+    sub = dict(n_events=2, layer_off=np.concatenate([lo[0], np.full(7, n0)]).astype(np.int32), x=h["x"][:n0].copy(), y=h["y"][:n0].copy(),
+               z=h["z"][:n0].copy(), V=np.ascontiguousarray(h["V"][:, :n0]))
+    from gpu_helpers import gpu_hit_index
+    ref = o.build_hit_index(sub)
+    got = gpu_hit_index(dict(geom=g, hits=sub), prm)
+    assert np.array_equal(got["bin_off"], ref["bin_off"]) and np.array_equal(got["sorted_id"], ref["sorted_id"])
+    assert np.array_equal(got["vmax"], ref["vmax"]) and np.all(got["vmax"][12:] == 0)
+    # seeds of event 0 only; the last seed gets hits that are not in plan order -> TRUNCATED seed returned
+    s = ev["seeds"]
+    m = s["event"] == 0
+    seeds = {k: np.ascontiguousarray(v[..., m]) for k, v in s.items() if k in ("par", "cov", "q", "plan", "event", "hits")}
+    seeds["hits"][:, -1] = seeds["hits"][::-1, -1]
+    r = o.build_tracks(sub, ref, seeds["par"], seeds["cov"], seeds["q"], seeds["event"], seeds["hits"], seeds["plan"])
+    ctx = B.Context(g, prm)
+    dh = B.hits_to_device(sub)
+    idx, ws = B.alloc_hit_index(ctx, 2, n0)
+    ctx.build_hit_index(dh, idx, ws)
+    sd = B.to_device(seeds, ["par", "cov", "q", "plan", "event", "hits"])
+    n = seeds["par"].shape[1]
+    out = B.alloc_build_out(n, ctx.max_plan_len)
+    ctx.build_tracks(dh, idx, sd, sd["event"], sd["hits"], sd["plan"], out, out["chi2"], out["score"], out["nhits"], out["nmiss"],
+                     out["hit_ids"], out["status"])
+    torch.cuda.synchronize()
+    hid = out["hit_ids"].cpu().numpy()
+    same = np.all(hid == r["hit_ids"], axis=0)
+    assert same.mean() >= 0.97 and np.all(r["margin"][~same] < 1e-3)
+    st = out["status"].cpu().numpy().view(np.uint32)
+    assert np.array_equal(st[same], r["status"][same]) and (r["status"][-1] & 32) and same[-1]
+    assert np.array_equal(out["nhits"].cpu().numpy()[same], r["nhits"][same])
+    # zero seeds: nothing launched
+    e = {k: v[..., :0].contiguous() for k, v in sd.items()}
+    out0 = B.alloc_build_out(0, ctx.max_plan_len)
+    before = ctx.launch_count()
+    ctx.build_tracks(dh, idx, e, e["event"], e["hits"], e["plan"], out0, out0["chi2"], out0["score"], out0["nhits"], out0["nmiss"],
+                     out0["hit_ids"], out0["status"])
+    assert ctx.launch_count() == before
+    # duplicate removal with an event that has no tracks
+    toff = torch.tensor([0, n, n], dtype=torch.int32, device="cuda")
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda"); nk = torch.empty(2, dtype=torch.int32, device="cuda")
+    ws2 = torch.empty(ctx.workspace_bytes(B.CALL_REMOVE_DUPLICATES, 2, n0, n), dtype=torch.uint8, device="cuda")
+    ctx.remove_duplicates(n0, toff, out["hit_ids"], out["nhits"], out["score"], keep, nk, ws2)
+    torch.cuda.synchronize()
+    d = o.remove_duplicates(np.array([0, n, n], np.int32), hid, out["nhits"].cpu().numpy(), out["score"].cpu().numpy())
+    assert np.array_equal(keep.cpu().numpy(), d["keep"]) and np.array_equal(nk.cpu().numpy(), d["n_kept"]) and nk[1].item() == 0
+    # workspace too small is an error code, not a crash
+    with pytest.raises(B.MkfError):
+        ctx.remove_duplicates(n0, toff, out["hit_ids"], out["nhits"], out["score"], keep, nk, ws2[:64])
+    ctx.close()
