@@ -41,7 +41,8 @@ void helix_step(double bz, int q, const double* u, double s, double* u1) {
 
 // C2: transverse path to the cylinder r = R by circle-circle intersection; exit point (outward radial velocity).
 // C3: path to the plane z = Z.  Returns false if unreachable (U5, U6).
-bool path_to_surface(int kind, double pos, double bz, int q, const double* u, double* s_out) {
+// dir = +1: forward (outward) step; dir = -1: backward step, s <= 0 (reading R7).
+bool path_to_surface(int kind, double pos, double bz, int q, const double* u, double* s_out, int dir = 1) {
   double w = -q * KAPPA * bz * u[IIPT];
   double s;
   if (kind == 1) {
@@ -81,7 +82,8 @@ bool path_to_surface(int kind, double pos, double bz, int q, const double* u, do
       s = best_s;                                                // may be < 0: wrapped principal value
     }
   }
-  if (s < -S_BACK) return false;                                 // backward, or forward arc >= pi (U5/U6)
+  if (dir > 0 && s < -S_BACK) return false;                      // backward, or forward arc >= pi (U5/U6)
+  if (dir < 0 && s > S_BACK) return false;                       // R7: the same rule mirrored
   if (std::fabs(w * s) >= PI) return false;                      // U6
   *s_out = s;
   return true;
@@ -122,9 +124,9 @@ void fcft(const double* F, const double* C, double* out) {
     double m = 0.5 * (out[i * 6 + j] + out[j * 6 + i]); out[i * 6 + j] = out[j * 6 + i] = m; }
 }
 
-int propagate(int kind, double pos, double bz, const State& in, State& out, double* F_out, double* s_out) {
+int propagate(int kind, double pos, double bz, const State& in, State& out, double* F_out, double* s_out, int dir = 1) {
   double s;
-  if (!path_to_surface(kind, pos, bz, in.q, in.u, &s)) return MKFO_PROP_UNREACHABLE;
+  if (!path_to_surface(kind, pos, bz, in.q, in.u, &s, dir)) return MKFO_PROP_UNREACHABLE;
   helix_step(bz, in.q, in.u, s, out.u);
   double F[36];
   jacobian(kind, pos, bz, in.q, in.u, out.u, s, F);
@@ -152,7 +154,9 @@ double highland(double p, double t) {
   return 0.0136 / (beta * p) * std::sqrt(t) * (1.0 + 0.038 * std::log(t));
 }
 
-int material(int kind, double xx0, int flags, double* u, double* C, double* th0_out, double* dE_out) {
+// dir = -1 (R7): the layer is crossed against the particle's motion: the mean energy loss is given back, the
+// scattering noise is added all the same; both are evaluated with the momentum the state arrives with.
+int material(int kind, double xx0, int flags, double* u, double* C, double* th0_out, double* dE_out, int dir = 1) {
   if (th0_out) *th0_out = 0; if (dE_out) *dE_out = 0;
   if (!(xx0 > 0) || (flags & 3) == 0) return 0;
   double st = std::sin(u[ITH]), ct = std::cos(u[ITH]);
@@ -167,7 +171,7 @@ int material(int kind, double xx0, int flags, double* u, double* C, double* th0_
   double th0 = highland(p, t);                                   // with p before the energy loss
   if (flags & 2) {
     double dE = dedx(p) * t * SI_X0;
-    double E1 = E - dE;
+    double E1 = dir > 0 ? E - dE : E + dE;
     if (dE_out) *dE_out = dE;
     if (E1 <= m) return MKFO_STOPPED_ELOSS;
     double p1 = std::sqrt(E1 * E1 - m * m), beta1 = p1 / E1;
@@ -369,6 +373,19 @@ int mkfo_propagate(int kind, double pos, double bz, int q, const double* u, cons
 int mkfo_material(int kind, double xx0, int flags, double* u, double* C, double* theta0_out, double* dE_out) {
   return material(kind, xx0, flags, u, C, theta0_out, dE_out);
 }
+int mkfo_propagate_dir(int kind, double pos, double bz, int q, int dir, const double* u, const double* C, double* u1,
+                       double* F, double* C1, double* s) {
+  State in, out; std::memcpy(in.u, u, sizeof(in.u)); in.q = q;
+  if (C) std::memcpy(in.C, C, sizeof(in.C)); else std::memset(in.C, 0, sizeof(in.C));
+  int rc = propagate(kind, pos, bz, in, out, F, s, dir);
+  if (rc) return rc;
+  std::memcpy(u1, out.u, sizeof(out.u));
+  if (C1) std::memcpy(C1, out.C, sizeof(out.C));
+  return 0;
+}
+int mkfo_material_dir(int kind, double xx0, int flags, int dir, double* u, double* C, double* theta0_out, double* dE_out) {
+  return material(kind, xx0, flags, u, C, theta0_out, dE_out, dir);
+}
 double mkfo_dedx(double p) { return dedx(p); }
 double mkfo_highland(double p, double t) { return highland(p, t); }
 
@@ -446,6 +463,60 @@ int mkfo_fit(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, i
       if (rc) { stat |= (unsigned)rc; break; }
       if (has_nan(nx)) { stat |= MKFO_NAN; break; }
       st = nx; c2tot += c2; nf++;
+    }
+    store_state(n, i, st, par_out, cov_out);
+    chi2[i] = c2tot; nfit[i] = nf; status[i] = stat;
+  }
+  return 0;
+}
+
+// ---- R7: backward (outside-in) fit -------------------------------------------------------------------
+// PAPER.md:25 "Fitting simply applies the KF procedure to all hits identified during building"; the same
+// filter run from the outermost hit inwards gives the parameters at the innermost hit. The seed is a state on the
+// outer side of the layer of the track's LAST hit. Per hit, from the last to the first: (not for the first one
+// processed) give back the material of the layer just left (C5 with dir = -1), propagate backward to the hit's layer
+// (C2/C3 with s <= 0), grazing test (U7), transport (C4), update (C6). A state arriving from outside describes the
+// particle on the outer side of the layer (after its scattering there), so the layer's material is given back after
+// the update, before moving further in; the result is the state at the innermost hit before that layer's material.
+// A track that stops early keeps the state after its last good update (material of that layer not given back).
+int mkfo_fit_backward(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, int n, const float* par,
+             const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
+             int max_plan_len, double* par_out, double* cov_out, double* chi2, int* nfit, unsigned* status) {
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < n; i++) {
+    State st; load_state(n, i, par, cov, q, st);
+    const int* pl = g->plan_layers + g->plan_off[plan[i]];
+    int plen = g->plan_off[plan[i] + 1] - g->plan_off[plan[i]];
+    if (plen > max_plan_len) plen = max_plan_len;
+    double c2tot = 0; int nf = 0; unsigned stat = 0; int prev = -1;
+    for (int s = plen - 1; s >= 0; s--) {
+      int hid = track_hits[(size_t)s * n + i];
+      if (hid < 0) continue;
+      const mkfo_layer& L = g->layers[pl[s]];
+      State cur = st;
+      if (prev >= 0) {
+        const mkfo_layer& Lp = g->layers[prev];
+        int rc = material(Lp.kind, (double)Lp.xx0, p->material_flags, cur.u, cur.C, nullptr, nullptr, -1);
+        if (rc) { stat |= (unsigned)rc; break; }
+      }
+      State nx;
+      int rc = propagate(L.kind, (double)L.pos, (double)g->bz, cur, nx, nullptr, nullptr, -1);
+      if (rc) { stat |= (unsigned)rc; break; }
+      if (L.kind == 0) { if (cos_alpha(nx.u) < (double)p->graze_cos_min) { stat |= MKFO_GRAZING; break; } }
+      else { if (std::fabs(std::cos(nx.u[ITH])) < DISK_GRAZE_COS) { stat |= MKFO_GRAZING; break; } }
+      double m[3], V6[6]; load_hit(h, hid, m, V6);
+      double c2;
+      rc = chi2_update(nx.u, nx.C, m, V6, &c2, true);
+      if (rc) { stat |= (unsigned)rc; break; }
+      if (has_nan(nx)) { stat |= MKFO_NAN; break; }
+      st = nx; c2tot += c2; nf++; prev = pl[s];
+    }
+    // the layer of the innermost fitted hit is given back too: the result is the state BEFORE that layer's material
+    // (scattering there is not constrained by any hit further in)
+    if (prev >= 0 && stat == 0) {
+      const mkfo_layer& Lp = g->layers[prev];
+      State cur = st;
+      if (material(Lp.kind, (double)Lp.xx0, p->material_flags, cur.u, cur.C, nullptr, nullptr, -1) == 0) st = cur;
     }
     store_state(n, i, st, par_out, cov_out);
     chi2[i] = c2tot; nfit[i] = nf; status[i] = stat;

@@ -48,6 +48,10 @@ void mkfo_helix_step(double bz, int q, const double* u, double s, double* u1);
 /* C5: material at a layer (state already on the surface). In/out u (6), C (36). Returns 0 or STOPPED_ELOSS.
  * theta0_out / dE_out (may be NULL) receive the Highland angle and the energy loss. */
 int mkfo_material(int kind, double xx0, int flags, double* u, double* C, double* theta0_out, double* dE_out);
+/* R7: the same with a direction: dir = +1 as above, dir = -1 backward (s <= 0; energy given back). */
+int mkfo_propagate_dir(int kind, double pos, double bz, int q, int dir, const double* u, const double* C,
+                       double* u1, double* F, double* C1, double* s);
+int mkfo_material_dir(int kind, double xx0, int flags, int dir, double* u, double* C, double* theta0_out, double* dE_out);
 /* Bethe-Bloch -dE/dx [GeV/cm] in silicon for a pion of momentum p [GeV]; Highland theta0 for thickness t. */
 double mkfo_dedx(double p);
 double mkfo_highland(double p, double t);
@@ -66,6 +70,11 @@ int mkfo_build_hit_index(const mkfo_geometry*, const mkfo_hits*, unsigned* bin_o
 /* C7. seeds par[6][n] cov[21][n] (fp32), q[n]; plan[n]; track_hits[max_plan_len][n] (global hit id or <0).
  * Outputs (double) par_out[6][n], cov_out[21][n], chi2[n], nfit[n], status[n]. */
 int mkfo_fit(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,
+             const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
+             int max_plan_len, double* par_out, double* cov_out, double* chi2, int* nfit, unsigned* status);
+/* R7. Backward fit: seeds are states on the layer of each track's LAST hit; hits are processed from the last to the
+ * first; output = state at the innermost hit before that layer's material. Same arguments as mkfo_fit. */
+int mkfo_fit_backward(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,
              const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
              int max_plan_len, double* par_out, double* cov_out, double* chi2, int* nfit, unsigned* status);
 /* C9. brute_force!=0: every hit of the layer is tried (small events); else the binned window search.

@@ -136,6 +136,19 @@ class Oracle:
         assert rc == 0
         return out
 
+    def fit_backward(self, h, par, cov, q, plan, track_hits):
+        hs = self.hits(h)
+        par, cov, q, plan, th = _f32(par), _f32(cov), _i8(q), _i8(plan), _i32(track_hits)
+        n = par.shape[1]
+        out = dict(par=np.zeros((6, n)), cov=np.zeros((21, n)), chi2=np.zeros(n), nfit=np.zeros(n, np.int32),
+                   status=np.zeros(n, np.uint32))
+        rc = self.L.mkfo_fit_backward(C.byref(self.g), C.byref(self.p), C.byref(hs), n, _p(par, C.c_float),
+                                      _p(cov, C.c_float), _p(q, C.c_byte), _p(plan, C.c_byte), _p(th, C.c_int), th.shape[0],
+                                      _dp(out["par"]), _dp(out["cov"]), _dp(out["chi2"]), _p(out["nfit"], C.c_int),
+                                      _p(out["status"], C.c_uint))
+        assert rc == 0
+        return out
+
     def build_tracks(self, h, idx, par, cov, q, seed_event, seed_hits, plan, brute_force=False, max_plan_len=None):
         hs = self.hits(h)
         par, cov, q, plan = _f32(par), _f32(cov), _i8(q), _i8(plan)
@@ -193,6 +206,25 @@ def propagate(kind, pos, bz, q, u, Cm=None):
     rc = L.mkfo_propagate(int(kind), C.c_double(pos), C.c_double(bz), int(q), _dp(u), Cp, _dp(u1), _dp(F), _dp(C1),
                           C.byref(s))
     return rc, u1, F, C1, s.value
+
+
+def propagate_dir(kind, pos, bz, q, dirn, u, Cm=None):
+    """Returns (rc, u1, F, C1, s); dirn = +1 forward, -1 backward."""
+    L = lib()
+    u = np.ascontiguousarray(u, np.float64)
+    u1, F, C1, s = np.zeros(6), np.zeros((6, 6)), np.zeros((6, 6)), C.c_double(0)
+    Cp = _dp(np.ascontiguousarray(Cm, np.float64)) if Cm is not None else None
+    rc = L.mkfo_propagate_dir(int(kind), C.c_double(pos), C.c_double(bz), int(q), int(dirn), _dp(u), Cp, _dp(u1), _dp(F),
+                              _dp(C1), C.byref(s))
+    return rc, u1, F, C1, s.value
+
+
+def material_dir(kind, xx0, flags, dirn, u, Cm):
+    u = np.array(u, np.float64)
+    Cm = np.array(Cm, np.float64)
+    th0, dE = C.c_double(0), C.c_double(0)
+    rc = lib().mkfo_material_dir(int(kind), C.c_double(xx0), int(flags), int(dirn), _dp(u), _dp(Cm), C.byref(th0), C.byref(dE))
+    return rc, u, Cm, th0.value, dE.value
 
 
 def helix_step(bz, q, u, s):
