@@ -114,6 +114,17 @@ int mkf_fit(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed cha
             int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
             void* ws, size_t ws_bytes, void* stream);
 
+/* SURVEY.md f1 / reading R7 of DESIGN.md: the same filter run from the outermost hit inwards, giving the parameters
+ * at the innermost hit ("Fitting simply applies the KF procedure to all hits"). Same arguments as
+ * mkf_fit; `seeds` are states on the layer of each track's LAST hit (e.g. mkf_fit's output with the covariance
+ * scaled up). Per hit, from the last to the first: give back the material of the layer being left (C5 with the
+ * energy loss as a gain), propagate backward (C2/C3 with s <= 0), grazing test, transport, chi2 + update; after the
+ * innermost hit that layer's material is given back too, so the output is the state before it. A track stops at its
+ * first failing step and keeps the state after its last good update. */
+int mkf_fit_backward(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed char* plan, const int* track_hits,
+            int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
+            void* ws, size_t ws_bytes, void* stream);
+
 /* a12 / C9. seeds: n states at their first hit; seed_event[n]; seed_hits[3][n] global hit ids;
  * plan[n]. Each seed is first fitted through its own three hits, then followed through the rest of its plan.
  * out: state of the winning candidate; chi2, score, nhits (incl. seed hits), nmiss;

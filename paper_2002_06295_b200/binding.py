@@ -17,7 +17,7 @@ PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8,
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
-           "mkf_build_hit_index", "mkf_fit", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host"]
+           "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host"]
 
 
 class Layer(C.Structure):
@@ -72,6 +72,7 @@ def lib():
         vp, sz, i = C.c_void_p, C.c_size_t, C.c_int
         L.mkf_build_hit_index.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), vp, sz, vp]
         L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
+        L.mkf_fit_backward.argtypes = L.mkf_fit.argtypes
         L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
                                        C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.mkf_remove_duplicates.argtypes = [vp, i, i, i, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
@@ -170,16 +171,21 @@ class Context:
                                         ws.numel() if ws is not None else 0, _stream())
         self._check(rc, "mkf_build_hit_index")
 
-    def fit(self, hits, seeds, plan, track_hits, out, chi2, nfit, status):
+    def fit_backward(self, hits, seeds, plan, track_hits, out, chi2, nfit, status):
+        """Outside-in fit (mkf_fit_backward); seeds sit on the layer of each track's last hit."""
+        return self.fit(hits, seeds, plan, track_hits, out, chi2, nfit, status, backward=True)
+
+    def fit(self, hits, seeds, plan, track_hits, out, chi2, nfit, status, backward=False):
         """seeds/out: dict(par float32 [6,n], cov float32 [21,n], q int8 [n]); plan int8 [n]; track_hits int32 [mpl,n]."""
         hs = self.hits_struct(hits, _dev)
         n = int(seeds["par"].shape[1])
         s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
         o = States(n, _dev(out["par"], torch.float32), _dev(out["cov"], torch.float32), _dev(seeds["q"], torch.int8))
-        rc = self.L.mkf_fit(self.h, C.byref(hs), C.byref(s), _dev(plan, torch.int8), _dev(track_hits, torch.int32),
+        call = self.L.mkf_fit_backward if backward else self.L.mkf_fit
+        rc = call(self.h, C.byref(hs), C.byref(s), _dev(plan, torch.int8), _dev(track_hits, torch.int32),
                             int(track_hits.shape[0]), C.byref(o), _dev(chi2, torch.float32), _dev(nfit, torch.int32),
                             _dev(status, torch.int32), None, 0, _stream())
-        self._check(rc, "mkf_fit")
+        self._check(rc, "mkf_fit_backward" if backward else "mkf_fit")
 
     def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status):
         hs = self.hits_struct(hits, _dev)

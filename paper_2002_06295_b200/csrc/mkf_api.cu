@@ -60,10 +60,34 @@ __global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_kernel(
   if (i < a.n) fit_one(g, p, a, i);
 }
 
+__global__ void __launch_bounds__(FIT_BLOCK, 4) mkf_fit_backward_kernel(const __grid_constant__ GeomDev g,
+                                                                        const __grid_constant__ ParamsDev p,
+                                                                        const __grid_constant__ FitArgs a) {
+  const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
+  if (i < a.n) fit_one_backward(g, p, a, i);
+}
+
+static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
+                      const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
+                      void* stream);
+
+extern "C" int mkf_fit_backward(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
+                                const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit,
+                                unsigned* status, void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  return fit_common(c, true, h, seeds, plan, track_hits, max_plan_len, out, chi2, nfit, status, stream);
+}
+
 extern "C" int mkf_fit(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
                        const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit,
                        unsigned* status, void* ws, size_t ws_bytes, void* stream) {
   (void)ws; (void)ws_bytes;
+  return fit_common(c, false, h, seeds, plan, track_hits, max_plan_len, out, chi2, nfit, status, stream);
+}
+
+static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
+                      const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
+                      void* stream) {
   if (!c) return MKF_INVALID_ARG;
   if (!h || !seeds || !out) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
   if (seeds->n < 0 || out->n != seeds->n || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_fit: bad sizes");
@@ -77,7 +101,12 @@ extern "C" int mkf_fit(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, c
   a.track_hits = track_hits; a.max_plan_len = max_plan_len;
   a.par_out = out->par; a.cov_out = out->cov; a.chi2 = chi2; a.nfit = nfit; a.status = status;
   const int grid = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
-  mkf_fit_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
-  MKF_LAUNCHED(c, "mkf_fit_kernel");
+  if (backward) {
+    mkf_fit_backward_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
+    MKF_LAUNCHED(c, "mkf_fit_backward_kernel");
+  } else {
+    mkf_fit_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
+    MKF_LAUNCHED(c, "mkf_fit_kernel");
+  }
   return MKF_OK;
 }

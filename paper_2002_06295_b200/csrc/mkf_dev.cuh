@@ -136,4 +136,81 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
   a.chi2[i] = c2tot; a.nfit[i] = nf; a.status[i] = stat;
 }
 
+// ---- backward fit of one track (reading R7) ---------------------------------------------------------
+// Seeds are states on the layer of each track's LAST hit. Hits are taken from the last to the first: give back the
+// material of the layer being left, propagate backward (s <= 0), transport, update. After the innermost hit that
+// layer's material is given back too (done on the covariance at the output boundary), so the result is the state
+// before it. A failing step stops the track, which keeps the state after its last good update.
+MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
+  const size_t n = (size_t)a.n;
+  const int pl = a.plan[i];
+  const int p0 = g.plan_off[pl];
+  int plen = g.plan_off[pl + 1] - p0;
+  if (plen > a.max_plan_len) plen = a.max_plan_len;
+  const float aq = -(float)a.q[i] * KAPPA * g.bz;
+  unsigned stat = 0;
+  int stop_at = -1;                                              // steps <= stop_at are not processed
+  KState S;
+  float c2tot; int nf, prev;
+  for (int pass = 0; pass < 3; pass++) {
+    const bool check = pass == 1;
+    load_params(S, a.par, n, (size_t)i);
+    c2tot = 0.f; nf = 0; prev = -1;
+    bool redo = false;
+    for (int s = plen - 1; s > stop_at; s--) {
+      const int hid = a.track_hits[(size_t)s * n + i];
+      if (hid < 0) continue;
+      const int li = g.plan_layers[p0 + s];
+      const LayerDev L = g.layers[li];
+      Hit H; load_hit(H, a.hits, hid);
+      Prop P;
+      if (nf == 0) {                                             // first hit: onto its own layer, no material yet
+        const unsigned rc = propagate_geom<-1>(S, L, aq, p.graze_cos_min, 0, false, P);
+        if (rc) { stat |= rc; break; }
+        float c[21]; load_cov(c, a.cov, n, (size_t)i);
+        commit_first(S, c, P, 0);
+      } else {
+        const LayerDev Lp = g.layers[prev];
+        float rp, J, th02;
+        material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
+        const float ipt_old = S.ipt;
+        S.ipt = ipt_old * rp;                                    // the geometry uses the momentum after the give-back
+        const unsigned rc = propagate_geom<-1>(S, L, aq, p.graze_cos_min, 0, false, P);
+        if (rc) { S.ipt = ipt_old; stat |= rc; break; }
+        commit_step_backward(S, P, J, th02, p.material_flags);
+      }
+      SInv o; float c2;
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
+      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; break; }
+      c2tot += c2; nf++; prev = li;
+    }
+    if (redo) continue;
+    if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
+    break;
+  }
+  if (nf > 0) {
+    float l[15], c[21];
+    ud_to_cov(S.u, S.d, l);
+    if (stat == 0) {                                             // give back the innermost layer's material
+      const LayerDev Lp = g.layers[prev];
+      float rp, J, th02;
+      material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
+      S.ipt *= rp;
+#pragma unroll
+      for (int k = 0; k < 5; k++) l[LI(1, k)] *= (k == 1 ? J * J : J);
+      if (p.material_flags & 1) {
+        const float g3 = -S.ipt * fast_div(S.cth, S.sth), g2 = fast_rcp(S.sth);
+        l[LI(1, 1)] += g3 * g3 * th02; l[LI(2, 1)] += g3 * th02; l[LI(2, 2)] += th02; l[LI(0, 0)] += g2 * g2 * th02;
+      }
+    }
+    cov_from_local(l, S.f, c);
+    a.par_out[i] = S.x + S.xl; a.par_out[n + i] = S.y + S.yl; a.par_out[2 * n + i] = S.z + S.zl;
+    a.par_out[3 * n + i] = S.ipt; a.par_out[4 * n + i] = wrap_phi(S.phi); a.par_out[5 * n + i] = S.th;
+#pragma unroll
+    for (int k = 0; k < 21; k++) a.cov_out[(size_t)k * n + i] = c[k];
+  } else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
+  a.chi2[i] = c2tot; a.nfit[i] = nf; a.status[i] = stat;
+}
+
 }  // namespace mkf

@@ -5,14 +5,14 @@ import torch
 from paper_2002_06295_b200 import binding as B
 
 
-def gpu_fit(ev, prm, seeds=None):
+def gpu_fit(ev, prm, seeds=None, backward=False):
     s = seeds if seeds is not None else ev["seeds"]
     ctx = B.Context(ev["geom"], prm)
     hits = B.hits_to_device(ev["hits"])
     sd = B.to_device(s, ["par", "cov", "q", "plan", "track_hits"])
     n = s["par"].shape[1]
     out = B.alloc_fit_out(n)
-    ctx.fit(hits, sd, sd["plan"], sd["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+    ctx.fit(hits, sd, sd["plan"], sd["track_hits"], out, out["chi2"], out["nfit"], out["status"], backward=backward)
     torch.cuda.synchronize()
     r = {k: v.cpu().numpy() for k, v in out.items()}
     r["status"] = r["status"].view(np.uint32)

@@ -147,3 +147,43 @@ def test_fit_quarter_of_configs1_in_bench_launch_configuration_sampled():
     dR = R[fitted] - radii[h["nfit"][fitted] - 1]
     assert dR.min() > -2e-5 * 110 and dR.max() < 0.1 and np.quantile(np.abs(dR), 0.99) < 1e-3
     assert np.isfinite(h["chi2"]).all() and np.isfinite(h["cov"]).all()
+
+
+def check_backward(ev, prm):
+    """mkf_fit_backward against the oracle (R7). Seeds: the ORACLE's forward fit (so that both sides start from the
+    same float32 numbers) with the covariance x100, hit lists cut at the last fitted hit."""
+    from gpu_helpers import gpu_fit
+    s = ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], prm)
+    f = o.fit(ev["hits"], s["par"], s["cov"], s["q"], s["plan"], s["track_hits"])
+    th = s["track_hits"].copy()
+    th[np.cumsum(th >= 0, 0) > f["nfit"][None]] = -1
+    sb = dict(par=f["par"].astype(np.float32), cov=(100.0 * f["cov"]).astype(np.float32), q=s["q"], plan=s["plan"],
+              track_hits=np.ascontiguousarray(th))
+    r = o.fit_backward(ev["hits"], sb["par"], sb["cov"], sb["q"], sb["plan"], sb["track_hits"])
+    h = gpu_fit(ev, prm, sb, backward=True)
+    assert np.array_equal(h["nfit"], r["nfit"]) and np.array_equal(h["status"], r["status"])
+    has = th >= 0
+    ok = (r["nfit"] > 0) & (r["nfit"] == has.sum(0))                   # went all the way in: state on the first hit's layer
+    assert ok.mean() > 0.95
+    geom = ev["geom"]
+    lay = np.asarray(geom["plan_layers"])[np.asarray(geom["plan_off"])[s["plan"].astype(int)] + np.argmax(has, 0)]
+    kinds = np.array([l["kind"] for l in geom["layers"]])[lay]
+    pos = np.array([abs(l["pos"]) for l in geom["layers"]])[lay]
+    assert parity.param_errors(h["par"], r["par"], pos)[ok].max() <= parity.TOL_PAR
+    assert parity.cov_errors(h["cov"], r["cov"], r["par"], kinds)[ok].max() <= parity.TOL_COV
+    assert parity.chi2_errors(h["chi2"], r["chi2"])[ok].max() <= parity.TOL_CHI2
+    return r, h
+
+
+def test_fit_backward_barrel():
+    ev, prm = datagen.config(0, scale=0.5)
+    check_backward(ev, prm)
+    ev, prm = datagen.config(1, scale=0.005)          # 20 000 helices, 17 layers, tracks of unequal length
+    check_backward(ev, prm)
+
+
+def test_fit_backward_barrel_endcap_with_curling_tracks():
+    ev, prm = datagen.config(3, scale=0.01)           # disks and cylinders, soft tracks that come back in radius
+    r, h = check_backward(ev, prm)
+    assert (r["status"] != 0).sum() >= 1
