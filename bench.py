@@ -141,14 +141,14 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------
 # oracle legs (cpu_baseline of the mkf arm, and the whole --impl reference arm)
 # ---------------------------------------------------------------------------------------------------------------
-def oracle_fit_rate(geom, prm, hits, seeds, n_tracks, repeat=1):
+def oracle_fit_rate(geom, prm, hits, seeds, n_tracks, repeat=1, backward=False):
     from oracle import mkfo
     o = mkfo.Oracle(geom, prm)
     sl = slice(0, n_tracks)
     args = (hits, seeds["par"][:, sl], seeds["cov"][:, sl], seeds["q"][sl], seeds["plan"][sl], np.ascontiguousarray(seeds["track_hits"][:, sl]))
     t = time.perf_counter()
     for _ in range(repeat):
-        r = o.fit(*args)
+        r = o.fit_backward(*args) if backward else o.fit(*args)
     dt = (time.perf_counter() - t) / repeat
     return float(r["nfit"].sum()) / dt, dt, o.num_threads(), int(r["nfit"].sum()), r
 
@@ -181,7 +181,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mkf", choices=["mkf", "reference"])
-    ap.add_argument("--workload", default="fit", choices=["fit", "build2", "build3", "build4"])
+    ap.add_argument("--workload", default="fit", choices=["fit", "fitback", "build2", "build3", "build4"])
     ap.add_argument("--scale", type=float, default=1.0, help="shrinks the workload (testing only; the JSON says so)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -191,10 +191,12 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     warm = max(a.warmup, 3)
-    is_fit = a.workload == "fit"
+    backward = a.workload == "fitback"
+    is_fit = a.workload in ("fit", "fitback")
     metric = "KF layer-steps/s (propagate+update)" if is_fit else "built events/s"
     unit = "layer-steps/s" if is_fit else "events/s"
-    names = dict(fit="configs[1]: track fit, 4M helices x 17 barrel layers, MS + dE/dx, seeds from 3 hits, cov x100",
+    names = dict(fitback="configs[1] workload, backward fit (SURVEY f1): seeds = forward fit at the last hit, covariance x100",
+                 fit="configs[1]: track fit, 4M helices x 17 barrel layers, MS + dE/dx, seeds from 3 hits, cov x100",
                  build2="configs[2]: building, barrel, 100 events x 1000 tracks + 20k noise hits, top 6",
                  build3="configs[3]: building, barrel+endcap, 200 events x 1500 seeds, ~80k hits/event",
                  build4="configs[4]: batched building + duplicate removal, 64 events x 6000 seeds, ~300k hits/event, top 8")
@@ -257,13 +259,27 @@ def main():
         n = seeds["par"].shape[1]
         out = B.alloc_fit_out(n)
 
-        def step():
+        if backward:                                      # seeds of the backward fit: one untimed forward fit
             ctx.fit(dh, ds, ds["plan"], ds["track_hits"], out, out["chi2"], out["nfit"], out["status"])
+            th = ds["track_hits"].clone()
+            th[torch.cumsum((th >= 0).to(torch.int32), 0) > out["nfit"][None]] = -1
+            ds = dict(ds, par=out["par"].clone(), cov=(100.0 * out["cov"]), track_hits=th.contiguous())
+            seeds = {k: v.cpu().numpy() for k, v in ds.items()}
+
+        def step():
+            ctx.fit(dh, ds, ds["plan"], ds["track_hits"], out, out["chi2"], out["nfit"], out["status"], backward=backward)
 
         def units():
             return float(out["nfit"].sum().item())
 
         def e2e_step():
+            if backward:                                  # no host entry point for the backward fit: pinned copies by torch
+                hd = {k: (torch.from_numpy(v).cuda(non_blocking=True) if isinstance(v, np.ndarray) else v) for k, v in hits_p.items()}
+                sd2 = {k: torch.from_numpy(v).cuda(non_blocking=True) for k, v in seeds_p.items()}
+                ctx.fit(hd, sd2, sd2["plan"], sd2["track_hits"], out, out["chi2"], out["nfit"], out["status"], backward=True)
+                res = [out[k].cpu() for k in ("par", "cov", "chi2", "nfit", "status")]
+                h2d = sum(v.nbytes for v in hits_p.values() if isinstance(v, np.ndarray)) + sum(v.nbytes for v in seeds_p.values())
+                return float(res[3].sum()), h2d, sum(t.numel() * t.element_size() for t in res)
             r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"])
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
     else:
@@ -342,8 +358,8 @@ def main():
         steps_per_launch = u                                  # one launch = one step = all layer-steps of this rank
         t_launch = ms_total / a.steps * 1e-3
         ach = ALGO_FLOP_PER_LAYER_STEP * steps_per_launch / t_launch / 1e12
-        roof = dict(bound="alu", kernel="mkf_fit_kernel", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
-                    traffic=NCU_TRAFFIC_BYTES_FIT_FULL if a.scale == 1.0 else None,
+        roof = dict(bound="alu", kernel="mkf_fit_backward_kernel" if backward else "mkf_fit_kernel", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
+                    traffic=NCU_TRAFFIC_BYTES_FIT_FULL if (a.scale == 1.0 and not backward) else None,
                     algorithmic_bytes=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch, peak_source="148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (%s max clock)" % (pk["sm_max_mhz"], pk["source"]),
                     algorithmic_flop_per_layer_step=ALGO_FLOP_PER_LAYER_STEP,
                     hbm=dict(achieved=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
@@ -356,13 +372,14 @@ def main():
     if not a.no_cpu_baseline:
         if is_fit:
             n_s = min(n, 1000000)
-            rate, dt, cores, st, r = oracle_fit_rate(geom, prm, hits, seeds, n_s)
+            rate, dt, cores, st, r = oracle_fit_rate(geom, prm, hits, seeds, n_s, backward=backward)
             cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d helices of the workload (%d layer-steps, %.1f s)" % (n_s, st, dt))
             # parity of the timed launch configuration on that same sample (the oracle results are already here)
             from paper_2002_06295_b200 import parity
             g = {k: out[k][..., :n_s].cpu().numpy() for k in ("par", "cov", "chi2", "nfit", "status")}
             ok = r["nfit"] > 0
-            lay, kinds, pos = parity.last_layer_of_fit(geom, seeds["plan"][:n_s], seeds["track_hits"][:, :n_s], r["nfit"])
+            where = parity.first_layer_of_backward_fit if backward else parity.last_layer_of_fit
+            lay, kinds, pos = where(geom, seeds["plan"][:n_s], seeds["track_hits"][:, :n_s], r["nfit"])
             cpu["parity"] = dict(n=int(n_s), nfit_identical=bool(np.array_equal(g["nfit"], r["nfit"])),
                                  status_identical=bool(np.array_equal(g["status"].view(np.uint32), r["status"])),
                                  par_max=float(parity.param_errors(g["par"], r["par"], pos)[ok].max()),

@@ -73,3 +73,15 @@ def last_layer_of_fit(geom, plan, track_hits, nfit):
     kinds = np.array([l["kind"] for l in geom["layers"]])[lay]
     pos = np.array([abs(l["pos"]) for l in geom["layers"]])[lay]
     return lay, kinds, pos
+
+
+def first_layer_of_backward_fit(geom, plan, track_hits, nfit):
+    """Same for the backward fit: the layer of the nfit-th hit counted from the END of the hit list."""
+    plan_off, plan_layers = np.asarray(geom["plan_off"]), np.asarray(geom["plan_layers"])
+    has = track_hits >= 0
+    cs = np.cumsum(has[::-1], 0)[::-1]
+    step = np.argmax(has & (cs == np.maximum(nfit, 1)[None]), 0)
+    lay = plan_layers[plan_off[np.asarray(plan, int)] + step]
+    kinds = np.array([l["kind"] for l in geom["layers"]])[lay]
+    pos = np.array([abs(l["pos"]) for l in geom["layers"]])[lay]
+    return lay, kinds, pos
