@@ -107,25 +107,28 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
     const bool check = pass == 1;
     load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0;
-    bool redo = false;
+    bool redo = false, stopped = false;
     const int* th = a.track_hits + i;
     int hid_next = stop_at > 0 ? *th : -1;                       // the hit id is fetched one step ahead
+    // no `continue` / `break` out of the layer loop: a thread that skipped a layer without a hit would run ahead of
+    // its warp and never rejoin it; the body is a plain if-region, so the warp reconverges after every layer
     for (int s = 0; s < stop_at; s++) {
       const int hid = hid_next;
       th += n;
       hid_next = s + 1 < stop_at ? *th : -1;
-      if (hid < 0) continue;
-      const LayerDev L = g.layers[g.plan_layers[p0 + s]];
-      Hit H; load_hit(H, a.hits, hid);
-      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
-      if (rc) { stat |= rc; break; }
-      SInv o; float c2;
-      hit_to_local(S, H, o);
-      if (!kalman_update(S, o, c2)) {                          // state untouched by the failed update, but already
-        stat |= ST_S_NOT_PD; stop_at = s; redo = true; break;  // propagated: re-run up to the step before
-      }
-      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; break; }
-      c2tot += c2; nf++;
+      if (hid >= 0 && !stopped) do {
+        const LayerDev L = g.layers[g.plan_layers[p0 + s]];
+        Hit H; load_hit(H, a.hits, hid);
+        const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
+        if (rc) { stat |= rc; stopped = true; break; }
+        SInv o; float c2;
+        hit_to_local(S, H, o);
+        if (!kalman_update(S, o, c2)) {                        // state untouched by the failed update, but already
+          stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break;  // propagated: re-run up to the step before
+        }
+        if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; break; }
+        c2tot += c2; nf++;
+      } while (0);
     }
     if (redo) continue;
     if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
@@ -156,34 +159,34 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     const bool check = pass == 1;
     load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0; prev = -1;
-    bool redo = false;
+    bool redo = false, stopped = false;
+    // no `continue` / `break` out of the layer loop: tracks of one warp meet their first hit at different steps, and
+    // threads that ran ahead would never rejoin the others (measured: 3x the instructions); the body is a plain
+    // if-region, so the warp reconverges after every layer
     for (int s = plen - 1; s > stop_at; s--) {
       const int hid = a.track_hits[(size_t)s * n + i];
-      if (hid < 0) continue;
-      const int li = g.plan_layers[p0 + s];
-      const LayerDev L = g.layers[li];
-      Hit H; load_hit(H, a.hits, hid);
-      Prop P;
-      if (nf == 0) {                                             // first hit: onto its own layer, no material yet
+      if (hid >= 0 && !stopped) do {
+        const int li = g.plan_layers[p0 + s];
+        const LayerDev L = g.layers[li];
+        Hit H; load_hit(H, a.hits, hid);
+        Prop P;
+        float J = 1.f, th02 = 0.f, ipt_old = S.ipt;
+        if (nf > 0) {                                            // give back the material of the layer being left
+          const LayerDev Lp = g.layers[prev];
+          float rp;
+          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
+          S.ipt = ipt_old * rp;                                  // the geometry uses the momentum after the give-back
+        }
         const unsigned rc = propagate_geom<-1>(S, L, aq, p.graze_cos_min, 0, false, P);
-        if (rc) { stat |= rc; break; }
-        float c[21]; load_cov(c, a.cov, n, (size_t)i);
-        commit_first(S, c, P, 0);
-      } else {
-        const LayerDev Lp = g.layers[prev];
-        float rp, J, th02;
-        material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
-        const float ipt_old = S.ipt;
-        S.ipt = ipt_old * rp;                                    // the geometry uses the momentum after the give-back
-        const unsigned rc = propagate_geom<-1>(S, L, aq, p.graze_cos_min, 0, false, P);
-        if (rc) { S.ipt = ipt_old; stat |= rc; break; }
-        commit_step_backward(S, P, J, th02, p.material_flags);
-      }
-      SInv o; float c2;
-      hit_to_local(S, H, o);
-      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; break; }
-      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; break; }
-      c2tot += c2; nf++; prev = li;
+        if (rc) { S.ipt = ipt_old; stat |= rc; stopped = true; break; }
+        if (nf == 0) { float c[21]; load_cov(c, a.cov, n, (size_t)i); commit_first(S, c, P, 0); }
+        else commit_step_backward(S, P, J, th02, p.material_flags);
+        SInv o; float c2;
+        hit_to_local(S, H, o);
+        if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break; }
+        if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; break; }
+        c2tot += c2; nf++; prev = li;
+      } while (0);
     }
     if (redo) continue;
     if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
