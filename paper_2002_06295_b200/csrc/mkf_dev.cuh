@@ -99,6 +99,9 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
   const float aq = -(float)a.q[i] * KAPPA * g.bz;
   unsigned stat = 0;
   int stop_at = plen;
+#ifdef __CUDA_ARCH__
+  const unsigned wmask = __activemask();                         // the threads of this warp that own a track
+#endif
   KState S;
   float c2tot; int nf;
   // pass 0 runs without per-step finiteness checks; only if its result is not finite, pass 1 finds the step
@@ -109,26 +112,30 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
     c2tot = 0.f; nf = 0;
     bool redo = false, stopped = false;
     const int* th = a.track_hits + i;
+    const int stop_at_loop = stop_at;
     int hid_next = stop_at > 0 ? *th : -1;                       // the hit id is fetched one step ahead
-    // no `continue` / `break` out of the layer loop: a thread that skipped a layer without a hit would run ahead of
-    // its warp and never rejoin it; the body is a plain if-region, so the warp reconverges after every layer
-    for (int s = 0; s < stop_at; s++) {
+    // every thread of the warp goes through every iteration and the warp is re-joined at its top: a thread that
+    // skipped a layer without a hit (or stopped) would otherwise run ahead of its warp and never rejoin it
+    // (measured on hit lists with 5 % gaps: 14.7 instead of 34.5 G layer-steps/s)
+    for (int s = 0; s < stop_at_loop; s++) {
+#ifdef __CUDA_ARCH__
+      __syncwarp(wmask);
+#endif
       const int hid = hid_next;
       th += n;
-      hid_next = s + 1 < stop_at ? *th : -1;
-      if (hid >= 0 && !stopped) do {
-        const LayerDev L = g.layers[g.plan_layers[p0 + s]];
-        Hit H; load_hit(H, a.hits, hid);
-        const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
-        if (rc) { stat |= rc; stopped = true; break; }
-        SInv o; float c2;
-        hit_to_local(S, H, o);
-        if (!kalman_update(S, o, c2)) {                        // state untouched by the failed update, but already
-          stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break;  // propagated: re-run up to the step before
-        }
-        if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; break; }
-        c2tot += c2; nf++;
-      } while (0);
+      hid_next = s + 1 < stop_at_loop ? *th : -1;
+      if (hid < 0 || stopped) continue;
+      const LayerDev L = g.layers[g.plan_layers[p0 + s]];
+      Hit H; load_hit(H, a.hits, hid);
+      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
+      if (rc) { stat |= rc; stopped = true; continue; }
+      SInv o; float c2;
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) {                          // state untouched by the failed update, but already
+        stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; continue;   // propagated: re-run up to the step before
+      }
+      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; continue; }
+      c2tot += c2; nf++;
     }
     if (redo) continue;
     if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
