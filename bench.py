@@ -26,8 +26,8 @@ ALGO_FLOP_PER_LAYER_STEP = 1000.0        # DESIGN.md §6 (SURVEY.md §8 d): prop
 ALGO_BYTES_PER_LAYER_STEP = 54.0         # hit 36 B + index 4 B + state in/out amortised 14 B
 FP32_LANES_PER_SM, N_SM = 128, 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one mkf_fit_kernel launch on the full configs[1] workload, from
-# the `ncu --set full` capture summarised in profiles/r1_fit_kernel_ncu.md (3.1227 GB + 0.5236 GB)
-NCU_TRAFFIC_BYTES_FIT_FULL = 3.646e9
+# the `ncu --set full` capture summarised in profiles/r1_fit_kernel_ncu.md (3.1226 GB + 0.4689 GB)
+NCU_TRAFFIC_BYTES_FIT_FULL = 3.591e9
 
 
 def peaks():
