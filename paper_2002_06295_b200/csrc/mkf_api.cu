@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_kernel(
   if (i < a.n) fit_one(g, p, a, i);
 }
 
-__global__ void __launch_bounds__(FIT_BLOCK, 4) mkf_fit_backward_kernel(const __grid_constant__ GeomDev g,
+__global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_backward_kernel(const __grid_constant__ GeomDev g,
                                                                         const __grid_constant__ ParamsDev p,
                                                                         const __grid_constant__ FitArgs a) {
   const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
