@@ -702,4 +702,55 @@ int mkfo_remove_duplicates(const mkfo_params* p, int n_events, const int* track_
   return 0;
 }
 
+// ---- R8: strip clustering (section 4) --------------------------------------------
+// "first, seed strips with ADC values greater than 3 times the expected noise are identified; second, clusters are
+// formed adding to the seed all strips with ADC values above twice the expected noise that are either consecutive or
+// have a small gap (the size of the allowed gap depends on the presence of bad strips in the module); finally, the
+// cluster is required to have a quadrature sum of the strip ADCs larger than 5 times the quadrature sum of the
+// expected noise, and to have a minimum total charge."
+// Reading R8: a bad strip never passes a threshold; consecutive passing strips i < j of one module belong to the same
+// cluster iff at most max_holes good strips and at most max_bad bad strips lie strictly between them; a cluster is
+// kept iff it holds a seed strip, sum(adc^2) > clus_thr^2 * sum(noise^2) (over its passing strips, fp64, strip order)
+// and sum(adc) >= min_charge. Strip thresholds are compared in fp32: (float)adc > thr * noise.
+// Output, ordered by (module, first strip): module, first strip and last strip (index inside the module), charge,
+// barycentre = sum(adc * (strip + 0.5)) / sum(adc) (fp64, strip order, stored as float). Returns the number kept.
+int mkfo_cluster_strips(int n_modules, const int* module_off, const unsigned short* adc, const float* noise,
+                        const unsigned char* bad, float seed_thr, float chan_thr, float clus_thr, int min_charge,
+                        int max_holes, int max_bad, int* out_module, int* out_first, int* out_last,
+                        unsigned* out_charge, float* out_bary) {
+  int nout = 0;
+  for (int m = 0; m < n_modules; m++) {
+    int b = module_off[m], e = module_off[m + 1];
+    int i = b;
+    while (i < e) {
+      bool pass_i = !bad[i] && (float)adc[i] > chan_thr * noise[i];
+      if (!pass_i) { i++; continue; }
+      // grow the cluster from strip i
+      int first = i, last = i;
+      bool seed = false; unsigned long long q2 = 0; double n2 = 0, wsum = 0; unsigned charge = 0;
+      int j = i, holes = 0, nbad = 0;
+      while (j < e) {
+        bool pj = !bad[j] && (float)adc[j] > chan_thr * noise[j];
+        if (pj) {
+          last = j; holes = 0; nbad = 0;
+          if ((float)adc[j] > seed_thr * noise[j]) seed = true;
+          q2 += (unsigned long long)adc[j] * adc[j]; n2 += (double)noise[j] * (double)noise[j];
+          charge += adc[j]; wsum += (double)adc[j] * ((double)(j - b) + 0.5);
+        } else {
+          if (bad[j]) nbad++; else holes++;
+          if (holes > max_holes || nbad > max_bad) break;
+        }
+        j++;
+      }
+      if (seed && (double)q2 > (double)clus_thr * (double)clus_thr * n2 && (long long)charge >= (long long)min_charge) {
+        out_module[nout] = m; out_first[nout] = first - b; out_last[nout] = last - b; out_charge[nout] = charge;
+        out_bary[nout] = (float)(wsum / (double)charge);
+        nout++;
+      }
+      i = last + 1;
+    }
+  }
+  return nout;
+}
+
 }  // extern "C"

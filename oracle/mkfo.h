@@ -89,6 +89,11 @@ int mkfo_build_tracks(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*
 /* C10. track_off[n_events+1]; hit_ids[max_plan_len][n]; keep[n], n_kept[n_events]. */
 int mkfo_remove_duplicates(const mkfo_params*, int n_events, const int* track_off, const int* hit_ids,
              int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept);
+/* R8: three-threshold strip clustering. Outputs sized for the worst case (n_strips). */
+int mkfo_cluster_strips(int n_modules, const int* module_off, const unsigned short* adc, const float* noise,
+                        const unsigned char* bad, float seed_thr, float chan_thr, float clus_thr, int min_charge,
+                        int max_holes, int max_bad, int* out_module, int* out_first, int* out_last,
+                        unsigned* out_charge, float* out_bary);
 int mkfo_num_threads(void);
 #ifdef __cplusplus
 }

@@ -264,3 +264,17 @@ def update(u, Cm, m, V6):
     rc = lib().mkfo_update(_dp(u), _dp(Cm), _dp(np.ascontiguousarray(m, np.float64)),
                            _dp(np.ascontiguousarray(V6, np.float64)), C.byref(c2))
     return rc, u, Cm, c2.value
+
+
+def cluster_strips(module_off, adc, noise, bad, seed_thr=3.0, chan_thr=2.0, clus_thr=5.0, min_charge=0, max_holes=0, max_bad=1):
+    """R8: returns dict(module, first, last, charge, bary) of the kept clusters, ordered by (module, first strip)."""
+    mo = _i32(module_off)
+    adc = np.ascontiguousarray(adc, np.uint16); noise = _f32(noise); bad = np.ascontiguousarray(bad, np.uint8)
+    n = adc.shape[0]
+    om, of, ol = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32)
+    oc, ob = np.zeros(n, np.uint32), np.zeros(n, np.float32)
+    L = lib()
+    k = L.mkfo_cluster_strips(mo.shape[0] - 1, _p(mo, C.c_int), _p(adc, C.c_ushort), _p(noise, C.c_float), _p(bad, C.c_ubyte),
+                              C.c_float(seed_thr), C.c_float(chan_thr), C.c_float(clus_thr), int(min_charge), int(max_holes),
+                              int(max_bad), _p(om, C.c_int), _p(of, C.c_int), _p(ol, C.c_int), _p(oc, C.c_uint), _p(ob, C.c_float))
+    return dict(module=om[:k].copy(), first=of[:k].copy(), last=ol[:k].copy(), charge=oc[:k].copy(), bary=ob[:k].copy())

@@ -395,3 +395,39 @@ def config(i, scale=1.0, seed=0):
                             pt_range=(0.3, 50.0), n_hard=0, eta_max=2.5, eff=0.95, seed_on_pixel=True),
                 default_params(max_cand=8, min_hits_keep=4))
     raise ValueError(i)
+
+
+# ------------------------------------------------------------------------------------------------------
+# raw strip data for the clustering step. A toy stand-in for unpacked, calibrated
+# silicon-strip ADC counts: no detector data is available here.
+# ------------------------------------------------------------------------------------------------------
+def make_strips(seed, n_modules, strips_per_module=512, occupancy=0.01, bad_frac=0.01, noise_mean=4.0):
+    """Per strip: pedestal-subtracted ADC (uint16: Gaussian noise rounded and clipped at 0, plus charge deposits of
+    1-5 strips with an exponential-tailed total charge), its expected noise (float32, per strip, ~N(noise_mean, 5 %)),
+    a bad-strip flag (bad strips read 0). Modules of unequal length (every 7th module is half as long).
+    Draw order: noise level, bad flags, noise samples, deposit positions, widths, charges, shares."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    lens = np.where(np.arange(n_modules) % 7 == 6, strips_per_module // 2, strips_per_module).astype(np.int64)
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    n = int(off[-1])
+    noise = (noise_mean * (1 + 0.05 * rng.standard_normal(n))).clip(0.5 * noise_mean).astype(np.float32)
+    bad = (rng.random(n) < bad_frac).astype(np.uint8)
+    sig = rng.standard_normal(n) * noise
+    ndep = int(occupancy * n / 3)
+    pos = rng.integers(0, n, ndep)
+    width = rng.integers(1, 6, ndep)
+    charge = 60.0 + rng.exponential(80.0, ndep)
+    for k in range(5):
+        m = width > k
+        idx = np.minimum(pos[m] + k, n - 1)
+        share = charge[m] / width[m] * (0.6 + 0.8 * rng.random(m.sum()))
+        np.add.at(sig, idx, share)
+    adc = np.clip(np.rint(sig), 0, 1023).astype(np.uint16)
+    adc[bad != 0] = 0
+    return dict(module_off=off, adc=adc, noise=noise, bad=bad)
+
+
+def default_strip_params(**kw):
+    p = dict(seed_thr=3.0, chan_thr=2.0, clus_thr=5.0, min_charge=30, max_holes=0, max_bad=1)
+    p.update(kw)
+    return p
