@@ -45,7 +45,8 @@ enum { MKF_PROP_UNREACHABLE = 1, /* next surface not reachable going forward wit
 enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total over plans */, MKF_MAX_CAND = 8 };
 
 /* workspace query ids */
-enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3 };
+enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3,
+       MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips */ };
 
 typedef struct mkf_ctx mkf_ctx;       /* opaque: geometry, parameters, last error text */
 
@@ -141,6 +142,38 @@ int mkf_remove_duplicates(mkf_ctx*, int n_events, int n, int n_hits, const int* 
             int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept,
             void* ws, size_t ws_bytes, void* stream);
 
+/* ---- SURVEY.md f3 / reading R8 of DESIGN.md: strip clustering ------------------------------
+ * "seed strips with ADC values greater than 3 times the expected noise are identified; second, clusters are formed
+ * adding to the seed all strips with ADC values above twice the expected noise that are either consecutive or have
+ * a small gap (the size of the allowed gap depends on the presence of bad strips in the module); finally, the
+ * cluster is required to have a quadrature sum of the strip ADCs larger than 5 times the quadrature sum of the
+ * expected noise, and to have a minimum total charge."
+ * Input: the strips of all modules of all events of the batch, concatenated; module m owns strips
+ * module_off[m]..module_off[m+1]-1 (ascending; empty modules allowed). adc: pedestal-subtracted counts; noise: the
+ * expected noise of each strip; bad: non-zero = bad strip (never counted, may be bridged). adc and noise must be
+ * 16-byte aligned and bad 8-byte aligned; n_strips <= 2^31 - 4096; max_holes + max_bad <= 31.
+ * Output (ordered by module, then first strip): module, first and last strip (index inside the module), charge =
+ * sum adc, bary = sum adc (strip + 1/2) / sum adc in strip units. *n_clusters = number of clusters found; only the
+ * first `capacity` are written (n_clusters > capacity tells the caller to retry with more room). */
+typedef struct { float seed_thr, chan_thr, clus_thr; int min_charge, max_holes, max_bad; } mkf_strip_params;
+typedef struct {
+  int n_modules, n_strips;
+  const int* module_off;            /* [n_modules + 1] */
+  const unsigned short* adc;        /* [n_strips] */
+  const float* noise;               /* [n_strips] */
+  const unsigned char* bad;         /* [n_strips] */
+} mkf_strips;
+typedef struct {
+  int capacity;
+  int *module, *first, *last;       /* [capacity] */
+  unsigned* charge;                 /* [capacity] */
+  float* bary;                      /* [capacity] */
+  int* n_clusters;                  /* [1] */
+} mkf_clusters;
+/* Device pointers, caller's stream, no synchronisation. ws: mkf_workspace_bytes(MKF_CALL_CLUSTER_STRIPS, 0, n_strips, 0). */
+int mkf_cluster_strips(mkf_ctx*, const mkf_strips*, const mkf_strip_params*, const mkf_clusters* out,
+            void* ws, size_t ws_bytes, void* stream);
+
 /* ---- host-buffer entry points (end-to-end use: all pointers HOST; synchronous) ------------------------- */
 /* Same semantics as mkf_fit, every pointer (hits arrays included) in host memory. Device memory is taken from
  * the CUDA stream-ordered pool and released before returning. h2d_bytes/d2h_bytes (may be NULL) receive the
@@ -153,6 +186,11 @@ int mkf_fit_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_ho
 int mkf_build_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_host, const int* seed_event,
             const int* seed_hits, const signed char* plan, int max_plan_len, mkf_states* out_host, float* chi2,
             float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, unsigned char* keep,
+            long long* h2d_bytes, long long* d2h_bytes);
+/* mkf_cluster_strips on host buffers (pinned memory makes the copies asynchronous). Device memory comes from the
+ * stream-ordered pool, so repeated calls pay no allocation ("using a memory pool to pay the allocation
+ * overhead only at the beginning and end of job"). *out->n_clusters is the number found; min(that, capacity) are copied. */
+int mkf_cluster_strips_host(mkf_ctx*, const mkf_strips* strips_host, const mkf_strip_params*, const mkf_clusters* out_host,
             long long* h2d_bytes, long long* d2h_bytes);
 #ifdef __cplusplus
 }

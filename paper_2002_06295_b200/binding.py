@@ -17,7 +17,8 @@ PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8,
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
-           "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host"]
+           "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host",
+           "mkf_cluster_strips", "mkf_cluster_strips_host"]
 
 
 class Layer(C.Structure):
@@ -50,6 +51,24 @@ class States(C.Structure):
     _fields_ = [("n", C.c_int), ("par", C.c_void_p), ("cov", C.c_void_p), ("q", C.c_void_p)]
 
 
+class StripParams(C.Structure):
+    _fields_ = [("seed_thr", C.c_float), ("chan_thr", C.c_float), ("clus_thr", C.c_float), ("min_charge", C.c_int),
+                ("max_holes", C.c_int), ("max_bad", C.c_int)]
+
+
+class Strips(C.Structure):
+    _fields_ = [("n_modules", C.c_int), ("n_strips", C.c_int), ("module_off", C.c_void_p), ("adc", C.c_void_p),
+                ("noise", C.c_void_p), ("bad", C.c_void_p)]
+
+
+class Clusters(C.Structure):
+    _fields_ = [("capacity", C.c_int), ("module", C.c_void_p), ("first", C.c_void_p), ("last", C.c_void_p),
+                ("charge", C.c_void_p), ("bary", C.c_void_p), ("n_clusters", C.c_void_p)]
+
+
+MKF_CALL_CLUSTER_STRIPS = 4
+
+
 _lib = None
 
 
@@ -77,6 +96,8 @@ def lib():
                                        C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.mkf_remove_duplicates.argtypes = [vp, i, i, i, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
         ll = C.POINTER(C.c_longlong)
+        L.mkf_cluster_strips.argtypes = [vp, C.POINTER(Strips), C.POINTER(StripParams), C.POINTER(Clusters), vp, sz, vp]
+        L.mkf_cluster_strips_host.argtypes = [vp, C.POINTER(Strips), C.POINTER(StripParams), C.POINTER(Clusters), ll, ll]
         L.mkf_fit_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, ll, ll]
         L.mkf_build_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, vp, i, C.POINTER(States), vp, vp,
                                      vp, vp, vp, vp, vp, ll, ll]
@@ -210,6 +231,39 @@ class Context:
                                           ws.data_ptr(), ws.numel(), _stream())
         self._check(rc, "mkf_remove_duplicates")
 
+    def cluster_strips(self, strips, prm, out, ws):
+        """strips / out: dicts of CUDA tensors (strips_to_device, alloc_clusters); prm: dict (datagen.default_strip_params)."""
+        n = int(strips["adc"].shape[0])
+        s = Strips(int(strips["module_off"].shape[0]) - 1, n, _dev(strips["module_off"], torch.int32),
+                   _dev(strips["adc"], torch.uint16), _dev(strips["noise"], torch.float32), _dev(strips["bad"], torch.uint8))
+        o = Clusters(int(out["module"].shape[0]), _dev(out["module"], torch.int32), _dev(out["first"], torch.int32),
+                     _dev(out["last"], torch.int32), _dev(out["charge"], torch.int32), _dev(out["bary"], torch.float32),
+                     _dev(out["n_clusters"], torch.int32))
+        sp = strip_params(prm)
+        rc = self.L.mkf_cluster_strips(self.h, C.byref(s), C.byref(sp), C.byref(o), ws.data_ptr() if ws is not None else None,
+                                       ws.numel() if ws is not None else 0, _stream())
+        self._check(rc, "mkf_cluster_strips")
+
+    def cluster_strips_host(self, strips, prm, capacity):
+        """strips: dict of numpy arrays / CPU (pinned) tensors. Returns dict of numpy arrays cut to the number found."""
+        i32, f32 = np.int32, np.float32
+        n = int(strips["adc"].shape[0])
+        s = Strips(int(strips["module_off"].shape[0]) - 1, n, _host(strips["module_off"], i32), _host(strips["adc"], np.uint16),
+                   _host(strips["noise"], f32), _host(strips["bad"], np.uint8))
+        out = dict(module=np.empty(capacity, i32), first=np.empty(capacity, i32), last=np.empty(capacity, i32),
+                   charge=np.empty(capacity, np.uint32), bary=np.empty(capacity, f32))
+        nc = np.zeros(1, i32)
+        o = Clusters(capacity, out["module"].ctypes.data, out["first"].ctypes.data, out["last"].ctypes.data,
+                     out["charge"].ctypes.data, out["bary"].ctypes.data, nc.ctypes.data)
+        sp = strip_params(prm)
+        h2d, d2h = C.c_longlong(0), C.c_longlong(0)
+        rc = self.L.mkf_cluster_strips_host(self.h, C.byref(s), C.byref(sp), C.byref(o), C.byref(h2d), C.byref(d2h))
+        self._check(rc, "mkf_cluster_strips_host")
+        k = min(int(nc[0]), capacity)
+        out = {key: v[:k] for key, v in out.items()}
+        out["n_clusters"], out["h2d_bytes"], out["d2h_bytes"] = int(nc[0]), h2d.value, d2h.value
+        return out
+
     # ---- host-buffer entry points -------------------------------------------------------------------------
     def fit_host(self, hits, seeds, plan, track_hits):
         """All arguments numpy / CPU tensors; returns dict of numpy arrays plus the bytes copied each way."""
@@ -249,6 +303,23 @@ class Context:
             out["keep"] = keep
         out["h2d_bytes"], out["d2h_bytes"] = h2d.value, d2h.value
         return out
+
+
+def strip_params(p):
+    return StripParams(p["seed_thr"], p["chan_thr"], p["clus_thr"], p["min_charge"], p["max_holes"], p["max_bad"])
+
+
+def strips_to_device(d, device="cuda"):
+    return dict(module_off=torch.from_numpy(d["module_off"]).to(device), adc=torch.from_numpy(d["adc"]).to(device),
+                noise=torch.from_numpy(d["noise"]).to(device), bad=torch.from_numpy(d["bad"]).to(device))
+
+
+def alloc_clusters(capacity, device="cuda"):
+    i32 = torch.int32
+    return dict(module=torch.empty(capacity, dtype=i32, device=device), first=torch.empty(capacity, dtype=i32, device=device),
+                last=torch.empty(capacity, dtype=i32, device=device), charge=torch.empty(capacity, dtype=i32, device=device),
+                bary=torch.empty(capacity, dtype=torch.float32, device=device),
+                n_clusters=torch.zeros(1, dtype=i32, device=device))
 
 
 # ---- convenience: allocate outputs on the device (still marshalling only) ---------------------------------------

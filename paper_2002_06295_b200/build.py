@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmkf.so")
-SOURCES = ["mkf_api.cu", "mkf_hit_index.cu", "mkf_build.cu", "mkf_dedup.cu", "mkf_host.cu"]
+SOURCES = ["mkf_api.cu", "mkf_hit_index.cu", "mkf_build.cu", "mkf_dedup.cu", "mkf_strips.cu", "mkf_host.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--shared", "-cudart", "shared"]
 

@@ -5,6 +5,7 @@
 namespace mkf {
 size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits);
 size_t dedup_ws_bytes(int n_hits, int n, int mpl);
+size_t strips_ws_bytes(int n_strips);
 }
 using namespace mkf;
 
@@ -13,6 +14,7 @@ extern "C" size_t mkf_workspace_bytes(const mkf_ctx* c, int call_id, int n_event
   switch (call_id) {
     case MKF_CALL_BUILD_HIT_INDEX: return hit_index_ws_bytes(c, n_events, n_hits);
     case MKF_CALL_REMOVE_DUPLICATES: return dedup_ws_bytes(n_hits, n_seeds, c->max_plan_len);
+    case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits);
     default: return 0;      // fit and build keep everything in registers / shared memory
   }
 }
@@ -132,6 +134,38 @@ extern "C" int mkf_build_host(mkf_ctx* c, const mkf_hits* h, const mkf_states* s
   A.down(hit_ids, dhid, n * max_plan_len); A.down(status, dstat, n);
   if (A.err == cudaSuccess) A.err = cudaStreamSynchronize(A.st);
   if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_build_host");
+  if (h2d_bytes) *h2d_bytes = A.h2d;
+  if (d2h_bytes) *d2h_bytes = A.d2h;
+  return MKF_OK;
+}
+
+extern "C" int mkf_cluster_strips_host(mkf_ctx* c, const mkf_strips* s, const mkf_strip_params* p, const mkf_clusters* out,
+                                       long long* h2d_bytes, long long* d2h_bytes) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!s || !p || !out || s->n_strips < 0 || s->n_modules < 0 || out->capacity < 0 || !out->n_clusters ||
+      (s->n_strips > 0 && (!s->module_off || !s->adc || !s->noise || !s->bad)))
+    return fail(c, MKF_INVALID_ARG, "mkf_cluster_strips_host: bad argument");
+  const size_t n = (size_t)s->n_strips, cap = (size_t)out->capacity;
+  Arena A;
+  mkf_strips ds = *s;
+  ds.module_off = A.up(s->module_off, (size_t)s->n_modules + 1);
+  ds.adc = A.up(s->adc, n); ds.noise = A.up(s->noise, n); ds.bad = A.up(s->bad, n);
+  mkf_clusters dc = *out;
+  dc.module = A.alloc<int>(cap); dc.first = A.alloc<int>(cap); dc.last = A.alloc<int>(cap);
+  dc.charge = A.alloc<unsigned>(cap); dc.bary = A.alloc<float>(cap); dc.n_clusters = A.alloc<int>(1);
+  const size_t wsb = strips_ws_bytes(s->n_strips);
+  char* ws = A.alloc<char>(wsb);
+  if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_cluster_strips_host: staging");
+  const int rc = mkf_cluster_strips(c, &ds, p, &dc, ws, wsb, A.st);
+  if (rc) return rc;
+  A.down(out->n_clusters, dc.n_clusters, 1);
+  if (A.err == cudaSuccess) A.err = cudaStreamSynchronize(A.st);           // the count decides how much comes back
+  if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_cluster_strips_host");
+  const size_t k = (size_t)(*out->n_clusters < out->capacity ? *out->n_clusters : out->capacity);
+  A.down(out->module, dc.module, k); A.down(out->first, dc.first, k); A.down(out->last, dc.last, k);
+  A.down(out->charge, dc.charge, k); A.down(out->bary, dc.bary, k);
+  if (A.err == cudaSuccess) A.err = cudaStreamSynchronize(A.st);
+  if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_cluster_strips_host");
   if (h2d_bytes) *h2d_bytes = A.h2d;
   if (d2h_bytes) *d2h_bytes = A.d2h;
   return MKF_OK;

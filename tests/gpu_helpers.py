@@ -63,3 +63,34 @@ def gpu_build(ev, prm, packed=True, dedup=False):
     r["launches"] = ctx.launch_count()
     ctx.close()
     return r
+
+
+_strip_ctx = None
+
+
+def strip_context():
+    """Clustering uses no geometry; any context will do."""
+    global _strip_ctx
+    if _strip_ctx is None:
+        from paper_2002_06295_b200 import datagen
+        ev, prm = datagen.config(0, scale=0.01)
+        _strip_ctx = B.Context(ev["geom"], prm)
+    return _strip_ctx
+
+
+def gpu_cluster_strips(d, sp, capacity=None):
+    """mkf_cluster_strips on the strips dict of datagen.make_strips; returns numpy arrays cut to the number found."""
+    ctx = strip_context()
+    n = int(d["adc"].shape[0])
+    cap = n // 2 + 1 if capacity is None else capacity
+    sd = B.strips_to_device(d)
+    out = B.alloc_clusters(cap)
+    nb = ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, 0)
+    ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")
+    ctx.cluster_strips(sd, sp, out, ws)
+    torch.cuda.synchronize()
+    k = int(out["n_clusters"].item())
+    res = {key: out[key][:min(k, cap)].cpu().numpy() for key in ("module", "first", "last", "charge", "bary")}
+    res["charge"] = res["charge"].view(np.uint32)
+    res["n_clusters"] = k
+    return res
