@@ -1,7 +1,7 @@
 """bench.py — KF layer-steps/s of mkf_fit on BASELINE.json configs[1] (4 M helices x 17 barrel layers), or built
 events/s of the building path on configs[2..4] (--workload build2|build3|build4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mkf|reference] [--workload fit|build2|build3|build4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mkf|reference] [--workload fit|fitback|build2|build3|build4|strips]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...
 
 One JSON line on rank 0 (contract in DESIGN.md §8). A "step" is one pass of the whole path over the workload with
@@ -28,6 +28,10 @@ FP32_LANES_PER_SM, N_SM = 128, 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one mkf_fit_kernel launch on the full configs[1] workload, from
 # the `ncu --set full` capture summarised in profiles/r1_fit_kernel_ncu.md (3.1226 GB + 0.4689 GB)
 NCU_TRAFFIC_BYTES_FIT_FULL = 3.591e9
+
+
+STRIP_BYTES_IN, STRIP_BYTES_PER_CLUSTER = 7, 20
+NCU_TRAFFIC_BYTES_STRIPS_FULL = None
 
 
 def peaks():
@@ -80,6 +84,33 @@ def make_build_workload(which, seed, scale):
 # ---------------------------------------------------------------------------------------------------------------
 # ranks: events / tracks are independent, so a rank owns its own workload and nothing but timings is exchanged
 # ---------------------------------------------------------------------------------------------------------------
+STRIP_EVENTS, STRIP_MODULES = 16, 15000
+
+
+def make_strip_workload(seed, scale):
+    """STRIP_EVENTS x scale events of STRIP_MODULES modules (about the module count of a strip tracker), generated one
+    event at a time (seeds 64 seed + k) and concatenated: the batch is one flat module list."""
+    from paper_2002_06295_b200 import datagen
+    n_ev = max(1, int(round(STRIP_EVENTS * scale))) if scale >= 1.0 / STRIP_EVENTS else 1
+    n_mod = STRIP_MODULES if scale >= 1.0 / STRIP_EVENTS else max(8, int(round(STRIP_MODULES * STRIP_EVENTS * scale)))
+    parts = [datagen.make_strips(64 * seed + k, n_mod) for k in range(n_ev)]
+    off, base = [np.zeros(1, np.int32)], 0
+    for p in parts:
+        off.append((p["module_off"][1:].astype(np.int64) + base).astype(np.int32)); base += int(p["module_off"][-1])
+    d = dict(module_off=np.concatenate(off), adc=np.concatenate([p["adc"] for p in parts]),
+             noise=np.concatenate([p["noise"] for p in parts]), bad=np.concatenate([p["bad"] for p in parts]))
+    return d, datagen.default_strip_params()
+
+
+def oracle_strip_rate(d, sp, n_modules):
+    from oracle import mkfo
+    ns = int(d["module_off"][n_modules])
+    t = time.perf_counter()
+    r = mkfo.cluster_strips(d["module_off"][:n_modules + 1], d["adc"][:ns], d["noise"][:ns], d["bad"][:ns], **sp)
+    dt = time.perf_counter() - t
+    return ns / dt, dt, 1, r
+
+
 def rank_seed(seed, rank):
     """Seed of the workload a rank owns (weak scaling: every rank generates a full-size workload of its own)."""
     return seed + rank
@@ -181,7 +212,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mkf", choices=["mkf", "reference"])
-    ap.add_argument("--workload", default="fit", choices=["fit", "fitback", "build2", "build3", "build4"])
+    ap.add_argument("--workload", default="fit", choices=["fit", "fitback", "build2", "build3", "build4", "strips"])
     ap.add_argument("--scale", type=float, default=1.0, help="shrinks the workload (testing only; the JSON says so)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -193,12 +224,15 @@ def main():
     warm = max(a.warmup, 3)
     backward = a.workload == "fitback"
     is_fit = a.workload in ("fit", "fitback")
-    metric = "KF layer-steps/s (propagate+update)" if is_fit else "built events/s"
-    unit = "layer-steps/s" if is_fit else "events/s"
+    is_strips = a.workload == "strips"
+    metric = "KF layer-steps/s (propagate+update)" if is_fit else "clustered strips/s" if is_strips else "built events/s"
+    unit = "layer-steps/s" if is_fit else "strips/s" if is_strips else "events/s"
     names = dict(fitback="configs[1] workload, backward fit (SURVEY f1): seeds = forward fit at the last hit, covariance x100",
                  fit="configs[1]: track fit, 4M helices x 17 barrel layers, MS + dE/dx, seeds from 3 hits, cov x100",
                  build2="configs[2]: building, barrel, 100 events x 1000 tracks + 20k noise hits, top 6",
                  build3="configs[3]: building, barrel+endcap, 200 events x 1500 seeds, ~80k hits/event",
+                 strips="strip clustering (SURVEY f3, reading R8): %d events x %d modules of 512 / 256 strips, ~1 %% occupancy, "
+                        "1 %% bad strips" % (STRIP_EVENTS, STRIP_MODULES),
                  build4="configs[4]: batched building + duplicate removal, 64 events x 6000 seeds, ~300k hits/event, top 8")
     cfg = dict(workload=names[a.workload], scale=a.scale, l2="inputs larger than L2 (no flush needed)", seed=a.seed)
 
@@ -215,6 +249,14 @@ def main():
                 if k >= warm:
                     rates.append((rate, dt))
             sample = "first %d helices of the workload per step (%d layer-steps)" % (n_s, steps)
+        elif is_strips:
+            d, sp = make_strip_workload(a.seed, min(1.0, a.scale) * 4.0 / STRIP_EVENTS)
+            rates = []
+            for k in range(warm + a.steps):
+                rate, dt, cores, _ = oracle_strip_rate(d, sp, len(d["module_off"]) - 1)
+                if k >= warm:
+                    rates.append((rate, dt))
+            sample = "%d modules (%d strips) of the workload per step" % (len(d["module_off"]) - 1, len(d["adc"]))
         else:
             which = int(a.workload[-1])
             nev_full = {2: 100, 3: 200, 4: 64}[which]
@@ -282,6 +324,26 @@ def main():
                 return float(res[3].sum()), h2d, sum(t.numel() * t.element_size() for t in res)
             r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"])
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
+    elif is_strips:
+        from paper_2002_06295_b200 import datagen
+        ev_g, prm_g = datagen.config(0, scale=0.001)              # clustering uses no geometry; a context needs one
+        ctx = B.Context(ev_g["geom"], prm_g)
+        sd_host, sp = make_strip_workload(rank_seed(a.seed, rank), a.scale)
+        n = len(sd_host["adc"])
+        cap = n // 8
+        sd = B.strips_to_device(sd_host)
+        out = B.alloc_clusters(cap)
+        ws = torch.empty(max(ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, 0), 256), dtype=torch.uint8, device="cuda")
+
+        def step():
+            ctx.cluster_strips(sd, sp, out, ws)
+
+        def units():
+            return float(n)
+
+        def e2e_step():
+            r = ctx.cluster_strips_host(strips_p, sp, cap)
+            return float(n), r["h2d_bytes"], r["d2h_bytes"]
     else:
         which = int(a.workload[-1])
         ev, prm = make_build_workload(which, rank_seed(a.seed, rank), a.scale)
@@ -338,8 +400,11 @@ def main():
     # ---- end to end through the host-buffer C-ABI call (pinned host memory) --------------------------------------
     def pin(d, keys):
         return {k: torch.from_numpy(np.ascontiguousarray(d[k])).pin_memory().numpy() for k in keys}
-    hits_p = pin(hits, ["layer_off", "x", "y", "z", "V"]); hits_p["n_events"] = hits["n_events"]
-    seeds_p = pin(seeds, list(seeds.keys()))
+    if is_strips:
+        strips_p = pin(sd_host, ["module_off", "adc", "noise", "bad"])
+    else:
+        hits_p = pin(hits, ["layer_off", "x", "y", "z", "V"]); hits_p["n_events"] = hits["n_events"]
+        seeds_p = pin(seeds, list(seeds.keys()))
     e2e_step()                                            # warm the stream-ordered pool
     barrier()
     te = time.perf_counter()
@@ -364,6 +429,14 @@ def main():
                     algorithmic_flop_per_layer_step=ALGO_FLOP_PER_LAYER_STEP,
                     hbm=dict(achieved=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
                              frac=ALGO_BYTES_PER_LAYER_STEP * steps_per_launch / t_launch / 1e9 / pk["hbm_gbs"]))
+    elif is_strips:
+        nclu = int(out["n_clusters"].item())
+        algo = STRIP_BYTES_IN * u + STRIP_BYTES_PER_CLUSTER * nclu
+        t_launch = ms_total / a.steps * 1e-3
+        roof = dict(bound="hbm", kernel="sc_cluster_kernel", achieved=algo / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
+                    frac=algo / t_launch / 1e9 / pk["hbm_gbs"], traffic=NCU_TRAFFIC_BYTES_STRIPS_FULL if a.scale == 1.0 else None,
+                    algorithmic_bytes=algo, clusters=nclu, peak_source=pk["source"],
+                    note="7 B per strip in (adc u16, noise f32, bad u8) + 20 B per cluster out; the timed step also holds one memset of the tile states")
     else:
         roof = dict(bound="hbm", kernel="mkf_build_kernel", achieved=None, peak=pk["hbm_gbs"], unit="GB/s", frac=None, traffic=None,
                     note="building is reported, not held to the 50% bar (BASELINE.json north_star); see DESIGN.md §6")
@@ -386,6 +459,14 @@ def main():
                                  cov_max=float(parity.cov_errors(g["cov"], r["cov"], r["par"], kinds)[ok].max()),
                                  chi2_max=float(parity.chi2_errors(g["chi2"], r["chi2"])[ok].max()),
                                  tol=dict(par=parity.TOL_PAR, cov=parity.TOL_COV, chi2=parity.TOL_CHI2))
+        elif is_strips:
+            nm = len(sd_host["module_off"]) - 1
+            rate, dt, cores, r = oracle_strip_rate(sd_host, sp, nm)
+            cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="the whole workload, %d strips (%.1f s)" % (n, dt))
+            k = len(r["module"])
+            g = {key: out[key][:k].cpu().numpy() for key in ("module", "first", "last", "charge", "bary")}
+            cpu["parity"] = dict(n_clusters_oracle=k, n_clusters_identical=bool(k == nclu),
+                                 identical=bool(k == nclu and all(np.array_equal(g[key].view(np.uint32), r[key].view(np.uint32)) for key in g)))
         else:
             n_ev = min(nev, 4)
             rate, dt, cores, r, m = oracle_build_rate(ev, prm, n_ev, dedup)
@@ -396,7 +477,7 @@ def main():
                                  mismatches_with_margin_above_1e_3=int((r["margin"][~same] >= 1e-3).sum()),
                                  chi2_max=float((np.abs(out["chi2"].cpu().numpy()[m] - r["chi2"]) / np.maximum(r["chi2"], 1.0))[same].max()))
     print(json.dumps(dict(metric=metric, value=value, unit=unit, n_gpus=world, steps=a.steps, warmup=warm, ms_per_step=ms_step,
-                          higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic", config=cfg,
+                          higher_is_better=True, scaling="weak", vs_baseline=None, dtype="u16/f32" if is_strips else "f32", data="synthetic", config=cfg,
                           clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, cpu_baseline=cpu, impl="mkf",
                           units_per_step=u_all)))
 

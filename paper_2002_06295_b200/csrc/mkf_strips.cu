@@ -18,6 +18,9 @@ namespace mkf {
 
 constexpr int SC_THREADS = 256, SC_PER = 8, SC_TILE = SC_THREADS * SC_PER, SC_HALO = 32;
 constexpr int SC_MS_WORDS = (SC_TILE + SC_HALO) / 32;
+#ifndef SC_MIN_BLOCKS
+#define SC_MIN_BLOCKS 6
+#endif
 
 struct ScArgs {
   int n_modules, n_strips, n_tiles;
@@ -26,6 +29,7 @@ struct ScArgs {
   int cap; int *o_module, *o_first, *o_last; unsigned* o_charge; float* o_bary; int* n_clusters;
   unsigned long long* tile_state;       // [n_tiles]: flag << 32 | value; flag 1 = tile aggregate, 2 = inclusive prefix
   unsigned* ticket;
+  const int* tile_mod;                  // [n_tiles]: module of the first strip of the tile's window
 };
 
 // largest m in [lo, hi) with moff[m] <= g (moff ascending; hi > lo and moff[lo] <= g)
@@ -63,28 +67,69 @@ __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pa
   }
 }
 
-__global__ void __launch_bounds__(SC_THREADS) sc_cluster_kernel(const ScArgs a) {
+// tile t -> the module that holds the first strip of its window, max(t * SC_TILE - SC_HALO, 0). One thread per module.
+__global__ void sc_tile_module_kernel(int n_modules, int n_tiles, const int* __restrict__ moff, int* __restrict__ tile_mod) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n_modules) return;
+  const int b = moff[m], e = moff[m + 1];
+  if (e <= b) return;
+  if (b == 0) tile_mod[0] = m;
+  const int tlo = max((b + SC_HALO + SC_TILE - 1) / SC_TILE, 1), thi = min((e - 1 + SC_HALO) / SC_TILE, n_tiles - 1);
+  for (int t = tlo; t <= thi; t++) tile_mod[t] = m;
+}
+
+struct ScRecord { int module, first, last; unsigned charge; float bary; };
+
+// R8 in strip order for the cluster that starts at strip g (a passing strip). Returns whether it is kept.
+__device__ __forceinline__ bool sc_walk(const ScArgs& a, int mlo, int mhi, int g, double cut, ScRecord& r) {
+  const int m = module_of(a.moff, mlo, mhi, g);
+  const int b = __ldg(a.moff + m), e = __ldg(a.moff + m + 1);
+  int j = g, last = g, holes = 0, nbad = 0;
+  bool seed = false;
+  unsigned long long q2 = 0, s1 = 0; unsigned charge = 0; double n2 = 0.0;
+  while (j < e) {
+    const unsigned adc = __ldg(a.adc + j); const float nz = __ldg(a.noise + j); const bool bd = __ldg(a.bad + j) != 0;
+    if (!bd && (float)adc > a.chan_thr * nz) {
+      last = j; holes = 0; nbad = 0;
+      seed |= (float)adc > a.seed_thr * nz;
+      q2 += adc * adc; charge += adc; s1 += (unsigned long long)adc * (unsigned)(j - b);
+      n2 = __dadd_rn(n2, __dmul_rn((double)nz, (double)nz));
+    } else {
+      if (bd) nbad++; else holes++;
+      if (holes > a.max_holes || nbad > a.max_bad) break;
+    }
+    j++;
+  }
+  if (!(seed && (double)q2 > __dmul_rn(cut, n2) && (long long)charge >= (long long)a.min_charge)) return false;
+  r.module = m; r.first = g - b; r.last = last - b; r.charge = charge;
+  r.bary = (float)__ddiv_rn(__dmul_rn((double)(2ull * s1 + charge), 0.5), (double)charge);
+  return true;
+}
+
+// sum and exclusive prefix (for this warp) of the SC_THREADS / 32 per-warp counts in s_w
+__device__ __forceinline__ void warp_counts(const int* s_w, int lane, int warp, int& before, int& total) {
+  const int v = lane < SC_THREADS / 32 ? s_w[lane] : 0;
+  int incl = v;
+#pragma unroll
+  for (int d = 1; d < SC_THREADS / 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+  total = __shfl_sync(0xffffffffu, incl, SC_THREADS / 32 - 1);
+  before = __shfl_sync(0xffffffffu, incl - v, warp);
+}
+
+__global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(const ScArgs a) {
   __shared__ unsigned char s_pass[SC_THREADS + 4], s_bad[SC_THREADS + 4];     // chunk c of the tile at [c + 4]; halo at [0..3]
   __shared__ unsigned s_ms[SC_MS_WORDS + 1];                                   // module-start bits, strip wbase + i at bit i
-  __shared__ int st_module[SC_TILE], st_first[SC_TILE], st_last[SC_TILE];     // staged cluster records, in strip order
-  __shared__ unsigned st_charge[SC_TILE];
-  __shared__ float st_bary[SC_TILE];
-  __shared__ int s_tile, s_mlo, s_mhi, s_kept, s_prefix, s_wsum[SC_THREADS / 32];
+  __shared__ unsigned short s_start[SC_TILE];                                  // cluster starts of the tile (tile-relative), ascending
+  __shared__ int s_tile, s_prefix, s_wa[SC_THREADS / 32], s_wb[SC_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-  if (tid == 0) { s_tile = (int)atomicAdd(a.ticket, 1u); s_kept = 0; }
+  if (tid == 0) s_tile = (int)atomicAdd(a.ticket, 1u);
   if (tid <= SC_MS_WORDS) s_ms[tid] = 0;
   __syncthreads();
   const int tile = s_tile;
   const int t0 = tile * SC_TILE, t1 = min(t0 + SC_TILE, a.n_strips);
-  const int wbase = t0 - SC_HALO;                                             // may be negative for tile 0
-  // modules that touch [max(wbase, 0), t1): m in [mlo, mhi)
-  if (tid == 0) s_mlo = module_of(a.moff, 0, a.n_modules, max(wbase, 0));
-  if (tid == 32) {                                                            // first m in [0, n_modules] with moff[m] >= t1
-    int lo = 0, hi = a.n_modules;                                             // moff[0] = 0 < t1 <= moff[n_modules]
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(a.moff + mid) < t1) lo = mid; else hi = mid; }
-    s_mhi = hi;
-  }
+  const int wbase = t0 - SC_HALO;                                             // negative for tile 0
+  const int mlo = __ldg(a.tile_mod + tile);
   // threshold bits: own chunk and (threads 0..3) the halo chunks
   const int g0 = t0 + tid * SC_PER;
   unsigned pass, bad;
@@ -95,13 +140,17 @@ __global__ void __launch_bounds__(SC_THREADS) sc_cluster_kernel(const ScArgs a) 
     if (tile > 0) strip_bits(a, wbase + tid * SC_PER, hp, hb);
     s_pass[tid] = (unsigned char)hp; s_bad[tid] = (unsigned char)hb;
   }
-  __syncthreads();
-  const int mlo = s_mlo, mhi = s_mhi;
-  for (int m = mlo + tid; m < mhi; m += SC_THREADS) {
-    const int pos = __ldg(a.moff + m) - wbase;
-    if (pos >= 0 && pos < SC_TILE + SC_HALO) atomicOr(&s_ms[pos >> 5], 1u << (pos & 31));
+  // modules that start before the end of the tile: m in [mlo, mhi); their first strips are marked in s_ms
+  int mhi = mlo;
+  for (int m0 = mlo;; m0 += SC_THREADS) {
+    const int m = m0 + tid;
+    int off = 0;
+    const bool in = m < a.n_modules && (off = __ldg(a.moff + m)) < t1;
+    if (in && off >= wbase) atomicOr(&s_ms[(off - wbase) >> 5], 1u << ((off - wbase) & 31));
+    const int c = __syncthreads_count(in);
+    mhi += c;
+    if (c < SC_THREADS) break;
   }
-  __syncthreads();
 
   // ---- which of my passing strips start a cluster: window bit 32 + k = my strip k, bit 31 = the strip before ...
   unsigned starts = 0;
@@ -113,108 +162,114 @@ __global__ void __launch_bounds__(SC_THREADS) sc_cluster_kernel(const ScArgs a) 
     const int wi = tid >> 2, sh = (tid & 3) * 8;
     const unsigned long long wm = ((unsigned long long)s_ms[wi] | ((unsigned long long)s_ms[wi + 1] << 32)) >> sh;
     for (unsigned rest = pass; rest; rest &= rest - 1) {
-      const int k = __ffs(rest) - 1;
-      int pos = 32 + k, holes = 0, nbad = 0;
+      const int k = __ffs(rest) - 1, P = 32 + k;
+      const unsigned long long below = wp & ((1ull << P) - 1ull);
       bool is_start = true;
-      while (!((wm >> pos) & 1ull) && pos > 0) {          // stop at the first strip of the module
-        pos--;
-        if ((wp >> pos) & 1ull) { is_start = false; break; }
-        if ((wb >> pos) & 1ull) nbad++; else holes++;
-        if (holes > a.max_holes || nbad > a.max_bad) break;
+      if (below) {                                      // p: the nearest passing strip before P
+        const int p = 63 - __clzll((long long)below);
+        const unsigned long long upto_p = (2ull << p) - 1ull;
+        const int nb = __popcll(wb & ((1ull << P) - 1ull) & ~upto_p);
+        const bool boundary = (wm & ((2ull << P) - 1ull) & ~upto_p) != 0;      // a module starts in (p, P]
+        is_start = boundary || nb > a.max_bad || (P - p - 1 - nb) > a.max_holes;
       }
       starts |= (unsigned)is_start << k;
     }
   }
-  // exclusive scan of the number of starts per thread -> staging slot
+  // exclusive scan of the number of starts per thread -> slot in the list of starts
   const int ns = __popc(starts);
   int incl = ns;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
-  if (lane == 31) s_wsum[warp] = incl;
+  if (lane == 31) s_wa[warp] = incl;
   __syncthreads();
-  int slot = incl - ns, nstart = 0;
-#pragma unroll
-  for (int w = 0; w < SC_THREADS / 32; w++) { const int v = s_wsum[w]; if (w < warp) slot += v; nstart += v; }
-
-  // ---- walk each cluster that starts in my chunk, in strip order (R8), and stage its record
-  int nkept = 0;
+  int before, nstart;
+  warp_counts(s_wa, lane, warp, before, nstart);
   {
-    int m = -1, b = 0, e = 0;
-    const double cut = __dmul_rn((double)a.clus_thr, (double)a.clus_thr);
-    for (unsigned rest = starts; rest; rest &= rest - 1, slot++) {
-      const int g = g0 + __ffs(rest) - 1;
-      if (g >= e) { m = module_of(a.moff, mlo, mhi, g); b = __ldg(a.moff + m); e = __ldg(a.moff + m + 1); }
-      int j = g, last = g, holes = 0, nbad = 0;
-      bool seed = false;
-      unsigned long long q2 = 0, s1 = 0; unsigned charge = 0; double n2 = 0.0;
-      while (j < e) {
-        const unsigned adc = __ldg(a.adc + j); const float nz = __ldg(a.noise + j); const bool bd = __ldg(a.bad + j) != 0;
-        if (!bd && (float)adc > a.chan_thr * nz) {
-          last = j; holes = 0; nbad = 0;
-          seed |= (float)adc > a.seed_thr * nz;
-          q2 += adc * adc; charge += adc; s1 += (unsigned long long)adc * (unsigned)(j - b);
-          n2 = __dadd_rn(n2, __dmul_rn((double)nz, (double)nz));
-        } else {
-          if (bd) nbad++; else holes++;
-          if (holes > a.max_holes || nbad > a.max_bad) break;
-        }
-        j++;
-      }
-      const bool kept = seed && (double)q2 > __dmul_rn(cut, n2) && (long long)charge >= (long long)a.min_charge;
-      st_module[slot] = kept ? m : -1;
-      if (kept) {
-        st_first[slot] = g - b; st_last[slot] = last - b; st_charge[slot] = charge;
-        st_bary[slot] = (float)__ddiv_rn(__dmul_rn((double)(2ull * s1 + charge), 0.5), (double)charge);
-        nkept++;
-      }
-    }
+    int slot = before + incl - ns;
+    for (unsigned rest = starts; rest; rest &= rest - 1) s_start[slot++] = (unsigned short)(tid * SC_PER + __ffs(rest) - 1);
   }
-  if (nkept) atomicAdd(&s_kept, nkept);
   __syncthreads();
 
-  // ---- decoupled look-back over the tiles: exclusive prefix of the kept counts
-  if (tid == 0) {
-    const unsigned long long mine = (unsigned)s_kept;
+  // ---- one cluster per thread: walk it; count the kept ones
+  const double cut = __dmul_rn((double)a.clus_thr, (double)a.clus_thr);
+  const int rounds = (nstart + SC_THREADS - 1) / SC_THREADS;
+  ScRecord rec;
+  bool kept = false;
+  int kept_before = 0, nkept = 0;                      // (single round) kept clusters of the lower warps; of the tile
+  for (int r = 0; r < rounds; r++) {
+    const int s = r * SC_THREADS + tid;
+    kept = s < nstart && sc_walk(a, mlo, mhi, t0 + s_start[s], cut, rec);
+    const unsigned bal = __ballot_sync(0xffffffffu, kept);
+    if (r > 0) __syncthreads();
+    if (lane == 0) s_wb[warp] = __popc(bal);
+    __syncthreads();
+    int tot;
+    warp_counts(s_wb, lane, warp, kept_before, tot);
+    kept_before += __popc(bal & ((1u << lane) - 1u));
+    nkept += tot;
+  }
+
+  // ---- decoupled look-back over the tiles (warp 0): exclusive prefix of the kept counts
+  if (warp == 0) {
     volatile unsigned long long* st = a.tile_state;
     unsigned excl = 0;
     if (tile > 0) {
-      st[tile] = (1ull << 32) | mine;
-      for (int i = tile - 1; i >= 0; i--) {
+      if (lane == 0) st[tile] = (1ull << 32) | (unsigned)nkept;
+      for (int top = tile - 1;; top -= 32) {
+        const int i = top - lane;
         unsigned long long v;
-        do { v = st[i]; } while ((v >> 32) == 0);
-        excl += (unsigned)v;
-        if ((v >> 32) == 2) break;
+        unsigned need, inc;
+        do {
+          v = i >= 0 ? st[i] : (2ull << 32);           // before tile 0: an inclusive prefix of 0
+          const unsigned ready = __ballot_sync(0xffffffffu, (v >> 32) != 0);
+          inc = __ballot_sync(0xffffffffu, (v >> 32) == 2);
+          need = inc ? 0xffffffffu >> (32 - __ffs(inc)) : 0xffffffffu;    // lanes up to the nearest inclusive prefix
+          if ((ready & need) == need) break;
+        } while (true);
+        unsigned c = ((need >> lane) & 1u) ? (unsigned)v : 0u;
+#pragma unroll
+        for (int d = 16; d; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+        excl += c;
+        if (inc) break;
       }
     }
-    st[tile] = (2ull << 32) | (unsigned long long)(excl + (unsigned)mine);
-    s_prefix = (int)excl;
-    if (tile == a.n_tiles - 1) *a.n_clusters = (int)(excl + (unsigned)mine);
+    if (lane == 0) {
+      st[tile] = (2ull << 32) | (unsigned long long)(excl + (unsigned)nkept);
+      s_prefix = (int)excl;
+      if (tile == a.n_tiles - 1) *a.n_clusters = (int)(excl + (unsigned)nkept);
+    }
   }
   __syncthreads();
 
-  // ---- ordered compaction of the staged records
+  // ---- write the kept clusters in (module, first strip) order
   int base = s_prefix;
-  for (int c0 = 0; c0 < nstart; c0 += SC_THREADS) {
-    const int s = c0 + tid;
-    const bool f = s < nstart && st_module[s] >= 0;
-    const unsigned bal = __ballot_sync(0xffffffffu, f);
-    __syncthreads();                                     // s_wsum of the previous round has been read
-    if (lane == 0) s_wsum[warp] = __popc(bal);
-    __syncthreads();
-    int off = base + __popc(bal & ((1u << lane) - 1u)), tot = 0;
-#pragma unroll
-    for (int w = 0; w < SC_THREADS / 32; w++) { const int v = s_wsum[w]; if (w < warp) off += v; tot += v; }
-    if (f && off < a.cap) {
-      a.o_module[off] = st_module[s]; a.o_first[off] = st_first[s]; a.o_last[off] = st_last[s];
-      a.o_charge[off] = st_charge[s]; a.o_bary[off] = st_bary[s];
+  if (rounds <= 1) {
+    const int off = base + kept_before;
+    if (kept && off < a.cap) {
+      a.o_module[off] = rec.module; a.o_first[off] = rec.first; a.o_last[off] = rec.last; a.o_charge[off] = rec.charge; a.o_bary[off] = rec.bary;
     }
-    base += tot;
+  } else {                                             // rare: more starts than threads -> walk again, round by round
+    for (int r = 0; r < rounds; r++) {
+      const int s = r * SC_THREADS + tid;
+      kept = s < nstart && sc_walk(a, mlo, mhi, t0 + s_start[s], cut, rec);
+      const unsigned bal = __ballot_sync(0xffffffffu, kept);
+      __syncthreads();
+      if (lane == 0) s_wb[warp] = __popc(bal);
+      __syncthreads();
+      int tot;
+      warp_counts(s_wb, lane, warp, kept_before, tot);
+      const int off = base + kept_before + __popc(bal & ((1u << lane) - 1u));
+      if (kept && off < a.cap) {
+        a.o_module[off] = rec.module; a.o_first[off] = rec.first; a.o_last[off] = rec.last; a.o_charge[off] = rec.charge; a.o_bary[off] = rec.bary;
+      }
+      base += tot;
+    }
   }
 }
 
 size_t strips_ws_bytes(int n_strips) {
   const size_t n_tiles = ((size_t)n_strips + SC_TILE - 1) / SC_TILE;
-  return align256(n_tiles * sizeof(unsigned long long)) + 256;
+  return align256(n_tiles * sizeof(unsigned long long)) + 256 + align256(n_tiles * sizeof(int));
 }
 }  // namespace mkf
 using namespace mkf;
@@ -248,8 +303,12 @@ extern "C" int mkf_cluster_strips(mkf_ctx* c, const mkf_strips* s, const mkf_str
   a.o_charge = out->charge; a.o_bary = out->bary; a.n_clusters = out->n_clusters;
   a.tile_state = (unsigned long long*)ws;
   a.ticket = (unsigned*)((char*)ws + align256((size_t)a.n_tiles * sizeof(unsigned long long)));
-  cudaError_t e = cudaMemsetAsync(ws, 0, need, st);
+  int* tile_mod = (int*)((char*)a.ticket + 256);
+  a.tile_mod = tile_mod;
+  cudaError_t e = cudaMemsetAsync(ws, 0, align256((size_t)a.n_tiles * sizeof(unsigned long long)) + 256, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_cluster_strips: memset");
+  sc_tile_module_kernel<<<(a.n_modules + 255) / 256, 256, 0, st>>>(a.n_modules, a.n_tiles, a.moff, tile_mod);
+  MKF_LAUNCHED(c, "sc_tile_module_kernel");
   sc_cluster_kernel<<<a.n_tiles, SC_THREADS, 0, st>>>(a);
   MKF_LAUNCHED(c, "sc_cluster_kernel");
   return MKF_OK;
