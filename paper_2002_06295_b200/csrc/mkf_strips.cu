@@ -16,7 +16,10 @@
 
 namespace mkf {
 
-constexpr int SC_THREADS = 256, SC_PER = 8, SC_TILE = SC_THREADS * SC_PER, SC_HALO = 32;
+#ifndef SC_SUB
+#define SC_SUB 4
+#endif
+constexpr int SC_THREADS = 256, SC_PER = 8, SC_CHUNKS = SC_THREADS * SC_SUB, SC_TILE = SC_CHUNKS * SC_PER, SC_HALO = 32;
 constexpr int SC_MS_WORDS = (SC_TILE + SC_HALO) / 32;
 #ifndef SC_MIN_BLOCKS
 #define SC_MIN_BLOCKS 6
@@ -80,29 +83,46 @@ __global__ void sc_tile_module_kernel(int n_modules, int n_tiles, const int* __r
 
 struct ScRecord { int module, first, last; unsigned charge; float bary; };
 
-// R8 in strip order for the cluster that starts at strip g (a passing strip). Returns whether it is kept.
-__device__ __forceinline__ bool sc_walk(const ScArgs& a, int mlo, int mhi, int g, double cut, ScRecord& r) {
-  const int m = module_of(a.moff, mlo, mhi, g);
-  const int b = __ldg(a.moff + m), e = __ldg(a.moff + m + 1);
-  int j = g, last = g, holes = 0, nbad = 0;
-  bool seed = false;
-  unsigned long long q2 = 0, s1 = 0; unsigned charge = 0; double n2 = 0.0;
-  while (j < e) {
-    const unsigned adc = __ldg(a.adc + j); const float nz = __ldg(a.noise + j); const bool bd = __ldg(a.bad + j) != 0;
-    if (!bd && (float)adc > a.chan_thr * nz) {
-      last = j; holes = 0; nbad = 0;
-      seed |= (float)adc > a.seed_thr * nz;
-      q2 += adc * adc; charge += adc; s1 += (unsigned long long)adc * (unsigned)(j - b);
-      n2 = __dadd_rn(n2, __dmul_rn((double)nz, (double)nz));
-    } else {
-      if (bd) nbad++; else holes++;
-      if (holes > a.max_holes || nbad > a.max_bad) break;
-    }
-    j++;
+// largest k in [0, n) with s_off[k] <= g (shared copy of module_off[mlo ..]; s_off[0] <= g)
+__device__ __forceinline__ int module_of_shared(const int* s_off, int n, int g) {
+  int lo = 0, hi = n;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_off[mid] <= g) lo = mid; else hi = mid; }
+  return lo;
+}
+
+struct ScSums { int last, holes, nbad; bool seed, open; unsigned long long q2, s1; unsigned charge; double n2; };
+
+// one strip of the walk of R8 (strip order); open = false once the gap rule has closed the cluster
+__device__ __forceinline__ void sc_strip(const ScArgs& a, ScSums& w, int j, int b, unsigned adc, float nz, bool bd) {
+  if (!bd && (float)adc > a.chan_thr * nz) {
+    w.last = j; w.holes = 0; w.nbad = 0;
+    w.seed |= (float)adc > a.seed_thr * nz;
+    w.q2 += adc * adc; w.charge += adc; w.s1 += (unsigned long long)adc * (unsigned)(j - b);
+    w.n2 = __dadd_rn(w.n2, __dmul_rn((double)nz, (double)nz));
+  } else {
+    if (bd) w.nbad++; else w.holes++;
+    if (w.holes > a.max_holes || w.nbad > a.max_bad) w.open = false;
   }
-  if (!(seed && (double)q2 > __dmul_rn(cut, n2) && (long long)charge >= (long long)a.min_charge)) return false;
-  r.module = m; r.first = g - b; r.last = last - b; r.charge = charge;
-  r.bary = (float)__ddiv_rn(__dmul_rn((double)(2ull * s1 + charge), 0.5), (double)charge);
+}
+
+// R8 in strip order for the cluster that starts at strip g (a passing strip) of module m = [b, e). Returns whether
+// it is kept. The first SC_PRE strips are loaded together (one round trip for the usual short cluster).
+constexpr int SC_PRE = 4;
+__device__ __forceinline__ bool sc_walk(const ScArgs& a, int m, int b, int e, int g, double cut, ScRecord& r) {
+  unsigned av[SC_PRE]; float nv[SC_PRE]; unsigned char bv[SC_PRE];
+#pragma unroll
+  for (int q = 0; q < SC_PRE; q++) {
+    const bool in = g + q < e;
+    av[q] = in ? __ldg(a.adc + g + q) : 0u; nv[q] = in ? __ldg(a.noise + g + q) : 0.0f; bv[q] = in ? __ldg(a.bad + g + q) : (unsigned char)0;
+  }
+  ScSums w; w.last = g; w.holes = 0; w.nbad = 0; w.seed = false; w.open = true; w.q2 = 0; w.s1 = 0; w.charge = 0; w.n2 = 0.0;
+#pragma unroll
+  for (int q = 0; q < SC_PRE; q++)
+    if (w.open && g + q < e) sc_strip(a, w, g + q, b, av[q], nv[q], bv[q] != 0);
+  for (int j = g + SC_PRE; w.open && j < e; j++) sc_strip(a, w, j, b, __ldg(a.adc + j), __ldg(a.noise + j), __ldg(a.bad + j) != 0);
+  if (!(w.seed && (double)w.q2 > __dmul_rn(cut, w.n2) && (long long)w.charge >= (long long)a.min_charge)) return false;
+  r.module = m; r.first = g - b; r.last = w.last - b; r.charge = w.charge;
+  r.bary = (float)__ddiv_rn(__dmul_rn((double)(2ull * w.s1 + w.charge), 0.5), (double)w.charge);
   return true;
 }
 
@@ -116,25 +136,32 @@ __device__ __forceinline__ void warp_counts(const int* s_w, int lane, int warp, 
   before = __shfl_sync(0xffffffffu, incl - v, warp);
 }
 
+constexpr int SC_MOFF = SC_THREADS;                       // module offsets of the tile kept in shared memory
+
 __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(const ScArgs a) {
-  __shared__ unsigned char s_pass[SC_THREADS + 4], s_bad[SC_THREADS + 4];     // chunk c of the tile at [c + 4]; halo at [0..3]
-  __shared__ unsigned s_ms[SC_MS_WORDS + 1];                                   // module-start bits, strip wbase + i at bit i
+  __shared__ unsigned char s_pass[SC_CHUNKS + 4], s_bad[SC_CHUNKS + 4];       // chunk c of the tile at [c + 4]; halo at [0..3]
+  __shared__ unsigned s_ms[SC_MS_WORDS + 2];                                   // module-start bits, strip wbase + i at bit i
   __shared__ unsigned short s_start[SC_TILE];                                  // cluster starts of the tile (tile-relative), ascending
-  __shared__ int s_tile, s_prefix, s_wa[SC_THREADS / 32], s_wb[SC_THREADS / 32];
+  __shared__ int s_moff[SC_MOFF];                                              // module_off[mlo + i]
+  __shared__ unsigned long long s_wa[SC_THREADS / 32];
+  __shared__ int s_tile, s_prefix, s_wb[SC_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   if (tid == 0) s_tile = (int)atomicAdd(a.ticket, 1u);
-  if (tid <= SC_MS_WORDS) s_ms[tid] = 0;
+  for (int i = tid; i < SC_MS_WORDS + 2; i += SC_THREADS) s_ms[i] = 0;
   __syncthreads();
   const int tile = s_tile;
   const int t0 = tile * SC_TILE, t1 = min(t0 + SC_TILE, a.n_strips);
   const int wbase = t0 - SC_HALO;                                             // negative for tile 0
   const int mlo = __ldg(a.tile_mod + tile);
-  // threshold bits: own chunk and (threads 0..3) the halo chunks
-  const int g0 = t0 + tid * SC_PER;
-  unsigned pass, bad;
-  strip_bits(a, g0, pass, bad);
-  s_pass[tid + 4] = (unsigned char)pass; s_bad[tid + 4] = (unsigned char)bad;
+  // threshold bits: own chunks (chunk c = sub * SC_THREADS + tid holds strips t0 + 8 c ..) and (threads 0..3) the halo
+  unsigned pass[SC_SUB], bad[SC_SUB];
+#pragma unroll
+  for (int u = 0; u < SC_SUB; u++) {
+    const int c = u * SC_THREADS + tid;
+    strip_bits(a, t0 + c * SC_PER, pass[u], bad[u]);
+    s_pass[c + 4] = (unsigned char)pass[u]; s_bad[c + 4] = (unsigned char)bad[u];
+  }
   if (tid < 4) {
     unsigned hp = 0, hb = 0;
     if (tile > 0) strip_bits(a, wbase + tid * SC_PER, hp, hb);
@@ -144,24 +171,29 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
   int mhi = mlo;
   for (int m0 = mlo;; m0 += SC_THREADS) {
     const int m = m0 + tid;
-    int off = 0;
-    const bool in = m < a.n_modules && (off = __ldg(a.moff + m)) < t1;
+    const int off = m <= a.n_modules ? __ldg(a.moff + m) : 0x7fffffff;
+    if (m0 == mlo) s_moff[tid] = off;
+    const bool in = m < a.n_modules && off < t1;
     if (in && off >= wbase) atomicOr(&s_ms[(off - wbase) >> 5], 1u << ((off - wbase) & 31));
     const int c = __syncthreads_count(in);
     mhi += c;
     if (c < SC_THREADS) break;
   }
+  const bool moff_shared = mhi - mlo < SC_MOFF;        // then s_moff holds module_off[mlo .. mhi]
 
-  // ---- which of my passing strips start a cluster: window bit 32 + k = my strip k, bit 31 = the strip before ...
-  unsigned starts = 0;
-  if (pass) {
-    const unsigned long long wp = (unsigned long long)s_pass[tid] | ((unsigned long long)s_pass[tid + 1] << 8) |
-        ((unsigned long long)s_pass[tid + 2] << 16) | ((unsigned long long)s_pass[tid + 3] << 24) | ((unsigned long long)pass << 32);
-    const unsigned long long wb = (unsigned long long)s_bad[tid] | ((unsigned long long)s_bad[tid + 1] << 8) |
-        ((unsigned long long)s_bad[tid + 2] << 16) | ((unsigned long long)s_bad[tid + 3] << 24) | ((unsigned long long)bad << 32);
-    const int wi = tid >> 2, sh = (tid & 3) * 8;
+  // ---- which of my passing strips start a cluster: window bit 32 + k = strip k of the chunk, bit 31 = the strip before ...
+  unsigned starts = 0;                                 // 8 bits per chunk
+#pragma unroll
+  for (int u = 0; u < SC_SUB; u++) {
+    if (pass[u] == 0) continue;
+    const int c = u * SC_THREADS + tid;
+    const unsigned long long wp = (unsigned long long)s_pass[c] | ((unsigned long long)s_pass[c + 1] << 8) |
+        ((unsigned long long)s_pass[c + 2] << 16) | ((unsigned long long)s_pass[c + 3] << 24) | ((unsigned long long)pass[u] << 32);
+    const unsigned long long wb = (unsigned long long)s_bad[c] | ((unsigned long long)s_bad[c + 1] << 8) |
+        ((unsigned long long)s_bad[c + 2] << 16) | ((unsigned long long)s_bad[c + 3] << 24) | ((unsigned long long)bad[u] << 32);
+    const int wi = c >> 2, sh = (c & 3) * 8;
     const unsigned long long wm = ((unsigned long long)s_ms[wi] | ((unsigned long long)s_ms[wi + 1] << 32)) >> sh;
-    for (unsigned rest = pass; rest; rest &= rest - 1) {
+    for (unsigned rest = pass[u]; rest; rest &= rest - 1) {
       const int k = __ffs(rest) - 1, P = 32 + k;
       const unsigned long long below = wp & ((1ull << P) - 1ull);
       bool is_start = true;
@@ -172,33 +204,54 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
         const bool boundary = (wm & ((2ull << P) - 1ull) & ~upto_p) != 0;      // a module starts in (p, P]
         is_start = boundary || nb > a.max_bad || (P - p - 1 - nb) > a.max_holes;
       }
-      starts |= (unsigned)is_start << k;
+      starts |= (unsigned)is_start << (8 * u + k);
     }
   }
-  // exclusive scan of the number of starts per thread -> slot in the list of starts
-  const int ns = __popc(starts);
-  int incl = ns;
+  // exclusive scan of the starts per (sub-tile, thread), all sub-tiles at once: 16 bits of a 64-bit word each
+  unsigned long long cnt = 0;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
+  for (int u = 0; u < SC_SUB; u++) cnt |= (unsigned long long)__popc((starts >> (8 * u)) & 0xffu) << (16 * u);
+  unsigned long long incl = cnt;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const unsigned long long v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
   if (lane == 31) s_wa[warp] = incl;
   __syncthreads();
-  int before, nstart;
-  warp_counts(s_wa, lane, warp, before, nstart);
+  int nstart;
   {
-    int slot = before + incl - ns;
-    for (unsigned rest = starts; rest; rest &= rest - 1) s_start[slot++] = (unsigned short)(tid * SC_PER + __ffs(rest) - 1);
+    const unsigned long long v = lane < SC_THREADS / 32 ? s_wa[lane] : 0ull;
+    unsigned long long wi = v;
+#pragma unroll
+    for (int d = 1; d < SC_THREADS / 32; d <<= 1) { const unsigned long long t = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += t; }
+    const unsigned long long total = __shfl_sync(0xffffffffu, wi, SC_THREADS / 32 - 1);
+    const unsigned long long mine = __shfl_sync(0xffffffffu, wi - v, warp) + incl - cnt;   // starts before me, per sub-tile
+    int base = 0;
+#pragma unroll
+    for (int u = 0; u < SC_SUB; u++) {
+      int slot = base + (int)((mine >> (16 * u)) & 0xffffu);
+      const int c = u * SC_THREADS + tid;
+      for (unsigned rest = (starts >> (8 * u)) & 0xffu; rest; rest &= rest - 1) s_start[slot++] = (unsigned short)(c * SC_PER + __ffs(rest) - 1);
+      base += (int)((total >> (16 * u)) & 0xffffu);
+    }
+    nstart = base;
   }
   __syncthreads();
 
   // ---- one cluster per thread: walk it; count the kept ones
   const double cut = __dmul_rn((double)a.clus_thr, (double)a.clus_thr);
   const int rounds = (nstart + SC_THREADS - 1) / SC_THREADS;
+  auto walk_slot = [&](int s, ScRecord& rec) -> bool {
+    if (s >= nstart) return false;
+    const int g = t0 + s_start[s];
+    int m, b, e;
+    if (moff_shared) { const int k = module_of_shared(s_moff, mhi - mlo, g); m = mlo + k; b = s_moff[k]; e = s_moff[k + 1]; }
+    else { m = module_of(a.moff, mlo, mhi, g); b = __ldg(a.moff + m); e = __ldg(a.moff + m + 1); }
+    return sc_walk(a, m, b, e, g, cut, rec);
+  };
   ScRecord rec;
   bool kept = false;
   int kept_before = 0, nkept = 0;                      // (single round) kept clusters of the lower warps; of the tile
   for (int r = 0; r < rounds; r++) {
-    const int s = r * SC_THREADS + tid;
-    kept = s < nstart && sc_walk(a, mlo, mhi, t0 + s_start[s], cut, rec);
+    kept = walk_slot(r * SC_THREADS + tid, rec);
     const unsigned bal = __ballot_sync(0xffffffffu, kept);
     if (r > 0) __syncthreads();
     if (lane == 0) s_wb[warp] = __popc(bal);
@@ -250,8 +303,7 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
     }
   } else {                                             // rare: more starts than threads -> walk again, round by round
     for (int r = 0; r < rounds; r++) {
-      const int s = r * SC_THREADS + tid;
-      kept = s < nstart && sc_walk(a, mlo, mhi, t0 + s_start[s], cut, rec);
+      kept = walk_slot(r * SC_THREADS + tid, rec);
       const unsigned bal = __ballot_sync(0xffffffffu, kept);
       __syncthreads();
       if (lane == 0) s_wb[warp] = __popc(bal);
