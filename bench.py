@@ -333,7 +333,7 @@ def main():
         cap = n // 8
         sd = B.strips_to_device(sd_host)
         out = B.alloc_clusters(cap)
-        ws = torch.empty(max(ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, 0), 256), dtype=torch.uint8, device="cuda")
+        ws = torch.empty(max(ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, cap), 256), dtype=torch.uint8, device="cuda")
 
         def step():
             ctx.cluster_strips(sd, sp, out, ws)

@@ -46,7 +46,7 @@ enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total
 
 /* workspace query ids */
 enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3,
-       MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips */ };
+       MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips, n_seeds = capacity */ };
 
 typedef struct mkf_ctx mkf_ctx;       /* opaque: geometry, parameters, last error text */
 
@@ -154,7 +154,8 @@ int mkf_remove_duplicates(mkf_ctx*, int n_events, int n, int n_hits, const int* 
  * 16-byte aligned and bad 8-byte aligned; n_strips <= 2^31 - 4096; max_holes + max_bad <= 31.
  * Output (ordered by module, then first strip): module, first and last strip (index inside the module), charge =
  * sum adc, bary = sum adc (strip + 1/2) / sum adc in strip units. *n_clusters = number of clusters found; only the
- * first `capacity` are written (n_clusters > capacity tells the caller to retry with more room). */
+ * first `capacity` records are kept: with n_clusters > capacity the output is incomplete and the caller retries with
+ * more room. */
 typedef struct { float seed_thr, chan_thr, clus_thr; int min_charge, max_holes, max_bad; } mkf_strip_params;
 typedef struct {
   int n_modules, n_strips;
@@ -170,7 +171,7 @@ typedef struct {
   float* bary;                      /* [capacity] */
   int* n_clusters;                  /* [1] */
 } mkf_clusters;
-/* Device pointers, caller's stream, no synchronisation. ws: mkf_workspace_bytes(MKF_CALL_CLUSTER_STRIPS, 0, n_strips, 0). */
+/* Device pointers, caller's stream, no synchronisation. ws: mkf_workspace_bytes(ctx, MKF_CALL_CLUSTER_STRIPS, 0, n_strips, capacity). */
 int mkf_cluster_strips(mkf_ctx*, const mkf_strips*, const mkf_strip_params*, const mkf_clusters* out,
             void* ws, size_t ws_bytes, void* stream);
 

@@ -5,7 +5,7 @@
 namespace mkf {
 size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits);
 size_t dedup_ws_bytes(int n_hits, int n, int mpl);
-size_t strips_ws_bytes(int n_strips);
+size_t strips_ws_bytes(int n_strips, int capacity);
 }
 using namespace mkf;
 
@@ -14,7 +14,7 @@ extern "C" size_t mkf_workspace_bytes(const mkf_ctx* c, int call_id, int n_event
   switch (call_id) {
     case MKF_CALL_BUILD_HIT_INDEX: return hit_index_ws_bytes(c, n_events, n_hits);
     case MKF_CALL_REMOVE_DUPLICATES: return dedup_ws_bytes(n_hits, n_seeds, c->max_plan_len);
-    case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits);
+    case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits, n_seeds);
     default: return 0;      // fit and build keep everything in registers / shared memory
   }
 }
@@ -153,7 +153,7 @@ extern "C" int mkf_cluster_strips_host(mkf_ctx* c, const mkf_strips* s, const mk
   mkf_clusters dc = *out;
   dc.module = A.alloc<int>(cap); dc.first = A.alloc<int>(cap); dc.last = A.alloc<int>(cap);
   dc.charge = A.alloc<unsigned>(cap); dc.bary = A.alloc<float>(cap); dc.n_clusters = A.alloc<int>(1);
-  const size_t wsb = strips_ws_bytes(s->n_strips);
+  const size_t wsb = strips_ws_bytes(s->n_strips, out->capacity);
   char* ws = A.alloc<char>(wsb);
   if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_cluster_strips_host: staging");
   const int rc = mkf_cluster_strips(c, &ds, p, &dc, ws, wsb, A.st);

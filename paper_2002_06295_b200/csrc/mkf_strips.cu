@@ -1,15 +1,17 @@
 // mkf_strips.cu — strip clustering (reading R8 of DESIGN.md) in ONE pass over the strips.
 //
 // HBM-bound: 7 bytes per strip in (adc u16, noise f32, bad u8), 20 bytes per kept cluster out. One CTA takes a tile
-// of SC_TILE consecutive strips of the concatenated batch (tiles are handed out by a ticket so that a tile's
-// predecessors are always resident), each thread 8 consecutive strips with 16-byte loads:
+// of SC_TILE consecutive strips of the concatenated batch, each thread SC_SUB chunks of 8 consecutive strips with
+// 16-byte loads. Tiles do not wait for one another:
 //   1. threshold bits (pass / bad) of the tile and of a 32-strip halo to its left, module-start bits from module_off;
 //   2. a passing strip starts a cluster iff no passing strip of its module lies within the allowed gap to its left
-//      (bit tests on a 40-strip window per thread);
-//   3. the thread that owns a start walks its cluster in strip order (the sums of R8 are order-dependent in fp64)
-//      and stages the record in shared memory;
-//   4. the number of kept clusters of the tile goes through a decoupled look-back scan over the tiles, and the
-//      staged records are written compacted, in (module, first strip) order.
+//      (bit tests on a 40-strip window per chunk);
+//   3. the starts are listed in shared memory and walked one per thread, in strip order (the sums of R8 are
+//      order-dependent in fp64);
+//   4. the kept records of the tile go to staging arrays at a position taken from one global counter;
+//   5. sc_scan_tiles_kernel + sc_gather_kernel put the tiles' records in order: (module, first strip).
+// (A single-kernel version with a decoupled look-back over the tiles was 2x slower: the tiles of a wave then finish
+// together, and loads and arithmetic stop overlapping across CTAs.)
 // Nothing here is shared with oracle/.
 #include "mkf_ctx.h"
 #include <cstdint>
@@ -22,7 +24,7 @@ namespace mkf {
 constexpr int SC_THREADS = 256, SC_PER = 8, SC_CHUNKS = SC_THREADS * SC_SUB, SC_TILE = SC_CHUNKS * SC_PER, SC_HALO = 32;
 constexpr int SC_MS_WORDS = (SC_TILE + SC_HALO) / 32;
 #ifndef SC_MIN_BLOCKS
-#define SC_MIN_BLOCKS 6
+#define SC_MIN_BLOCKS 8
 #endif
 
 struct ScArgs {
@@ -30,8 +32,9 @@ struct ScArgs {
   const int* moff; const unsigned short* adc; const float* noise; const unsigned char* bad;
   float seed_thr, chan_thr, clus_thr; int min_charge, max_holes, max_bad;
   int cap; int *o_module, *o_first, *o_last; unsigned* o_charge; float* o_bary; int* n_clusters;
-  unsigned long long* tile_state;       // [n_tiles]: flag << 32 | value; flag 1 = tile aggregate, 2 = inclusive prefix
-  unsigned* ticket;
+  unsigned* total;                      // clusters found so far = next free record of the staging arrays
+  int *tile_cnt, *tile_base;            // [n_tiles]: kept clusters of the tile, where its records are staged
+  int stage_cap; int *g_module, *g_first, *g_last; unsigned* g_charge; float* g_bary;     // staging, tile by tile in arrival order
   const int* tile_mod;                  // [n_tiles]: module of the first strip of the tile's window
 };
 
@@ -144,13 +147,12 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
   __shared__ unsigned short s_start[SC_TILE];                                  // cluster starts of the tile (tile-relative), ascending
   __shared__ int s_moff[SC_MOFF];                                              // module_off[mlo + i]
   __shared__ unsigned long long s_wa[SC_THREADS / 32];
-  __shared__ int s_tile, s_prefix, s_wb[SC_THREADS / 32];
+  __shared__ int s_prefix, s_wb[SC_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-  if (tid == 0) s_tile = (int)atomicAdd(a.ticket, 1u);
   for (int i = tid; i < SC_MS_WORDS + 2; i += SC_THREADS) s_ms[i] = 0;
   __syncthreads();
-  const int tile = s_tile;
+  const int tile = blockIdx.x;
   const int t0 = tile * SC_TILE, t1 = min(t0 + SC_TILE, a.n_strips);
   const int wbase = t0 - SC_HALO;                                             // negative for tile 0
   const int mlo = __ldg(a.tile_mod + tile);
@@ -262,44 +264,17 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
     nkept += tot;
   }
 
-  // ---- decoupled look-back over the tiles (warp 0): exclusive prefix of the kept counts
-  if (warp == 0) {
-    volatile unsigned long long* st = a.tile_state;
-    unsigned excl = 0;
-    if (tile > 0) {
-      if (lane == 0) st[tile] = (1ull << 32) | (unsigned)nkept;
-      for (int top = tile - 1;; top -= 32) {
-        const int i = top - lane;
-        unsigned long long v;
-        unsigned need, inc;
-        do {
-          v = i >= 0 ? st[i] : (2ull << 32);           // before tile 0: an inclusive prefix of 0
-          const unsigned ready = __ballot_sync(0xffffffffu, (v >> 32) != 0);
-          inc = __ballot_sync(0xffffffffu, (v >> 32) == 2);
-          need = inc ? 0xffffffffu >> (32 - __ffs(inc)) : 0xffffffffu;    // lanes up to the nearest inclusive prefix
-          if ((ready & need) == need) break;
-        } while (true);
-        unsigned c = ((need >> lane) & 1u) ? (unsigned)v : 0u;
-#pragma unroll
-        for (int d = 16; d; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
-        excl += c;
-        if (inc) break;
-      }
-    }
-    if (lane == 0) {
-      st[tile] = (2ull << 32) | (unsigned long long)(excl + (unsigned)nkept);
-      s_prefix = (int)excl;
-      if (tile == a.n_tiles - 1) *a.n_clusters = (int)(excl + (unsigned)nkept);
-    }
+  // ---- room for the tile's records in the staging arrays (tiles arrive in any order; sc_gather_kernel orders them)
+  if (tid == 0) {
+    const int base = nkept ? (int)atomicAdd(a.total, (unsigned)nkept) : 0;
+    s_prefix = base; a.tile_cnt[tile] = nkept; a.tile_base[tile] = base;
   }
   __syncthreads();
-
-  // ---- write the kept clusters in (module, first strip) order
   int base = s_prefix;
   if (rounds <= 1) {
     const int off = base + kept_before;
-    if (kept && off < a.cap) {
-      a.o_module[off] = rec.module; a.o_first[off] = rec.first; a.o_last[off] = rec.last; a.o_charge[off] = rec.charge; a.o_bary[off] = rec.bary;
+    if (kept && off < a.stage_cap) {
+      a.g_module[off] = rec.module; a.g_first[off] = rec.first; a.g_last[off] = rec.last; a.g_charge[off] = rec.charge; a.g_bary[off] = rec.bary;
     }
   } else {                                             // rare: more starts than threads -> walk again, round by round
     for (int r = 0; r < rounds; r++) {
@@ -311,17 +286,65 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
       int tot;
       warp_counts(s_wb, lane, warp, kept_before, tot);
       const int off = base + kept_before + __popc(bal & ((1u << lane) - 1u));
-      if (kept && off < a.cap) {
-        a.o_module[off] = rec.module; a.o_first[off] = rec.first; a.o_last[off] = rec.last; a.o_charge[off] = rec.charge; a.o_bary[off] = rec.bary;
+      if (kept && off < a.stage_cap) {
+        a.g_module[off] = rec.module; a.g_first[off] = rec.first; a.g_last[off] = rec.last; a.g_charge[off] = rec.charge; a.g_bary[off] = rec.bary;
       }
       base += tot;
     }
   }
 }
 
-size_t strips_ws_bytes(int n_strips) {
+// exclusive scan of the kept counts over the tiles (one CTA; n_tiles is small: one tile = SC_TILE strips)
+constexpr int SC_SCAN_THREADS = 1024;
+__global__ void __launch_bounds__(SC_SCAN_THREADS) sc_scan_tiles_kernel(int n_tiles, const int* __restrict__ tile_cnt,
+                                                                        int* __restrict__ tile_out, int* __restrict__ n_clusters) {
+  __shared__ int s_w[SC_SCAN_THREADS / 32];
+  __shared__ int s_carry;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  for (int i0 = 0; i0 < n_tiles; i0 += SC_SCAN_THREADS) {
+    const int i = i0 + tid;
+    const int v = i < n_tiles ? tile_cnt[i] : 0;
+    int incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      const int w = s_w[lane];
+      int wi = w;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += t; }
+      s_w[lane] = wi - w;
+    }
+    __syncthreads();
+    const int carry = s_carry;
+    if (i < n_tiles) tile_out[i] = carry + s_w[warp] + incl - v;
+    __syncthreads();
+    if (tid == SC_SCAN_THREADS - 1) s_carry = carry + s_w[warp] + incl;
+    __syncthreads();
+  }
+  if (tid == 0) *n_clusters = s_carry;
+}
+
+// staged records -> output arrays in tile order = (module, first strip) order. One warp per tile.
+__global__ void __launch_bounds__(256) sc_gather_kernel(const ScArgs a, const int* __restrict__ tile_out) {
+  const int tile = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (tile >= a.n_tiles) return;
+  const int n = a.tile_cnt[tile], src = a.tile_base[tile], dst = tile_out[tile];
+  for (int i = lane; i < n; i += 32) {
+    if (src + i < a.stage_cap && dst + i < a.cap) {
+      a.o_module[dst + i] = a.g_module[src + i]; a.o_first[dst + i] = a.g_first[src + i]; a.o_last[dst + i] = a.g_last[src + i];
+      a.o_charge[dst + i] = a.g_charge[src + i]; a.o_bary[dst + i] = a.g_bary[src + i];
+    }
+  }
+}
+
+// workspace: total counter | tile_mod, tile_cnt, tile_base, tile_out [n_tiles] | staging 5 x capacity
+size_t strips_ws_bytes(int n_strips, int capacity) {
   const size_t n_tiles = ((size_t)n_strips + SC_TILE - 1) / SC_TILE;
-  return align256(n_tiles * sizeof(unsigned long long)) + 256 + align256(n_tiles * sizeof(int));
+  return 256 + 4 * align256(n_tiles * sizeof(int)) + 5 * align256((size_t)capacity * sizeof(int));
 }
 }  // namespace mkf
 using namespace mkf;
@@ -344,7 +367,7 @@ extern "C" int mkf_cluster_strips(mkf_ctx* c, const mkf_strips* s, const mkf_str
     return fail(c, MKF_INVALID_ARG, "mkf_cluster_strips: null pointer");
   if (((uintptr_t)s->adc & 15) || ((uintptr_t)s->noise & 15) || ((uintptr_t)s->bad & 7))
     return fail(c, MKF_INVALID_ARG, "mkf_cluster_strips: adc / noise must be 16-byte aligned, bad 8-byte aligned");
-  const size_t need = strips_ws_bytes(s->n_strips);
+  const size_t need = strips_ws_bytes(s->n_strips, out->capacity);
   if (!ws || ws_bytes < need) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_cluster_strips: workspace too small");
   ScArgs a;
   a.n_modules = s->n_modules; a.n_strips = s->n_strips; a.n_tiles = (s->n_strips + SC_TILE - 1) / SC_TILE;
@@ -353,15 +376,24 @@ extern "C" int mkf_cluster_strips(mkf_ctx* c, const mkf_strips* s, const mkf_str
   a.min_charge = p->min_charge; a.max_holes = p->max_holes; a.max_bad = p->max_bad;
   a.cap = out->capacity; a.o_module = out->module; a.o_first = out->first; a.o_last = out->last;
   a.o_charge = out->charge; a.o_bary = out->bary; a.n_clusters = out->n_clusters;
-  a.tile_state = (unsigned long long*)ws;
-  a.ticket = (unsigned*)((char*)ws + align256((size_t)a.n_tiles * sizeof(unsigned long long)));
-  int* tile_mod = (int*)((char*)a.ticket + 256);
-  a.tile_mod = tile_mod;
-  cudaError_t e = cudaMemsetAsync(ws, 0, align256((size_t)a.n_tiles * sizeof(unsigned long long)) + 256, st);
+  char* w = (char*)ws;
+  const size_t tb = align256((size_t)a.n_tiles * sizeof(int)), cb = align256((size_t)out->capacity * sizeof(int));
+  a.total = (unsigned*)w; w += 256;
+  int* tile_mod = (int*)w; w += tb; a.tile_mod = tile_mod;
+  a.tile_cnt = (int*)w; w += tb; a.tile_base = (int*)w; w += tb;
+  int* tile_out = (int*)w; w += tb;
+  a.stage_cap = out->capacity;
+  a.g_module = (int*)w; w += cb; a.g_first = (int*)w; w += cb; a.g_last = (int*)w; w += cb;
+  a.g_charge = (unsigned*)w; w += cb; a.g_bary = (float*)w;
+  cudaError_t e = cudaMemsetAsync(a.total, 0, 256, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_cluster_strips: memset");
   sc_tile_module_kernel<<<(a.n_modules + 255) / 256, 256, 0, st>>>(a.n_modules, a.n_tiles, a.moff, tile_mod);
   MKF_LAUNCHED(c, "sc_tile_module_kernel");
   sc_cluster_kernel<<<a.n_tiles, SC_THREADS, 0, st>>>(a);
   MKF_LAUNCHED(c, "sc_cluster_kernel");
+  sc_scan_tiles_kernel<<<1, SC_SCAN_THREADS, 0, st>>>(a.n_tiles, a.tile_cnt, tile_out, a.n_clusters);
+  MKF_LAUNCHED(c, "sc_scan_tiles_kernel");
+  sc_gather_kernel<<<(a.n_tiles + 7) / 8, 256, 0, st>>>(a, tile_out);
+  MKF_LAUNCHED(c, "sc_gather_kernel");
   return MKF_OK;
 }

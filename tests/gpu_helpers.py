@@ -85,7 +85,7 @@ def gpu_cluster_strips(d, sp, capacity=None):
     cap = n // 2 + 1 if capacity is None else capacity
     sd = B.strips_to_device(d)
     out = B.alloc_clusters(cap)
-    nb = ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, 0)
+    nb = ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, cap)
     ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")
     ctx.cluster_strips(sd, sp, out, ws)
     torch.cuda.synchronize()
