@@ -24,7 +24,7 @@ namespace mkf {
 constexpr int SC_THREADS = 256, SC_PER = 8, SC_CHUNKS = SC_THREADS * SC_SUB, SC_TILE = SC_CHUNKS * SC_PER, SC_HALO = 32;
 constexpr int SC_MS_WORDS = (SC_TILE + SC_HALO) / 32;
 #ifndef SC_MIN_BLOCKS
-#define SC_MIN_BLOCKS 8
+#define SC_MIN_BLOCKS 6
 #endif
 
 struct ScArgs {
@@ -47,6 +47,12 @@ __device__ __forceinline__ int module_of(const int* __restrict__ moff, int lo, i
   return lo;
 }
 
+// bit i = byte i of w is non-zero
+__device__ __forceinline__ unsigned nonzero_bytes(unsigned w) {
+  const unsigned t = (((w & 0x7f7f7f7fu) + 0x7f7f7f7fu) | w) & 0x80808080u;
+  return (t * 0x00204081u) >> 28;
+}
+
 // threshold bits of 8 consecutive strips starting at g0 (multiple of 8): bit k of pass / bad
 __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pass, unsigned& bad) {
   pass = 0; bad = 0;
@@ -57,13 +63,14 @@ __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pa
     const uint2 bv = __ldg(reinterpret_cast<const uint2*>(a.bad + g0));
     const unsigned aw[4] = {av.x, av.y, av.z, av.w};
     const float nz[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+    bad = nonzero_bytes(bv.x) | (nonzero_bytes(bv.y) << 4);
+    unsigned above = 0;
 #pragma unroll
     for (int k = 0; k < 8; k++) {
-      const unsigned adc = (aw[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-      const unsigned b = (((k < 4 ? bv.x : bv.y) >> ((k & 3) * 8)) & 0xffu) != 0;
-      bad |= b << k;
-      pass |= (unsigned)(!b && (float)adc > a.chan_thr * nz[k]) << k;
+      const unsigned adc = (k & 1) ? aw[k >> 1] >> 16 : aw[k >> 1] & 0xffffu;
+      above |= (unsigned)((float)adc > a.chan_thr * nz[k]) << k;
     }
+    pass = above & ~bad;
   } else {
     for (int k = 0; k < 8 && g0 + k < a.n_strips; k++) {
       const unsigned b = a.bad[g0 + k] != 0;
@@ -185,10 +192,22 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
 
   // ---- which of my passing strips start a cluster: window bit 32 + k = strip k of the chunk, bit 31 = the strip before ...
   unsigned starts = 0;                                 // 8 bits per chunk
+  const bool short_gap = a.max_holes == 0 && a.max_bad <= 1;     // the gap reaches at most two strips back
 #pragma unroll
   for (int u = 0; u < SC_SUB; u++) {
     if (pass[u] == 0) continue;
     const int c = u * SC_THREADS + tid;
+    if (short_gap) {
+      // 16-bit windows: bit 8 + k = strip k of the chunk, bits 0..7 = the chunk before. A passing strip i is linked
+      // to the left iff no module starts at i and (i-1 passes, or i-1 is bad, no module starts there and i-2 passes)
+      const unsigned wp = (unsigned)s_pass[c + 3] | (pass[u] << 8), wb = (unsigned)s_bad[c + 3] | (bad[u] << 8);
+      const int bit = SC_HALO - 8 + 8 * c;
+      const unsigned wm = __funnelshift_r(s_ms[bit >> 5], s_ms[(bit >> 5) + 1], bit & 31);
+      const unsigned over_bad = a.max_bad ? (wb << 1) & ~(wm << 1) & (wp << 2) : 0u;
+      const unsigned linked = ~wm & ((wp << 1) | over_bad);
+      starts |= (pass[u] & ~(linked >> 8) & 0xffu) << (8 * u);
+      continue;
+    }
     const unsigned long long wp = (unsigned long long)s_pass[c] | ((unsigned long long)s_pass[c + 1] << 8) |
         ((unsigned long long)s_pass[c + 2] << 16) | ((unsigned long long)s_pass[c + 3] << 24) | ((unsigned long long)pass[u] << 32);
     const unsigned long long wb = (unsigned long long)s_bad[c] | ((unsigned long long)s_bad[c + 1] << 8) |
