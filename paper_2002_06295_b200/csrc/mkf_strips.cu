@@ -53,6 +53,14 @@ __device__ __forceinline__ unsigned nonzero_bytes(unsigned w) {
   return (t * 0x00204081u) >> 28;
 }
 
+// (float)adc > t for a 16-bit adc, without the integer-to-float conversion: adc_magic = adc | 0x4b000000 is the bit
+// pattern of 2^23 + adc, and 2^23 + t rounded towards zero that of 2^23 + floor(t) for 0 <= t < 2^23, so the signed
+// comparison of the patterns is adc > floor(t), which for an integer adc is adc > t. t < 0 gives a smaller (or negative)
+// pattern: true; t >= 2^23, inf and NaN give a larger one: false. Exactly the float comparison in every case.
+__device__ __forceinline__ bool above_threshold(unsigned adc_magic, float t) {
+  return (int)adc_magic > __float_as_int(__fadd_rz(t, 8388608.0f));
+}
+
 // threshold bits of 8 consecutive strips starting at g0 (multiple of 8): bit k of pass / bad
 __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pass, unsigned& bad) {
   pass = 0; bad = 0;
@@ -67,8 +75,7 @@ __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pa
     unsigned above = 0;
 #pragma unroll
     for (int k = 0; k < 8; k++) {
-      const unsigned adc = (k & 1) ? aw[k >> 1] >> 16 : aw[k >> 1] & 0xffffu;
-      above |= (unsigned)((float)adc > a.chan_thr * nz[k]) << k;
+      above |= (unsigned)above_threshold(__byte_perm(aw[k >> 1], 0x4b000000u, (k & 1) ? 0x7632 : 0x7610), a.chan_thr * nz[k]) << k;
     }
     pass = above & ~bad;
   } else {
@@ -313,38 +320,33 @@ __global__ void __launch_bounds__(SC_THREADS, SC_MIN_BLOCKS) sc_cluster_kernel(c
   }
 }
 
-// exclusive scan of the kept counts over the tiles (one CTA; n_tiles is small: one tile = SC_TILE strips)
+// exclusive scan of the kept counts over the tiles (one CTA, one contiguous segment of tiles per thread; n_tiles is
+// small: one tile = SC_TILE strips)
 constexpr int SC_SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SC_SCAN_THREADS) sc_scan_tiles_kernel(int n_tiles, const int* __restrict__ tile_cnt,
                                                                         int* __restrict__ tile_out, int* __restrict__ n_clusters) {
   __shared__ int s_w[SC_SCAN_THREADS / 32];
-  __shared__ int s_carry;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) s_carry = 0;
+  const int seg = (n_tiles + SC_SCAN_THREADS - 1) / SC_SCAN_THREADS;
+  const int i0 = min(tid * seg, n_tiles), i1 = min(i0 + seg, n_tiles);
+  int sum = 0;
+  for (int i = i0; i < i1; i++) sum += tile_cnt[i];
+  int incl = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+  if (lane == 31) s_w[warp] = incl;
   __syncthreads();
-  for (int i0 = 0; i0 < n_tiles; i0 += SC_SCAN_THREADS) {
-    const int i = i0 + tid;
-    const int v = i < n_tiles ? tile_cnt[i] : 0;
-    int incl = v;
+  if (warp == 0) {
+    const int w = s_w[lane];
+    int wi = w;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
-    if (lane == 31) s_w[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-      const int w = s_w[lane];
-      int wi = w;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += t; }
-      s_w[lane] = wi - w;
-    }
-    __syncthreads();
-    const int carry = s_carry;
-    if (i < n_tiles) tile_out[i] = carry + s_w[warp] + incl - v;
-    __syncthreads();
-    if (tid == SC_SCAN_THREADS - 1) s_carry = carry + s_w[warp] + incl;
-    __syncthreads();
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += t; }
+    s_w[lane] = wi - w;
+    if (lane == 31) *n_clusters = wi;
   }
-  if (tid == 0) *n_clusters = s_carry;
+  __syncthreads();
+  int run = s_w[warp] + incl - sum;
+  for (int i = i0; i < i1; i++) { tile_out[i] = run; run += tile_cnt[i]; }
 }
 
 // staged records -> output arrays in tile order = (module, first strip) order. One warp per tile.
