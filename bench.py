@@ -31,7 +31,9 @@ NCU_TRAFFIC_BYTES_FIT_FULL = 3.591e9
 
 
 STRIP_BYTES_IN, STRIP_BYTES_PER_CLUSTER = 7, 20
-NCU_TRAFFIC_BYTES_STRIPS_FULL = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one sc_cluster_kernel launch on the full strips workload
+# (profiles/r1_strips_kernel_ncu.md)
+NCU_TRAFFIC_BYTES_STRIPS_FULL = 8.098e8
 
 
 def peaks():
@@ -151,9 +153,16 @@ class ClockSampler:
             self.samples.append((time.time(), line.strip()))
 
     def stop(self, t0, t1):
+        inside = [s for t, s in self.samples if t0 <= t <= t1]
+        in_window = bool(inside)
+        if not inside:                                   # timed region shorter than the sampling period: take the next samples
+            for _ in range(40):
+                if len(self.samples) >= 3:
+                    break
+                time.sleep(0.05)
+            inside = [s for _, s in self.samples[-3:]]
         if self.proc:
             self.proc.terminate()
-        inside = [s for t, s in self.samples if t0 <= t <= t1] or [s for _, s in self.samples[-3:]]
         mhz, mx, reasons = [], 0.0, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for s in inside:
@@ -166,7 +175,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(nme)
         return dict(sm_mhz=float(np.median(mhz)) if mhz else None, sm_max_mhz=mx or None, reasons=sorted(reasons),
-                    samples=len(mhz))
+                    samples=len(mhz), in_timed_region=in_window)
 
 
 # ---------------------------------------------------------------------------------------------------------------
