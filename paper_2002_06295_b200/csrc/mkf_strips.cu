@@ -87,14 +87,14 @@ __device__ __forceinline__ void strip_bits(const ScArgs& a, int g0, unsigned& pa
   }
 }
 
-// tile t -> the module that holds the first strip of its window, max(t * SC_TILE - SC_HALO, 0). One thread per module.
-__global__ void sc_tile_module_kernel(int n_modules, int n_tiles, const int* __restrict__ moff, int* __restrict__ tile_mod) {
+// tile t -> the module that holds the first strip of its window, max(t * tile_strips - SC_HALO, 0). One thread per module.
+__global__ void sc_tile_module_kernel(int n_modules, int n_tiles, int tile_strips, const int* __restrict__ moff, int* __restrict__ tile_mod) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= n_modules) return;
   const int b = moff[m], e = moff[m + 1];
   if (e <= b) return;
   if (b == 0) tile_mod[0] = m;
-  const int tlo = max((b + SC_HALO + SC_TILE - 1) / SC_TILE, 1), thi = min((e - 1 + SC_HALO) / SC_TILE, n_tiles - 1);
+  const int tlo = max((b + SC_HALO + tile_strips - 1) / tile_strips, 1), thi = min((e - 1 + SC_HALO) / tile_strips, n_tiles - 1);
   for (int t = tlo; t <= thi; t++) tile_mod[t] = m;
 }
 
@@ -408,7 +408,7 @@ extern "C" int mkf_cluster_strips(mkf_ctx* c, const mkf_strips* s, const mkf_str
   a.g_charge = (unsigned*)w; w += cb; a.g_bary = (float*)w;
   cudaError_t e = cudaMemsetAsync(a.total, 0, 256, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_cluster_strips: memset");
-  sc_tile_module_kernel<<<(a.n_modules + 255) / 256, 256, 0, st>>>(a.n_modules, a.n_tiles, a.moff, tile_mod);
+  sc_tile_module_kernel<<<(a.n_modules + 255) / 256, 256, 0, st>>>(a.n_modules, a.n_tiles, SC_TILE, a.moff, tile_mod);
   MKF_LAUNCHED(c, "sc_tile_module_kernel");
   sc_cluster_kernel<<<a.n_tiles, SC_THREADS, 0, st>>>(a);
   MKF_LAUNCHED(c, "sc_cluster_kernel");
