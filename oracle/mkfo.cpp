@@ -402,7 +402,16 @@ void mkfo_window(const mkfo_geometry* g, const mkfo_params* p, int layer, const 
 }
 
 // ---- C8 ---------------------------------------------------------------------------------------------
+// R9 ("Hits used in tracks reconstructed with high quality are masked to reduce the
+// combinatorics of the next iteration"): a masked hit (mask[i] != 0) is left out of the index altogether: it is in
+// no bin, it does not count for vmax, and sorted_id holds bin_off[last] < n_hits entries. mask == NULL: C8 as before.
+int mkfo_build_hit_index_masked(const mkfo_geometry* g, const mkfo_hits* h, const unsigned char* mask, unsigned* bin_off,
+                                int* sorted_id, float* vmax);
 int mkfo_build_hit_index(const mkfo_geometry* g, const mkfo_hits* h, unsigned* bin_off, int* sorted_id, float* vmax) {
+  return mkfo_build_hit_index_masked(g, h, nullptr, bin_off, sorted_id, vmax);
+}
+int mkfo_build_hit_index_masked(const mkfo_geometry* g, const mkfo_hits* h, const unsigned char* mask, unsigned* bin_off,
+                                int* sorted_id, float* vmax) {
   int nl = g->n_layers, nphi = g->n_phi_bins, neta = g->n_eta_bins, nb = nphi * neta;
   size_t nseg = (size_t)h->n_events * nl;
   std::vector<unsigned> cnt(nseg * nb + 1, 0u);
@@ -413,6 +422,7 @@ int mkfo_build_hit_index(const mkfo_geometry* g, const mkfo_hits* h, unsigned* b
     const mkfo_layer& L = g->layers[l];
     float vxy = 0.f, vzz = 0.f;
     for (int i = b; i < e; i++) {
+      if (mask && mask[i]) { key[i] = -1; continue; }
       double x = h->x[i], y = h->y[i], z = h->z[i];
       int ip = phi_bin(std::atan2(y, x), nphi);
       int ie = eta_bin(std::asinh(z / std::sqrt(x * x + y * y)), (double)L.eta_lo, (double)L.eta_hi, neta);
@@ -435,7 +445,7 @@ int mkfo_build_hit_index(const mkfo_geometry* g, const mkfo_hits* h, unsigned* b
   for (int ev = 0; ev < h->n_events; ev++) for (int l = 0; l < nl; l++) {
     size_t seg = (size_t)ev * nl + l;
     int b = h->layer_off[ev * (nl + 1) + l], e = h->layer_off[ev * (nl + 1) + l + 1];
-    for (int i = b; i < e; i++) sorted_id[cur[seg * nb + key[i]]++] = i;      // ascending id within a bin
+    for (int i = b; i < e; i++) if (key[i] >= 0) sorted_id[cur[seg * nb + key[i]]++] = i;      // ascending id within a bin
   }
   return 0;
 }
@@ -751,6 +761,27 @@ int mkfo_cluster_strips(int n_modules, const int* module_off, const unsigned sho
     }
   }
   return nout;
+}
+
+// ---- R9: which hits the next iteration no longer sees ------------------------------
+// The paper does not say what "high quality" is. Reading R9: a track is of high quality iff it survived duplicate
+// removal (keep[i] != 0; keep == NULL: every track), has nhits[i] >= min_hits, and chi2[i] <= max_chi2_ndf * ndf with
+// ndf = 2 nhits - 5 (two measured coordinates per hit, five parameters), compared in fp32 as the kernel does.
+// mask[h] is set to 1 for every hit (id >= 0) of such a track; other entries are left as they are, so that masks
+// accumulate over iterations.
+int mkfo_mask_hits(int n, int n_hits, const int* hit_ids, int max_plan_len, const int* nhits, const float* chi2,
+                   const unsigned char* keep, int min_hits, float max_chi2_ndf, unsigned char* mask) {
+  for (int i = 0; i < n; i++) {
+    if (keep && !keep[i]) continue;
+    if (nhits[i] < min_hits) continue;
+    const float ndf = (float)(2 * nhits[i] - 5);
+    if (!(chi2[i] <= max_chi2_ndf * ndf)) continue;
+    for (int s = 0; s < max_plan_len; s++) {
+      const int hid = hit_ids[(size_t)s * n + i];
+      if (hid >= 0 && hid < n_hits) mask[hid] = 1;
+    }
+  }
+  return 0;
 }
 
 }  // extern "C"

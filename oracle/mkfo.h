@@ -67,6 +67,12 @@ void mkfo_window(const mkfo_geometry* g, const mkfo_params* p, int layer, const 
 /* ---- the four calls named by BASELINE.json north_star -------------------------------------------- */
 /* C8. bin_off [n_events*n_layers*n_phi*n_eta + 1], sorted_id [n_hits], vmax [n_events*n_layers*2]. */
 int mkfo_build_hit_index(const mkfo_geometry*, const mkfo_hits*, unsigned* bin_off, int* sorted_id, float* vmax);
+/* R9: hits with mask[i] != 0 are left out (mask may be NULL) */
+int mkfo_build_hit_index_masked(const mkfo_geometry*, const mkfo_hits*, const unsigned char* mask, unsigned* bin_off,
+                                int* sorted_id, float* vmax);
+/* R9: mask[h] = 1 for the hits of high-quality tracks */
+int mkfo_mask_hits(int n, int n_hits, const int* hit_ids, int max_plan_len, const int* nhits, const float* chi2,
+                   const unsigned char* keep, int min_hits, float max_chi2_ndf, unsigned char* mask);
 /* C7. seeds par[6][n] cov[21][n] (fp32), q[n]; plan[n]; track_hits[max_plan_len][n] (global hit id or <0).
  * Outputs (double) par_out[6][n], cov_out[21][n], chi2[n], nfit[n], status[n]. */
 int mkfo_fit(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,

@@ -112,16 +112,20 @@ class Oracle:
         s._keep = keep
         return s
 
-    def build_hit_index(self, h):
+    def build_hit_index(self, h, mask=None):
+        """mask (uint8[n_hits], reading R9): hits with mask != 0 are left out; sorted_id is then cut to the hits placed."""
         hs = self.hits(h)
         nseg = hs.n_events * self.n_layers
         bin_off = np.zeros(nseg * self.nbins + 1, np.uint32)
         sorted_id = np.zeros(hs.n_hits, np.int32)
         vmax = np.zeros(nseg * 2, np.float32)
-        rc = self.L.mkfo_build_hit_index(C.byref(self.g), C.byref(hs), _p(bin_off, C.c_uint), _p(sorted_id, C.c_int),
-                                         _p(vmax, C.c_float))
+        if mask is not None:
+            mask = np.ascontiguousarray(mask, np.uint8)
+            assert mask.shape[0] == hs.n_hits
+        rc = self.L.mkfo_build_hit_index_masked(C.byref(self.g), C.byref(hs), _p(mask, C.c_ubyte) if mask is not None else None,
+                                                _p(bin_off, C.c_uint), _p(sorted_id, C.c_int), _p(vmax, C.c_float))
         assert rc == 0
-        return dict(bin_off=bin_off, sorted_id=sorted_id, vmax=vmax)
+        return dict(bin_off=bin_off, sorted_id=sorted_id[:int(bin_off[-1])], vmax=vmax)
 
     def fit(self, h, par, cov, q, plan, track_hits):
         hs = self.hits(h)
@@ -278,3 +282,18 @@ def cluster_strips(module_off, adc, noise, bad, seed_thr=3.0, chan_thr=2.0, clus
                               C.c_float(seed_thr), C.c_float(chan_thr), C.c_float(clus_thr), int(min_charge), int(max_holes),
                               int(max_bad), _p(om, C.c_int), _p(of, C.c_int), _p(ol, C.c_int), _p(oc, C.c_uint), _p(ob, C.c_float))
     return dict(module=om[:k].copy(), first=of[:k].copy(), last=ol[:k].copy(), charge=oc[:k].copy(), bary=ob[:k].copy())
+
+
+def mask_hits(n_hits, hit_ids, nhits, chi2, keep=None, min_hits=8, max_chi2_ndf=5.0, mask=None):
+    """Reading R9: mask[h] = 1 for the hits of high-quality tracks. Returns the mask."""
+    L = lib()
+    hi = np.ascontiguousarray(hit_ids, np.int32)
+    n = hi.shape[1]
+    nh, c2 = np.ascontiguousarray(nhits, np.int32), np.ascontiguousarray(chi2, np.float32)
+    mask = np.zeros(n_hits, np.uint8) if mask is None else np.ascontiguousarray(mask, np.uint8).copy()
+    if keep is not None:
+        keep = np.ascontiguousarray(keep, np.uint8)
+    rc = L.mkfo_mask_hits(n, int(n_hits), _p(hi, C.c_int), hi.shape[0], _p(nh, C.c_int), _p(c2, C.c_float),
+                          _p(keep, C.c_ubyte) if keep is not None else None, int(min_hits), C.c_float(max_chi2_ndf), _p(mask, C.c_ubyte))
+    assert rc == 0
+    return mask
