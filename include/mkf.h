@@ -142,6 +142,20 @@ int mkf_remove_duplicates(mkf_ctx*, int n_events, int n, int n_hits, const int* 
             int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept,
             void* ws, size_t ws_bytes, void* stream);
 
+/* ---- SURVEY.md f4 / reading R9 of DESIGN.md: hit masking between iterations ("Hits used in tracks
+ * reconstructed with high quality are masked to reduce the combinatorics of the next iteration") ------------------
+ * mkf_mask_hits: mask[h] = 1 for every hit (id >= 0) of a high-quality track; other entries are left as they are, so
+ * masks accumulate over iterations (the caller zeroes the mask before the first). High quality (R9; the paper gives no
+ * definition): keep[i] != 0 (keep == NULL: every track), nhits[i] >= min_hits and chi2[i] <= max_chi2_ndf * (2 nhits[i] - 5),
+ * compared in fp32. hit_ids[max_plan_len][n], nhits, chi2, keep as written by mkf_build_tracks / mkf_remove_duplicates.
+ * mkf_build_hit_index_masked: mkf_build_hit_index without the hits with mask[i] != 0: they are in no bin and do not
+ * count for vmax; sorted_id / packed hold bin_off[last] <= n_hits entries. mask == NULL: the plain index. Same workspace.
+ * All pointers device; caller's stream; no synchronisation. */
+int mkf_mask_hits(mkf_ctx*, int n, int n_hits, const int* hit_ids, int max_plan_len, const int* nhits, const float* chi2,
+            const unsigned char* keep, int min_hits, float max_chi2_ndf, unsigned char* mask, void* stream);
+int mkf_build_hit_index_masked(mkf_ctx*, const mkf_hits*, const unsigned char* mask, mkf_hit_index* out,
+            void* ws, size_t ws_bytes, void* stream);
+
 /* ---- SURVEY.md f3 / reading R8 of DESIGN.md: strip clustering ------------------------------
  * "seed strips with ADC values greater than 3 times the expected noise are identified; second, clusters are formed
  * adding to the seed all strips with ADC values above twice the expected noise that are either consecutive or have

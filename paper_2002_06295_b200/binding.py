@@ -18,7 +18,7 @@ CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
            "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host",
-           "mkf_cluster_strips", "mkf_cluster_strips_host"]
+           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked"]
 
 
 class Layer(C.Structure):
@@ -90,6 +90,8 @@ def lib():
         L.mkf_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(Geometry), C.POINTER(Params)]
         vp, sz, i = C.c_void_p, C.c_size_t, C.c_int
         L.mkf_build_hit_index.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), vp, sz, vp]
+        L.mkf_build_hit_index_masked.argtypes = [vp, C.POINTER(Hits), vp, C.POINTER(HitIndex), vp, sz, vp]
+        L.mkf_mask_hits.argtypes = [vp, i, i, vp, i, vp, vp, vp, i, C.c_float, vp, vp]
         L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
         L.mkf_fit_backward.argtypes = L.mkf_fit.argtypes
         L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
@@ -180,17 +182,31 @@ class Context:
                     ptr(h["z"], f32), ptr(h["V"], f32))
 
     # ---- the four calls -----------------------------------------------------------------------------------
-    def build_hit_index(self, hits, out, ws):
-        """hits: dict of CUDA tensors (layer_off int32, x,y,z float32 [n], V float32 [6,n]); out: dict(bin_off int32
+    def build_hit_index(self, hits, out, ws, mask=None):
+        """mask (uint8 CUDA tensor [n_hits] or None): mkf_build_hit_index_masked (reading R9).
+        hits: dict of CUDA tensors (layer_off int32, x,y,z float32 [n], V float32 [6,n]); out: dict(bin_off int32
         [n_events*n_layers*n_bins+1] (unsigned offsets), sorted_id int32 [n], vmax float32 [n_events*n_layers*2],
         packed float32 [n*12] or None); ws: uint8 CUDA tensor."""
         hs = self.hits_struct(hits, _dev)
         packed = out.get("packed")
         idx = HitIndex(_dev(out["bin_off"], torch.int32), _dev(out["sorted_id"], torch.int32), _dev(out["vmax"], torch.float32),
                        _dev(packed, torch.float32) if packed is not None else None)
-        rc = self.L.mkf_build_hit_index(self.h, C.byref(hs), C.byref(idx), ws.data_ptr() if ws is not None else None,
-                                        ws.numel() if ws is not None else 0, _stream())
+        wsp, wsn = (ws.data_ptr(), ws.numel()) if ws is not None else (None, 0)
+        if mask is not None:
+            rc = self.L.mkf_build_hit_index_masked(self.h, C.byref(hs), _dev(mask, torch.uint8), C.byref(idx), wsp, wsn, _stream())
+        else:
+            rc = self.L.mkf_build_hit_index(self.h, C.byref(hs), C.byref(idx), wsp, wsn, _stream())
         self._check(rc, "mkf_build_hit_index")
+
+    build_hit_index_masked = build_hit_index
+
+    def mask_hits(self, hit_ids, nhits, chi2, keep, min_hits, max_chi2_ndf, mask):
+        """mkf_mask_hits (reading R9): sets mask[h] = 1 for the hits of high-quality tracks; keep may be None."""
+        rc = self.L.mkf_mask_hits(self.h, int(hit_ids.shape[1]), int(mask.shape[0]), _dev(hit_ids, torch.int32), int(hit_ids.shape[0]),
+                                  _dev(nhits, torch.int32), _dev(chi2, torch.float32),
+                                  _dev(keep, torch.uint8) if keep is not None else None, int(min_hits), float(max_chi2_ndf),
+                                  _dev(mask, torch.uint8), _stream())
+        self._check(rc, "mkf_mask_hits")
 
     def fit_backward(self, hits, seeds, plan, track_hits, out, chi2, nfit, status):
         """Outside-in fit (mkf_fit_backward); seeds sit on the layer of each track's last hit."""

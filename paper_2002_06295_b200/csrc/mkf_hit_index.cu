@@ -24,6 +24,8 @@ struct HiArgs {
   int* key;            // [n_hits] bin inside the segment
   unsigned* cnt;       // [n_bins_total] counts, later the scatter cursors
   unsigned* bin_off; int* sorted_id; float* vmax; float4* packed;
+  const unsigned char* mask;     // R9: hits left out of the index (NULL: none)
+  size_t n_bins;
 };
 
 __device__ __forceinline__ int phi_bin_d(double phi, int nphi) {
@@ -49,6 +51,7 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_key_count(const __grid_constant__
   const size_t bin0 = (size_t)seg * (size_t)(a.n_phi * a.n_eta);
   float vxy = 0.f, vzz = 0.f;
   for (int i = b + threadIdx.x; i < e; i += HI_BLOCK) {
+    if (a.mask && a.mask[i]) { a.key[i] = -1; continue; }
     const double x = (double)a.hits.x[i], y = (double)a.hits.y[i], z = (double)a.hits.z[i];
     const int ip = phi_bin_d(atan2(y, x), a.n_phi);
     const int ie = eta_bin_d(asinh(z / sqrt(x * x + y * y)), elo, ehi, a.n_eta);
@@ -82,7 +85,9 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_place(const __grid_constant__ HiA
   const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
   const size_t bin0 = (size_t)seg * (size_t)(a.n_phi * a.n_eta);
   for (int i = b + threadIdx.x; i < e; i += HI_BLOCK) {
-    const unsigned pos = atomicAdd(&a.cnt[bin0 + a.key[i]], 1u);
+    const int key = a.key[i];
+    if (key < 0) continue;
+    const unsigned pos = atomicAdd(&a.cnt[bin0 + key], 1u);
     a.sorted_id[pos] = i;
   }
 }
@@ -119,7 +124,7 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_sort_bins(const unsigned* __restr
 
 __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiArgs a) {
   const int t = blockIdx.x * HI_BLOCK + threadIdx.x;
-  if (t >= a.hits.n_hits) return;
+  if (t >= a.hits.n_hits || (unsigned)t >= a.bin_off[a.n_bins]) return;       // masked hits are not in sorted_id
   const int id = a.sorted_id[t];
   const size_t nh = (size_t)a.hits.n_hits;
   const float* V = a.hits.V;
@@ -141,6 +146,11 @@ size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits) {
 }  // namespace mkf
 
 extern "C" int mkf_build_hit_index(mkf_ctx* c, const mkf_hits* h, mkf_hit_index* out, void* ws, size_t ws_bytes, void* stream) {
+  return mkf_build_hit_index_masked(c, h, nullptr, out, ws, ws_bytes, stream);
+}
+
+extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const unsigned char* mask, mkf_hit_index* out, void* ws,
+                                          size_t ws_bytes, void* stream) {
   if (!c) return MKF_INVALID_ARG;
   if (!h || !out || !out->bin_off || !out->sorted_id || !out->vmax || !h->layer_off)
     return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index: null argument");
@@ -159,11 +169,12 @@ extern "C" int mkf_build_hit_index(mkf_ctx* c, const mkf_hits* h, mkf_hit_index*
   a.cnt = (unsigned*)w; w += align256(nbins * 4);
   unsigned* partial = (unsigned*)w;
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
+  a.mask = mask; a.n_bins = nbins;
   cudaError_t e = cudaMemsetAsync(a.cnt, 0, nbins * 4, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_hit_index: memset");
   hi_key_count<<<nseg, HI_BLOCK, 0, st>>>(c->g, a);
   MKF_LAUNCHED(c, "hi_key_count");
-  { const int rc = exclusive_scan_u32(c, a.cnt, nbins, partial, a.bin_off, (unsigned)h->n_hits, st); if (rc) return rc; }
+  { const int rc = exclusive_scan_u32(c, a.cnt, nbins, partial, a.bin_off, mask ? SCAN_TOTAL_UNKNOWN : (unsigned)h->n_hits, st); if (rc) return rc; }
   if (h->n_hits > 0) {
     hi_place<<<nseg, HI_BLOCK, 0, st>>>(a);
     MKF_LAUNCHED(c, "hi_place");
@@ -174,5 +185,36 @@ extern "C" int mkf_build_hit_index(mkf_ctx* c, const mkf_hits* h, mkf_hit_index*
       MKF_LAUNCHED(c, "hi_pack");
     }
   }
+  return MKF_OK;
+}
+
+// ---- R9: the hits of high-quality tracks, masked for the next iteration ------------
+namespace {
+__global__ void __launch_bounds__(256) mh_mask_kernel(int n, int n_hits, const int* __restrict__ hit_ids, int mpl,
+                                                      const int* __restrict__ nhits, const float* __restrict__ chi2,
+                                                      const unsigned char* __restrict__ keep, int min_hits, float max_chi2_ndf,
+                                                      unsigned char* mask) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (keep && !keep[i]) return;
+  const int nh = nhits[i];
+  if (nh < min_hits) return;
+  if (!(chi2[i] <= __fmul_rn(max_chi2_ndf, (float)(2 * nh - 5)))) return;
+  for (int s = 0; s < mpl; s++) {
+    const int hid = hit_ids[(size_t)s * n + i];              // coalesced: plane-major
+    if (hid >= 0 && hid < n_hits) mask[hid] = 1;             // every writer writes 1
+  }
+}
+}  // namespace
+
+extern "C" int mkf_mask_hits(mkf_ctx* c, int n, int n_hits, const int* hit_ids, int max_plan_len, const int* nhits, const float* chi2,
+                             const unsigned char* keep, int min_hits, float max_chi2_ndf, unsigned char* mask, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (n < 0 || n_hits < 0 || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_mask_hits: bad sizes");
+  if (n == 0) return MKF_OK;
+  if (!hit_ids || !nhits || !chi2 || (n_hits > 0 && !mask)) return fail(c, MKF_INVALID_ARG, "mkf_mask_hits: null argument");
+  mh_mask_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, n_hits, hit_ids, max_plan_len, nhits, chi2, keep, min_hits,
+                                                                    max_chi2_ndf, mask);
+  MKF_LAUNCHED(c, "mh_mask_kernel");
   return MKF_OK;
 }

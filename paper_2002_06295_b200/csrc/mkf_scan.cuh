@@ -7,6 +7,7 @@
 namespace mkf {
 
 constexpr int SCAN_BLOCK = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_BLOCK * SCAN_ITEMS;
+constexpr unsigned SCAN_TOTAL_UNKNOWN = 0xffffffffu;    // as `total` of exclusive_scan_u32: out[n] = the sum of the counts
 
 static __device__ __forceinline__ unsigned block_exclusive_scan(unsigned v, unsigned* total) {   // SCAN_BLOCK threads
   __shared__ unsigned s_w[SCAN_BLOCK / 32];
@@ -69,8 +70,9 @@ static __global__ void __launch_bounds__(SCAN_BLOCK) scan_down(unsigned* cnt, si
   for (int k = 0; k < SCAN_ITEMS; k++) {
     if (base + k < n) { bin_off[base + k] = run; cnt[base + k] = run; }
     run += v[k];
+    if (total_hits == SCAN_TOTAL_UNKNOWN && base + k == n - 1) bin_off[n] = run;       // the sum itself
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) bin_off[n] = total_hits;
+  if (total_hits != SCAN_TOTAL_UNKNOWN && blockIdx.x == 0 && threadIdx.x == 0) bin_off[n] = total_hits;
 }
 
 inline size_t scan_partial_bytes(size_t n) { return align256(((n + SCAN_TILE - 1) / SCAN_TILE + 1) * 4); }

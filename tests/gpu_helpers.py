@@ -94,3 +94,43 @@ def gpu_cluster_strips(d, sp, capacity=None):
     res["charge"] = res["charge"].view(np.uint32)
     res["n_clusters"] = k
     return res
+
+
+def gpu_two_iterations(ev, prm, min_hits, max_chi2_ndf):
+    """Iteration 1: index + build + duplicate removal on all seeds; mkf_mask_hits; iteration 2: masked index + build of the
+    same seeds. Returns the numpy results of both iterations, the mask and the masked index."""
+    s = ev["seeds"]
+    ctx = B.Context(ev["geom"], prm)
+    hits = B.hits_to_device(ev["hits"])
+    nh, nev = hits["x"].shape[0], hits["n_events"]
+    idx, ws = B.alloc_hit_index(ctx, nev, nh)
+    ctx.build_hit_index(hits, idx, ws)
+    sd = B.to_device(dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"]),
+                     ["par", "cov", "q", "plan", "event", "hits"])
+    n = s["par"].shape[1]
+
+    def build():
+        out = B.alloc_build_out(n, ctx.max_plan_len)
+        ctx.build_tracks(hits, idx, sd, sd["event"], sd["hits"], sd["plan"], out, out["chi2"], out["score"], out["nhits"],
+                         out["nmiss"], out["hit_ids"], out["status"])
+        return out
+    o1 = build()
+    counts = np.bincount(s["event"], minlength=nev)
+    toff = torch.from_numpy(np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)).cuda()
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+    nk = torch.empty(nev, dtype=torch.int32, device="cuda")
+    ws2 = torch.empty(max(ctx.workspace_bytes(B.CALL_REMOVE_DUPLICATES, nev, nh, n), 256), dtype=torch.uint8, device="cuda")
+    ctx.remove_duplicates(nh, toff, o1["hit_ids"], o1["nhits"], o1["score"], keep, nk, ws2)
+    mask = torch.zeros(nh, dtype=torch.uint8, device="cuda")
+    ctx.mask_hits(o1["hit_ids"], o1["nhits"], o1["chi2"], keep, min_hits, max_chi2_ndf, mask)
+    r1 = {k: v.cpu().numpy() for k, v in o1.items()}
+    r1["keep"] = keep.cpu().numpy()
+    ctx.build_hit_index(hits, idx, ws, mask=mask)
+    torch.cuda.synchronize()
+    im = dict(bin_off=idx["bin_off"].cpu().numpy().view(np.uint32), vmax=idx["vmax"].cpu().numpy())
+    im["sorted_id"] = idx["sorted_id"].cpu().numpy()[:int(im["bin_off"][-1])]
+    o2 = build()
+    torch.cuda.synchronize()
+    r2 = {k: v.cpu().numpy() for k, v in o2.items()}
+    ctx.close()
+    return r1, mask.cpu().numpy(), im, r2
