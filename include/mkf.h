@@ -165,7 +165,8 @@ int mkf_build_hit_index_masked(mkf_ctx*, const mkf_hits*, const unsigned char* m
  * Input: the strips of all modules of all events of the batch, concatenated; module m owns strips
  * module_off[m]..module_off[m+1]-1 (ascending; empty modules allowed). adc: pedestal-subtracted counts; noise: the
  * expected noise of each strip; bad: non-zero = bad strip (never counted, may be bridged). adc and noise must be
- * 16-byte aligned and bad 8-byte aligned; n_strips <= 2^31 - 4096; max_holes + max_bad <= 31.
+ * 16-byte aligned and bad 8-byte aligned; module_off[0] = 0 and module_off[n_modules] = n_strips (not checked: the
+ * offsets live on the device); n_strips <= 2^31 - 16384; max_holes + max_bad <= 31 (MKF_UNSUPPORTED otherwise).
  * Output (ordered by module, then first strip): module, first and last strip (index inside the module), charge =
  * sum adc, bary = sum adc (strip + 1/2) / sum adc in strip units. *n_clusters = number of clusters found; only the
  * first `capacity` records are kept: with n_clusters > capacity the output is incomplete and the caller retries with

@@ -390,6 +390,7 @@ extern "C" int mkf_cluster_strips(mkf_ctx* c, const mkf_strips* s, const mkf_str
     return fail(c, MKF_INVALID_ARG, "mkf_cluster_strips: adc / noise must be 16-byte aligned, bad 8-byte aligned");
   const size_t need = strips_ws_bytes(s->n_strips, out->capacity);
   if (!ws || ws_bytes < need) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_cluster_strips: workspace too small");
+  if ((uintptr_t)ws & 15) return fail(c, MKF_INVALID_ARG, "mkf_cluster_strips: workspace must be 16-byte aligned");
   ScArgs a;
   a.n_modules = s->n_modules; a.n_strips = s->n_strips; a.n_tiles = (s->n_strips + SC_TILE - 1) / SC_TILE;
   a.moff = s->module_off; a.adc = s->adc; a.noise = s->noise; a.bad = s->bad;

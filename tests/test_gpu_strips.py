@@ -76,3 +76,27 @@ def test_strips_empty_and_host_entry():
         assert np.array_equal(got[key], ref[key]), key
     assert np.array_equal(got["bary"].view(np.uint32), ref["bary"].view(np.uint32))
     assert got["h2d_bytes"] == 7 * len(d["adc"]) + 4 * len(d["module_off"]) and got["d2h_bytes"] == 4 + 20 * len(ref["module"])
+
+
+def test_strips_argument_errors():
+    import torch
+    from gpu_helpers import strip_context
+    from paper_2002_06295_b200 import binding as B
+    ctx = strip_context()
+    d = datagen.make_strips(15, 20)
+    sd = B.strips_to_device(d)
+    n = len(d["adc"])
+    out = B.alloc_clusters(n // 2 + 1)
+    ws = torch.empty(ctx.workspace_bytes(B.MKF_CALL_CLUSTER_STRIPS, 0, n, n // 2 + 1), dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.MkfError):                   # the gap must fit the 32-strip halo
+        ctx.cluster_strips(sd, datagen.default_strip_params(max_holes=20, max_bad=20), out, ws)
+    with pytest.raises(B.MkfError):                   # workspace too small
+        ctx.cluster_strips(sd, datagen.default_strip_params(), out, ws[:64])
+    with pytest.raises(B.MkfError):                   # adc not 16-byte aligned
+        bad = dict(sd, adc=sd["adc"][1:], noise=sd["noise"][1:], bad=sd["bad"][1:],
+                   module_off=torch.tensor([0, n - 1], dtype=torch.int32, device="cuda"))
+        ctx.cluster_strips(bad, datagen.default_strip_params(), out, ws)
+    ctx.cluster_strips(sd, datagen.default_strip_params(), out, ws)      # and the context still works afterwards
+    torch.cuda.synchronize()
+    ref = mkfo.cluster_strips(d["module_off"], d["adc"], d["noise"], d["bad"], **datagen.default_strip_params())
+    assert int(out["n_clusters"].item()) == len(ref["module"])
