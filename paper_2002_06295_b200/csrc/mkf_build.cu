@@ -17,7 +17,10 @@ using namespace mkf;
 namespace {
 
 constexpr int G = 8;                 // lanes per seed == MAX_CAND
-constexpr int BUILD_BLOCK = 128;     // 16 seeds per CTA
+#ifndef MKF_BUILD_BLOCK
+#define MKF_BUILD_BLOCK 64
+#endif
+constexpr int BUILD_BLOCK = MKF_BUILD_BLOCK;     // 8 seeds per CTA (64 threads: 2193 events/s on configs[4]; 128: 2108, 32: 2178)
 constexpr int HIT_NONE = 0x7fffffff; // "hit id" of miss / pass-through children in the order U14
 static_assert(G == MAX_CAND, "one lane per candidate slot");
 
@@ -98,7 +101,7 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
   } while (0)
 
 #ifndef MKF_BUILD_MIN_BLOCKS
-#define MKF_BUILD_MIN_BLOCKS 8
+#define MKF_BUILD_MIN_BLOCKS 16
 #endif
 __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
                                                                 const __grid_constant__ ParamsDev p,
