@@ -50,6 +50,13 @@ __device__ __forceinline__ void load_packed(Hit& H, int& id, const float4 a, con
   H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = c.x; H.v[5] = c.y;
 }
 
+// asinh to ~1e-6 absolute for |x| up to e^4 (one lg2.approx, one rsqrt-based sqrt): the eta edges of the window carry
+// a margin of 2e-5 + 1e-5 |eta| below
+__device__ __forceinline__ float window_asinh(float x) {
+  const float ax = fabsf(x);
+  return copysignf(fast_log(ax + good_sqrt(fmaf(ax, ax, 1.f))), x);
+}
+
 // U11: window of bins that contains every hit with chi2 < cut.
 __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, float cut, const KState& S,
                                        float tt, float zz_or_yy, float vxy, float vzz, int& e0, int& e1, int& p0, int& np) {
@@ -63,13 +70,13 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
     const float a2 = sqrtf(cut * vxy) / R + 2e-6f;
     dphi = a2 < 2.f ? acosf(1.f - a2) : PI_F;
     if (a1 < 1.f && dphi <= 0.5f * PI_F) dphi = fminf(dphi, asinf(a1));
-    eta_a = asinhf((z - dz) / R); eta_b = asinhf((z + dz) / R);
+    eta_a = window_asinh((z - dz) / R); eta_b = window_asinh((z + dz) / R);
   } else {
     const float r = sqrtf(fmaf(x, x, y * y));
     const float rw = sqrtf(cut * (fmaxf(tt + zz_or_yy, 0.f) + vxy)) * (1.f + 1e-5f);
     dphi = rw < r ? asinf(rw / r) : PI_F;
     const float rlo = fmaxf(r - rw, 1e-3f), rhi = r + rw;
-    const float ea = asinhf(L.pos / rlo), eb = asinhf(L.pos / rhi);
+    const float ea = window_asinh(L.pos / rlo), eb = window_asinh(L.pos / rhi);
     eta_a = fminf(ea, eb); eta_b = fmaxf(ea, eb);
   }
   // The (dphi, eta) box is already a proven superset of {chi2 < cut} (U11); it only needs margins for the fp32
