@@ -82,7 +82,7 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
   // The (dphi, eta) box is already a proven superset of {chi2 < cut} (U11); it only needs margins for the fp32
   // evaluation of its edges against the fp64 bin keys of the hits (C8), not whole extra bins.
   dphi = dphi * (1.f + 1e-4f) + 2e-5f;
-  const float esc = (float)g.n_eta / (L.eta_hi - L.eta_lo);
+  const float esc = fast_div((float)g.n_eta, L.eta_hi - L.eta_lo);
   const float em = 2e-5f + 1e-5f * fmaxf(fabsf(eta_a), fabsf(eta_b));
   int ia = (int)floorf((eta_a - em - L.eta_lo) * esc), ib = (int)floorf((eta_b + em - L.eta_lo) * esc);
   e0 = min(max(ia, 0), g.n_eta - 1); e1 = min(max(ib, 0), g.n_eta - 1);
@@ -92,7 +92,7 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
   const int b = (int)floorf((php + dphi + PI_F) * ibw);
   const int cnt = b - a + 1;
   if (cnt >= g.n_phi) { p0 = 0; np = g.n_phi; return; }
-  p0 = ((a % g.n_phi) + g.n_phi) % g.n_phi; np = cnt;
+  p0 = a < 0 ? a + g.n_phi : (a >= g.n_phi ? a - g.n_phi : a); np = cnt;          // dphi < pi: a in (-n_phi, 2 n_phi)
 }
 
 #define SHFL_STATE(S, src, gm)                                           \
