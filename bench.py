@@ -52,7 +52,7 @@ def peaks():
 # ---------------------------------------------------------------------------------------------------------------
 def make_fit_workload(seed, scale):
     """configs[1]: generated as chunks of 1 M helices (bounded host memory), hits concatenated, ids offset."""
-    from paper_2002_06295_b200 import datagen
+    from workloads import datagen
     total = max(1, int(round(4000000 * scale)))
     chunk = 1000000
     parts, nh0 = [], 0
@@ -78,7 +78,7 @@ def make_fit_workload(seed, scale):
 
 
 def make_build_workload(which, seed, scale):
-    from paper_2002_06295_b200 import datagen
+    from workloads import datagen
     ev, prm = datagen.config(which, scale=scale, seed=seed)
     return ev, prm
 
@@ -92,7 +92,7 @@ STRIP_EVENTS, STRIP_MODULES = 16, 15000
 def make_strip_workload(seed, scale):
     """STRIP_EVENTS x scale events of STRIP_MODULES modules (about the module count of a strip tracker), generated one
     event at a time (seeds 64 seed + k) and concatenated: the batch is one flat module list."""
-    from paper_2002_06295_b200 import datagen
+    from workloads import datagen
     n_ev = max(1, int(round(STRIP_EVENTS * scale))) if scale >= 1.0 / STRIP_EVENTS else 1
     n_mod = STRIP_MODULES if scale >= 1.0 / STRIP_EVENTS else max(8, int(round(STRIP_MODULES * STRIP_EVENTS * scale)))
     parts = [datagen.make_strips(64 * seed + k, n_mod) for k in range(n_ev)]
@@ -334,7 +334,7 @@ def main():
             r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"])
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
     elif is_strips:
-        from paper_2002_06295_b200 import datagen
+        from workloads import datagen
         ev_g, prm_g = datagen.config(0, scale=0.001)              # clustering uses no geometry; a context needs one
         ctx = B.Context(ev_g["geom"], prm_g)
         sd_host, sp = make_strip_workload(rank_seed(a.seed, rank), a.scale)
@@ -457,7 +457,7 @@ def main():
             rate, dt, cores, st, r = oracle_fit_rate(geom, prm, hits, seeds, n_s, backward=backward)
             cpu = dict(value=rate, unit=unit, cores=cores, kind="oracle", sample="first %d helices of the workload (%d layer-steps, %.1f s)" % (n_s, st, dt))
             # parity of the timed launch configuration on that same sample (the oracle results are already here)
-            from paper_2002_06295_b200 import parity
+            from workloads import parity
             g = {k: out[k][..., :n_s].cpu().numpy() for k in ("par", "cov", "chi2", "nfit", "status")}
             ok = r["nfit"] > 0
             where = parity.first_layer_of_backward_fit if backward else parity.last_layer_of_fit

@@ -15,5 +15,5 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def small_fit_event():
     """configs[0] at 1/5 size (2000 helices, 10 barrel layers)."""
-    from paper_2002_06295_b200 import datagen
+    from workloads import datagen
     return datagen.config(0, scale=0.2, seed=0)

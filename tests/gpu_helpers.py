@@ -72,7 +72,7 @@ def strip_context():
     """Clustering uses no geometry; any context will do."""
     global _strip_ctx
     if _strip_ctx is None:
-        from paper_2002_06295_b200 import datagen
+        from workloads import datagen
         ev, prm = datagen.config(0, scale=0.01)
         _strip_ctx = B.Context(ev["geom"], prm)
     return _strip_ctx

@@ -25,7 +25,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_create_validates_arguments_without_gpu():
-    from paper_2002_06295_b200 import datagen
+    from workloads import datagen
     g = datagen.geometry_barrel(4, 4.0, 16.0, 50.0, 0.02)
     ctx = binding.Context(g, datagen.default_params())
     assert ctx.max_plan_len == 4

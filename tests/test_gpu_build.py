@@ -4,8 +4,8 @@ import numpy as np
 import pytest
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
-from paper_2002_06295_b200 import parity
+from workloads import datagen
+from workloads import parity
 
 pytestmark = pytest.mark.gpu
 
@@ -89,7 +89,7 @@ def compare_build(ev, prm, r, h, min_same=0.999):
     layc = plan_layers[plan_off[ev["seeds"]["plan"].astype(int)] + lastc]
     kindc = np.array([l["kind"] for l in geom["layers"]])[layc]
     ce = parity.cov_errors(h["cov"], r["cov"], r["par"], kindc)[ok]
-    assert np.quantile(ce, 0.999) <= parity.TOL_COV and ce.max() <= 3 * parity.TOL_COV, (np.quantile(ce, 0.999), ce.max())
+    assert ce.max() <= parity.TOL_COV, ce.max()                              # north_star: 1e-3 on every element, every track
     return frac
 
 
@@ -279,3 +279,64 @@ def test_degenerate_inputs():
     with pytest.raises(B.MkfError):
         ctx.remove_duplicates(n0, toff, out["hit_ids"], out["nhits"], out["score"], keep, nk, ws2[:64])
     ctx.close()
+
+
+@pytest.mark.parametrize("cap", [1, 2])
+def test_u14_ties_lower_hit_id_then_lower_parent_rank(cap):
+    """Keys 3 and 4 of the total order U14 on the hand-placed twin-hit event (tests/hand_events.py): the expected lists
+    are written by hand; the oracle is pinned to the same lists in tests/test_oracle_build.py."""
+    from gpu_helpers import gpu_build
+    from hand_events import tie_event, TIE_EXPECTED
+    ev, prm = tie_event()
+    prm = dict(prm, max_cand=cap)
+    for packed in (True, False):
+        h = gpu_build(ev, prm, packed=packed)
+        assert list(h["hit_ids"][:, 0]) == TIE_EXPECTED[cap]
+        assert h["nhits"][0] == 5 and h["nmiss"][0] == 0 and h["status"][0] == 0
+    r, _ = run_build(ev, prm)
+    assert np.array_equal(h["hit_ids"], r["hit_ids"]) and abs(h["chi2"][0] - r["chi2"][0]) <= 1e-3 * max(r["chi2"][0], 1.0)
+
+
+def test_u14_tie_on_the_last_layer():
+    from gpu_helpers import gpu_build
+    from hand_events import tie_event
+    ev, prm = tie_event()
+    hh = ev["hits"]
+    g4 = dict(ev["geom"], layers=ev["geom"]["layers"][:4], plan_off=np.array([0, 4], np.int32), plan_layers=np.arange(4, dtype=np.int32))
+    sub = dict(n_events=1, x=hh["x"][:5].copy(), y=hh["y"][:5].copy(), z=hh["z"][:5].copy(), V=np.ascontiguousarray(hh["V"][:, :5]),
+               layer_off=np.array([0, 1, 2, 3, 5], np.int32))
+    h = gpu_build(dict(geom=g4, hits=sub, seeds=ev["seeds"]), dict(prm, max_cand=2))
+    assert list(h["hit_ids"][:, 0]) == [0, 1, 2, 3]
+
+
+def test_nan_child_is_dropped_and_its_parent_offered_to_best_short():
+    """Reading R1: same hand-placed event and hand-written lists as the oracle pin of the same name."""
+    from gpu_helpers import gpu_build
+    from hand_events import nan_child_event
+    ev, prm = nan_child_event(bad_layer=4)
+    h = gpu_build(ev, dict(prm, max_cand=1))
+    assert list(h["hit_ids"][:, 0]) == [0, 1, 2, 3, -2, -2]
+    assert h["nhits"][0] == 4 and h["nmiss"][0] == 0 and (h["status"][0] & 32) == 0
+    assert np.all(np.isfinite(h["par"][:, 0])) and np.all(np.isfinite(h["cov"][:, 0]))
+    r, _ = run_build(ev, dict(prm, max_cand=1))
+    lay = ev["geom"]["layers"][3]
+    assert parity.param_errors(h["par"], r["par"], np.array([abs(lay["pos"])])).max() <= parity.TOL_PAR
+    assert parity.cov_errors(h["cov"], r["cov"], r["par"], np.array([1])).max() <= parity.TOL_COV
+    assert abs(h["chi2"][0] - r["chi2"][0]) <= 1e-3 * max(r["chi2"][0], 1.0)
+    h3 = gpu_build(ev, dict(prm, max_cand=3))
+    assert list(h3["hit_ids"][:, 0]) == [0, 1, 2, 3, -1, 5] and h3["nhits"][0] == 5 and h3["nmiss"][0] == 1
+    ev3, _ = nan_child_event(bad_layer=3)
+    h4 = gpu_build(ev3, dict(prm, max_cand=1))
+    assert (h4["status"][0] & 32) and h4["nhits"][0] == 3 and list(h4["hit_ids"][:, 0]) == [0, 1, 2, -2, -2, -2]
+
+
+def test_build_with_scores_where_a_miss_can_outrank_a_hit():
+    """score_hit + score_miss < chi2_cut: a miss child (score - 1) outranks a hit child with chi2 > 6 (score + 5 - chi2),
+    so a parent's children are no longer ordered hits-first; the selection must still follow the total order U14
+    (on the oracle this changes 45 % of the hit lists of this sample)."""
+    ev, prm = datagen.config(2, scale=0.03)
+    prm = dict(prm, score_hit=5.0, score_miss=1.0)
+    r, h = run_build(ev, prm)
+    compare_build(ev, prm, r, h)
+    base = run_build(ev, datagen.default_params(max_cand=6))[0]
+    assert (np.any(base["hit_ids"] != r["hit_ids"], axis=0)).mean() > 0.3       # the parameters do change the answer

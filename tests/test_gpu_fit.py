@@ -4,8 +4,8 @@ import numpy as np
 import pytest
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
-from paper_2002_06295_b200 import parity
+from workloads import datagen
+from workloads import parity
 
 pytestmark = pytest.mark.gpu
 

@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
 
 pytestmark = pytest.mark.gpu
 

@@ -11,7 +11,7 @@ import os, sys, json
 sys.path.insert(0, %r)
 import numpy as np, torch, torch.distributed as dist
 import bench
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
 rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
 dist.init_process_group("gloo")
 seed = bench.rank_seed(7, rank)

@@ -10,7 +10,8 @@ import numpy as np
 import pytest
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
+from hand_events import tie_event, nan_child_event, TIE_EXPECTED
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -346,3 +347,72 @@ def test_remove_duplicates_on_built_tracks(small_build_event):
     d = o.remove_duplicates(np.array([0, len(sel)], np.int32), r["hit_ids"], r["nhits"], r["score"].astype(np.float32))
     assert np.all(d["keep"][100:] == 0)                                        # the later twin goes
     assert d["keep"][:100].mean() > 0.95
+
+
+# ---- U14 keys 3 and 4 (lower parent rank, lower hit id) ------------------------------------------------------
+@pytest.mark.parametrize("cap", [1, 2])
+def test_u14_ties_lower_hit_id_then_lower_parent_rank(cap):
+    ev, prm = tie_event()
+    s = ev["seeds"]
+    o = mkfo.Oracle(ev["geom"], dict(prm, max_cand=cap))
+    idx = o.build_hit_index(ev["hits"])
+    for brute in (False, True):
+        r = o.build_tracks(ev["hits"], idx, s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"], brute_force=brute)
+        assert list(r["hit_ids"][:, 0]) == TIE_EXPECTED[cap]
+        assert r["nhits"][0] == 5 and r["nmiss"][0] == 0 and r["status"][0] == 0
+    # the twins really tie: building with only one of them gives the same chi2 and score bit for bit
+    for drop in (3, 4):
+        keep = np.array([i for i in range(6) if i != drop])
+        h = ev["hits"]
+        sub = dict(n_events=1, x=h["x"][keep], y=h["y"][keep], z=h["z"][keep], V=np.ascontiguousarray(h["V"][:, keep]),
+                   layer_off=np.array([0, 1, 2, 3, 4, 5], np.int32))
+        r1 = o.build_tracks(sub, o.build_hit_index(sub), s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+        assert r1["chi2"][0] == r["chi2"][0] and r1["score"][0] == r["score"][0]
+
+
+def test_u14_tie_on_the_last_layer_reaches_the_output_through_best_short():
+    """The same twins on the LAST layer (no later layer to break the tie): the final choice among equal candidates is
+    the first in rank order (stable), i.e. again the lower hit id."""
+    ev, prm = tie_event()
+    h, s = ev["hits"], ev["seeds"]
+    g4 = datagen.geometry_barrel(5, 4.0, 20.0, 100.0, 0.0)
+    g4 = dict(g4, layers=g4["layers"][:4], plan_off=np.array([0, 4], np.int32), plan_layers=np.arange(4, dtype=np.int32))
+    sub = dict(n_events=1, x=h["x"][:5], y=h["y"][:5], z=h["z"][:5], V=np.ascontiguousarray(h["V"][:, :5]),
+               layer_off=np.array([0, 1, 2, 3, 5], np.int32))
+    o = mkfo.Oracle(g4, dict(prm, max_cand=2))
+    r = o.build_tracks(sub, o.build_hit_index(sub), s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    assert list(r["hit_ids"][:, 0]) == [0, 1, 2, 3]
+
+
+# ---- R1: a child whose update is not finite ------------------------------------------------------------------
+def test_nan_child_is_dropped_and_its_parent_offered_to_best_short():
+    """Reading R1 (C9.4 / C9.6): the non-finite child never becomes a candidate; its parent, as it stood before the
+    layer, competes for the seed's best-short slot. Expected lists written by hand."""
+    ev, prm = nan_child_event(bad_layer=4)
+    s = ev["seeds"]
+    # cap 1: on disk 4 the only ranked child is the accepted bad hit (chi2 < cut beats the miss child); it is not
+    # finite -> dropped, the live set is empty and the parent (hits 0..3, 4 >= min_hits_keep) is the best short
+    o = mkfo.Oracle(ev["geom"], dict(prm, max_cand=1))
+    idx = o.build_hit_index(ev["hits"])
+    r = o.build_tracks(ev["hits"], idx, s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    assert list(r["hit_ids"][:, 0]) == [0, 1, 2, 3, -2, -2]
+    assert r["nhits"][0] == 4 and r["nmiss"][0] == 0 and (r["status"][0] & 32) == 0
+    assert np.all(np.isfinite(r["par"][:, 0])) and np.all(np.isfinite(r["cov"][:, 0]))
+    # cap 3: after disk 3 the live set is [hits 0..3, hits 0..2 + one miss]. On disk 4 the ranked children are the bad
+    # hit on the first (score 150 - chi2), then the first one's miss child and the bad hit on the second (both
+    # 105 - chi2, in either order). Both bad-hit children are dropped (the second one's parent has 3 hits < 4: no
+    # offer); the miss child lives on, finds hit 5 and wins with 5 hits and one miss (135 - chi2) over the offered
+    # parent (120 - chi2')
+    o3 = mkfo.Oracle(ev["geom"], dict(prm, max_cand=3))
+    r2 = o3.build_tracks(ev["hits"], idx, s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    assert list(r2["hit_ids"][:, 0]) == [0, 1, 2, 3, -1, 5]
+    assert r2["nhits"][0] == 5 and r2["nmiss"][0] == 1
+    # with a sane covariance on that hit the full track is found
+    ev_ok = dict(ev, hits=dict(ev["hits"], V=ev["hits"]["V"].copy()))
+    ev_ok["hits"]["V"][0, 4] = ev["hits"]["V"][0, 3]
+    r3 = o.build_tracks(ev_ok["hits"], o.build_hit_index(ev_ok["hits"]), s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    assert list(r3["hit_ids"][:, 0]) == [0, 1, 2, 3, 4, 5]
+    # bad hit on the layer right after the seed: the parent has 3 hits < min_hits_keep -> nothing qualifies, TRUNCATED seed
+    ev3, _ = nan_child_event(bad_layer=3)
+    r4 = o.build_tracks(ev3["hits"], o.build_hit_index(ev3["hits"]), s["par"], s["cov"], s["q"], s["event"], s["hits"], s["plan"])
+    assert (r4["status"][0] & 32) and r4["nhits"][0] == 3 and list(r4["hit_ids"][:, 0]) == [0, 1, 2, -2, -2, -2]

@@ -2,7 +2,7 @@
 import numpy as np
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
 
 
 def cidx(i, j):

@@ -4,7 +4,7 @@ been taken out of the event."""
 import numpy as np
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
 
 
 def test_mask_rules_by_hand():

@@ -3,7 +3,7 @@ of the passage, and an independent brute-force formulation on random data."""
 import numpy as np
 
 from oracle import mkfo
-from paper_2002_06295_b200 import datagen
+from workloads import datagen
 
 
 def run(adc, noise=4.0, bad=None, off=None, **kw):
