@@ -40,7 +40,8 @@ enum { MKF_PROP_UNREACHABLE = 1, /* next surface not reachable going forward wit
        MKF_S_NOT_PD = 4,         /* residual covariance S = C(0:3,0:3)+V not positive definite (C6) */
        MKF_NAN = 8,              /* non-finite value after an update */
        MKF_STOPPED_ELOSS = 16,   /* energy exhausted by dE/dx (C5) */
-       MKF_TRUNCATED = 32 };     /* building: nothing with >= min_hits_keep hits; the seed itself is returned */
+       MKF_TRUNCATED = 32 };     /* building: nothing with >= min_hits_keep hits; the seed itself is returned. Also set on a
+                                    track whose plan id, event id or a hit id lies outside the ranges of the call */
 
 enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total over plans */, MKF_MAX_CAND = 8 };
 
@@ -72,9 +73,15 @@ typedef struct { float chi2_cut;      /* hit accepted iff chi2 < chi2_cut (30) *
                  float dup_frac;      /* duplicate if shared/min(nhits) > dup_frac (0.5) */ } mkf_params;
 
 /* Hits of n_events events, grouped by (event, layer): the hits of (ev, l) are the ids
- * layer_off[ev*(n_layers+1)+l] .. layer_off[ev*(n_layers+1)+l+1]; ids are global (0..n_hits). */
+ * layer_off[ev*(n_layers+1)+l] .. layer_off[ev*(n_layers+1)+l+1]; ids are global (0..n_hits).
+ * rec (may be NULL): the same hits as 48-byte records rec[12*id .. 12*id+11] = {x, y, z, Vxx | Vxy, Vyy, Vxz, Vyz |
+ * Vzz, 0, 0, 0}, 16-byte aligned, written by mkf_pack_hits (or by the caller). The SoA planes serve streaming
+ * access in id order (36 B per hit); a gather by scattered hit id (a fit over hit lists that are not sorted, the
+ * update step of the building) costs 9 sectors = 288 B per hit on the planes and 2 sectors = 64 B on a record, so
+ * every kernel that gathers by id reads `rec` when it is given. x, y, z, V must be valid in either case. */
 typedef struct { int n_events; int n_hits; const int* layer_off;
-                 const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */ } mkf_hits;
+                 const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */
+                 const float* rec; } mkf_hits;
 
 /* The phi/eta-binned hit index (C8), written by mkf_build_hit_index, read by mkf_build_tracks.
  * bin_off  [n_events*n_layers*n_phi*n_eta + 1]  exclusive prefix of hits per bin (bin = ie*n_phi + ip inside
@@ -100,6 +107,10 @@ size_t mkf_workspace_bytes(const mkf_ctx*, int call_id, int n_events, int n_hits
 long long mkf_launch_count(const mkf_ctx*);
 /* Longest plan of the geometry (the leading dimension callers give track_hits / hit_ids). */
 int mkf_max_plan_len(const mkf_ctx*);
+
+/* Writes the 48-byte hit records (see mkf_hits.rec) of hits->x,y,z,V to rec_out[12 * n_hits] (device, 16-byte
+ * aligned). One streaming pass: 36 B read + 48 B written per hit. hits->rec is ignored. Errors: INVALID_ARG, CUDA_ERROR. */
+int mkf_pack_hits(mkf_ctx*, const mkf_hits*, float* rec_out, void* stream);
 
 /* ---- the four calls of BASELINE.json north_star -------------------------------------------------------- */
 /* a1 / C8 ("data preparation ... for each event"). Errors: INVALID_ARG, WORKSPACE_TOO_SMALL,
@@ -135,6 +146,14 @@ int mkf_build_tracks(mkf_ctx*, const mkf_hits*, const mkf_hit_index*, const mkf_
             mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status,
             void* ws, size_t ws_bytes, void* stream);
 
+/* Work counters of mkf_build_tracks (SURVEY.md §8d asks for candidate-layer-steps/s and chi2 evaluations/s): while
+ * `counters` (device, 8 x unsigned long long, zeroed by the caller) is set, every mkf_build_tracks call on this context
+ * adds to it: [0] candidate-layer-steps (propagations that landed on a layer), [1] hit positions tested inside windows,
+ * [2] chi2 evaluations (hits that passed the position test: their covariance is read), [3] hits accepted (chi2 < cut),
+ * [4] Kalman updates, [5..7] reserved. NULL (the default) switches counting off. The counts do not depend on timing
+ * and equal the oracle's n_chi2_evals only in order of magnitude (the oracle evaluates chi2 on whole bins). */
+int mkf_set_build_counters(mkf_ctx*, unsigned long long* counters);
+
 /* a10 / C10 ("duplicate tracks ... explicitly removed in an additional processing step").
  * track_off[n_events+1] (device): tracks of event ev are track_off[ev]..track_off[ev+1]; n = total tracks (the
  * plane stride of hit_ids); n_hits = size of the hit-id space. keep[n] = 0/1, n_kept[n_events]. */
@@ -168,9 +187,10 @@ int mkf_build_hit_index_masked(mkf_ctx*, const mkf_hits*, const unsigned char* m
  * 16-byte aligned and bad 8-byte aligned; module_off[0] = 0 and module_off[n_modules] = n_strips (not checked: the
  * offsets live on the device); n_strips <= 2^31 - 16384; max_holes + max_bad <= 31 (MKF_UNSUPPORTED otherwise).
  * Output (ordered by module, then first strip): module, first and last strip (index inside the module), charge =
- * sum adc, bary = sum adc (strip + 1/2) / sum adc in strip units. *n_clusters = number of clusters found; only the
- * first `capacity` records are kept: with n_clusters > capacity the output is incomplete and the caller retries with
- * more room. */
+ * sum adc, bary = sum adc (strip + 1/2) / sum adc in strip units. *n_clusters = number of clusters found. With
+ * *n_clusters > capacity ONLY *n_clusters is defined (the record arrays then hold an unspecified subset with holes,
+ * because records are staged in tile-arrival order): the caller retries with more room. mkf_cluster_strips_host
+ * copies no records back in that case. */
 typedef struct { float seed_thr, chan_thr, clus_thr; int min_charge, max_holes, max_bad; } mkf_strip_params;
 typedef struct {
   int n_modules, n_strips;
@@ -191,10 +211,19 @@ int mkf_cluster_strips(mkf_ctx*, const mkf_strips*, const mkf_strip_params*, con
             void* ws, size_t ws_bytes, void* stream);
 
 /* ---- host-buffer entry points (end-to-end use: all pointers HOST; synchronous) ------------------------- */
-/* Same semantics as mkf_fit, every pointer (hits arrays included) in host memory. Device memory is taken from
- * the CUDA stream-ordered pool and released before returning. h2d_bytes/d2h_bytes (may be NULL) receive the
+/* Device memory of the host entry points is an arena owned by the context: it grows to the largest call seen and is
+ * freed by mkf_destroy, so repeated calls allocate nothing ("a memory pool to pay the allocation overhead
+ * only at the beginning and end of job"). Copies are asynchronous (and overlap the kernels) only from pinned host
+ * memory; pageable buffers work but are staged by the driver. One host call per context at a time.
+ *
+ * mkf_fit_host / mkf_fit_backward_host: same semantics as mkf_fit / mkf_fit_backward, every pointer (hits arrays
+ * included; hits->rec is ignored) in host memory. The hits go first; the tracks then travel in ranges of 256 k on three
+ * streams (copy in, fit, copy out) so that copies and kernels overlap. h2d_bytes/d2h_bytes (may be NULL) receive the
  * bytes copied each way. */
 int mkf_fit_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_host, const signed char* plan,
+            const int* track_hits, int max_plan_len, mkf_states* out_host, float* chi2, int* nfit, unsigned* status,
+            long long* h2d_bytes, long long* d2h_bytes);
+int mkf_fit_backward_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_host, const signed char* plan,
             const int* track_hits, int max_plan_len, mkf_states* out_host, float* chi2, int* nfit, unsigned* status,
             long long* h2d_bytes, long long* d2h_bytes);
 /* mkf_build_hit_index + mkf_build_tracks (+ mkf_remove_duplicates if keep != NULL; seeds must then be grouped
@@ -204,8 +233,9 @@ int mkf_build_host(mkf_ctx*, const mkf_hits* hits_host, const mkf_states* seeds_
             float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, unsigned char* keep,
             long long* h2d_bytes, long long* d2h_bytes);
 /* mkf_cluster_strips on host buffers (pinned memory makes the copies asynchronous). Device memory comes from the
- * stream-ordered pool, so repeated calls pay no allocation ("using a memory pool to pay the allocation
- * overhead only at the beginning and end of job"). *out->n_clusters is the number found; min(that, capacity) are copied. */
+ * context's arena, so repeated calls pay no allocation ("using a memory pool to pay the allocation
+ * overhead only at the beginning and end of job"). *out->n_clusters is the number found; the records are copied
+ * only if they all fit (n_clusters <= capacity), see mkf_cluster_strips. */
 int mkf_cluster_strips_host(mkf_ctx*, const mkf_strips* strips_host, const mkf_strip_params*, const mkf_clusters* out_host,
             long long* h2d_bytes, long long* d2h_bytes);
 #ifdef __cplusplus

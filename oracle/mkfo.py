@@ -14,16 +14,22 @@ _SRC = [os.path.join(_HERE, "mkfo.cpp"), os.path.join(_HERE, "mkfo.h")]
 
 
 def build(force=False):
-    """Compile the oracle. Returns the path of the shared library."""
-    if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in _SRC):
-        return _LIB
-    base = ["-O2", "-std=c++17", "-fPIC", "-shared", "-Wall", "-Wno-misleading-indentation", "-o", _LIB, _SRC[0]]
+    """Compile the oracle. Returns the path of the shared library.
+    MKFO_SANITIZE=1 in the environment builds oracle/libmkfo_san.so with -fsanitize=address,undefined instead (-O1 -g,
+    no OpenMP); run the tests with LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)"
+    and ASAN_OPTIONS=detect_leaks=0 (python itself leaks). DESIGN.md §2 records the outcome."""
+    san = os.environ.get("MKFO_SANITIZE") == "1"
+    out = os.path.join(_HERE, "libmkfo_san.so") if san else _LIB
+    if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(s) for s in _SRC):
+        return out
+    opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if san else ["-O2"]
+    base = opt + ["-std=c++17", "-fPIC", "-shared", "-Wall", "-Wno-misleading-indentation", "-o", out, _SRC[0]]
     errs = []
     for cxx in ("/usr/bin/g++", "g++", "c++"):
-        for omp in (["-fopenmp"], []):
+        for omp in ([[]] if san else (["-fopenmp"], [])):
             r = subprocess.run([cxx] + omp + base, capture_output=True, text=True)
             if r.returncode == 0:
-                return _LIB
+                return out
             errs.append(r.stderr[-500:])
     raise RuntimeError("oracle build failed:\n" + "\n".join(errs))
 

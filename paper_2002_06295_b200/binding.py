@@ -17,8 +17,8 @@ PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8,
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
-           "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_build_host",
-           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked"]
+           "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_fit_backward_host", "mkf_build_host",
+           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters"]
 
 
 class Layer(C.Structure):
@@ -40,7 +40,7 @@ class Params(C.Structure):
 
 class Hits(C.Structure):
     _fields_ = [("n_events", C.c_int), ("n_hits", C.c_int), ("layer_off", C.c_void_p), ("x", C.c_void_p),
-                ("y", C.c_void_p), ("z", C.c_void_p), ("V", C.c_void_p)]
+                ("y", C.c_void_p), ("z", C.c_void_p), ("V", C.c_void_p), ("rec", C.c_void_p)]
 
 
 class HitIndex(C.Structure):
@@ -94,6 +94,8 @@ def lib():
         L.mkf_mask_hits.argtypes = [vp, i, i, vp, i, vp, vp, vp, i, C.c_float, vp, vp]
         L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
         L.mkf_fit_backward.argtypes = L.mkf_fit.argtypes
+        L.mkf_pack_hits.argtypes = [vp, C.POINTER(Hits), vp, vp]
+        L.mkf_set_build_counters.argtypes = [vp, vp]
         L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
                                        C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.mkf_remove_duplicates.argtypes = [vp, i, i, i, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
@@ -101,6 +103,7 @@ def lib():
         L.mkf_cluster_strips.argtypes = [vp, C.POINTER(Strips), C.POINTER(StripParams), C.POINTER(Clusters), vp, sz, vp]
         L.mkf_cluster_strips_host.argtypes = [vp, C.POINTER(Strips), C.POINTER(StripParams), C.POINTER(Clusters), ll, ll]
         L.mkf_fit_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, ll, ll]
+        L.mkf_fit_backward_host.argtypes = L.mkf_fit_host.argtypes
         L.mkf_build_host.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, vp, i, C.POINTER(States), vp, vp,
                                      vp, vp, vp, vp, vp, ll, ll]
         _lib = L
@@ -178,8 +181,15 @@ class Context:
     # ---- marshalling helpers ------------------------------------------------------------------------------
     @staticmethod
     def hits_struct(h, ptr, i32=torch.int32, f32=torch.float32):
+        rec = h.get("rec")
         return Hits(int(h["n_events"]), int(h["x"].shape[0]), ptr(h["layer_off"], i32), ptr(h["x"], f32), ptr(h["y"], f32),
-                    ptr(h["z"], f32), ptr(h["V"], f32))
+                    ptr(h["z"], f32), ptr(h["V"], f32), ptr(rec, f32) if rec is not None else None)
+
+    def pack_hits(self, hits, rec):
+        """mkf_pack_hits: rec float32 CUDA tensor [n_hits * 12] receives the 48-byte hit records (mkf_hits.rec)."""
+        hs = self.hits_struct(hits, _dev)
+        rc = self.L.mkf_pack_hits(self.h, C.byref(hs), _dev(rec, torch.float32), _stream())
+        self._check(rc, "mkf_pack_hits")
 
     # ---- the four calls -----------------------------------------------------------------------------------
     def build_hit_index(self, hits, out, ws, mask=None):
@@ -224,7 +234,12 @@ class Context:
                             _dev(status, torch.int32), None, 0, _stream())
         self._check(rc, "mkf_fit_backward" if backward else "mkf_fit")
 
-    def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status):
+    def set_build_counters(self, counters):
+        """mkf_set_build_counters: int64 CUDA tensor [8] (zeroed by the caller) or None."""
+        self._counters = counters                               # keep the tensor alive while the library holds its address
+        self._check(self.L.mkf_set_build_counters(self.h, _dev(counters, torch.int64) if counters is not None else None), "mkf_set_build_counters")
+
+    def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status, ws=None):
         hs = self.hits_struct(hits, _dev)
         packed = idx.get("packed")
         ix = HitIndex(_dev(idx["bin_off"], torch.int32), _dev(idx["sorted_id"], torch.int32), _dev(idx["vmax"], torch.float32),
@@ -236,7 +251,7 @@ class Context:
                                      _dev(seed_hits, torch.int32), _dev(plan, torch.int8), int(hit_ids.shape[0]), C.byref(o),
                                      _dev(chi2, torch.float32), _dev(score, torch.float32), _dev(nhits, torch.int32),
                                      _dev(nmiss, torch.int32), _dev(hit_ids, torch.int32), _dev(status, torch.int32),
-                                     None, 0, _stream())
+                                     ws.data_ptr() if ws is not None else None, ws.numel() if ws is not None else 0, _stream())
         self._check(rc, "mkf_build_tracks")
 
     def remove_duplicates(self, n_hits, track_off, hit_ids, nhits, score, keep, n_kept, ws):
@@ -275,13 +290,13 @@ class Context:
         h2d, d2h = C.c_longlong(0), C.c_longlong(0)
         rc = self.L.mkf_cluster_strips_host(self.h, C.byref(s), C.byref(sp), C.byref(o), C.byref(h2d), C.byref(d2h))
         self._check(rc, "mkf_cluster_strips_host")
-        k = min(int(nc[0]), capacity)
+        k = int(nc[0]) if int(nc[0]) <= capacity else 0          # overflow: only the count is defined (mkf.h)
         out = {key: v[:k] for key, v in out.items()}
         out["n_clusters"], out["h2d_bytes"], out["d2h_bytes"] = int(nc[0]), h2d.value, d2h.value
         return out
 
     # ---- host-buffer entry points -------------------------------------------------------------------------
-    def fit_host(self, hits, seeds, plan, track_hits):
+    def fit_host(self, hits, seeds, plan, track_hits, backward=False):
         """All arguments numpy / CPU tensors; returns dict of numpy arrays plus the bytes copied each way."""
         f32, i32, i8 = np.float32, np.int32, np.int8
         hs = self.hits_struct(hits, _host, i32, f32)
@@ -291,7 +306,8 @@ class Context:
         s = States(n, _host(seeds["par"], f32), _host(seeds["cov"], f32), _host(seeds["q"], i8))
         o = States(n, out["par"].ctypes.data, out["cov"].ctypes.data, _host(seeds["q"], i8))
         h2d, d2h = C.c_longlong(0), C.c_longlong(0)
-        rc = self.L.mkf_fit_host(self.h, C.byref(hs), C.byref(s), _host(plan, i8), _host(track_hits, i32),
+        call = self.L.mkf_fit_backward_host if backward else self.L.mkf_fit_host
+        rc = call(self.h, C.byref(hs), C.byref(s), _host(plan, i8), _host(track_hits, i32),
                                  int(track_hits.shape[0]), C.byref(o), out["chi2"].ctypes.data, out["nfit"].ctypes.data,
                                  out["status"].ctypes.data, C.byref(h2d), C.byref(d2h))
         self._check(rc, "mkf_fit_host")
@@ -358,6 +374,10 @@ def alloc_hit_index(ctx, n_events, n_hits, packed=True, device="cuda"):
                packed=torch.empty(n_hits * 12, dtype=torch.float32, device=device) if packed else None)
     ws = torch.empty(max(ctx.workspace_bytes(CALL_BUILD_HIT_INDEX, n_events, n_hits, 0), 256), dtype=torch.uint8, device=device)
     return out, ws
+
+
+def alloc_build_ws(ctx, n_events, n_hits, n_seeds, device="cuda"):
+    return torch.empty(max(ctx.workspace_bytes(CALL_BUILD_TRACKS, n_events, n_hits, n_seeds), 256), dtype=torch.uint8, device=device)
 
 
 def alloc_fit_out(n, device="cuda"):

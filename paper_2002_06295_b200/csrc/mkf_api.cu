@@ -39,10 +39,34 @@ extern "C" int mkf_create(mkf_ctx** out, const mkf_geometry* geom, const mkf_par
   return MKF_OK;
 }
 
-extern "C" void mkf_destroy(mkf_ctx* c) { delete c; }
+namespace mkf { void host_state_free(mkf_ctx*); }
+extern "C" void mkf_destroy(mkf_ctx* c) { if (c) host_state_free(c); delete c; }
 extern "C" const char* mkf_last_error(const mkf_ctx* c) { return c ? c->err : "null context"; }
 extern "C" long long mkf_launch_count(const mkf_ctx* c) { return c ? c->launches : 0; }
 extern "C" int mkf_max_plan_len(const mkf_ctx* c) { return c ? c->max_plan_len : 0; }
+extern "C" int mkf_set_build_counters(mkf_ctx* c, unsigned long long* counters) { if (!c) return MKF_INVALID_ARG; c->build_counters = counters; return MKF_OK; }
+
+// ---- 48-byte hit records (mkf_hits.rec): one streaming pass over the SoA planes ------------------------------
+__global__ void __launch_bounds__(256) mkf_pack_hits_kernel(int n, const float* __restrict__ x, const float* __restrict__ y,
+                                                            const float* __restrict__ z, const float* __restrict__ V, float4* __restrict__ rec) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  const size_t nh = (size_t)n;
+  float4* r = rec + (size_t)3 * i;
+  r[0] = make_float4(x[i], y[i], z[i], V[i]);
+  r[1] = make_float4(V[nh + i], V[2 * nh + i], V[3 * nh + i], V[4 * nh + i]);
+  r[2] = make_float4(V[5 * nh + i], 0.f, 0.f, 0.f);
+}
+
+extern "C" int mkf_pack_hits(mkf_ctx* c, const mkf_hits* h, float* rec_out, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || h->n_hits < 0) return fail(c, MKF_INVALID_ARG, "mkf_pack_hits: bad argument");
+  if (h->n_hits == 0) return MKF_OK;
+  if (!h->x || !h->y || !h->z || !h->V || !rec_out || ((size_t)rec_out & 15)) return fail(c, MKF_INVALID_ARG, "mkf_pack_hits: null or misaligned array");
+  mkf_pack_hits_kernel<<<(h->n_hits + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->n_hits, h->x, h->y, h->z, h->V, (float4*)rec_out);
+  MKF_LAUNCHED(c, "mkf_pack_hits_kernel");
+  return MKF_OK;
+}
 
 // ---- fit (a11 / C7): one thread per track, state and covariance in registers for the whole layer loop ----
 #ifndef MKF_FIT_BLOCK
@@ -85,6 +109,23 @@ extern "C" int mkf_fit(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, c
   return fit_common(c, false, h, seeds, plan, track_hits, max_plan_len, out, chi2, nfit, status, stream);
 }
 
+namespace mkf {
+// One launch over the tracks [0, a.n) of FitArgs (plane stride a.ld); used by mkf_fit / mkf_fit_backward and, on
+// track ranges, by the host-buffer entry points.
+int fit_launch(mkf_ctx* c, bool backward, const FitArgs& a, cudaStream_t st) {
+  if (a.n <= 0) return MKF_OK;
+  const int grid = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
+  if (backward) {
+    mkf_fit_backward_kernel<<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
+    MKF_LAUNCHED(c, "mkf_fit_backward_kernel");
+  } else {
+    mkf_fit_kernel<<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
+    MKF_LAUNCHED(c, "mkf_fit_kernel");
+  }
+  return MKF_OK;
+}
+}  // namespace mkf
+
 static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
                       const int* track_hits, int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
                       void* stream) {
@@ -95,18 +136,11 @@ static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_st
   if (!plan || !track_hits || !chi2 || !nfit || !status) return fail(c, MKF_INVALID_ARG, "mkf_fit: null argument");
   if (!h->x || !h->y || !h->z || !h->V || !seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov)
     return fail(c, MKF_INVALID_ARG, "mkf_fit: null array");
+  if ((size_t)h->rec & 15) return fail(c, MKF_INVALID_ARG, "mkf_fit: hit records not 16-byte aligned");
   FitArgs a;
   a.hits = hits_dev(h);
-  a.n = seeds->n; a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.plan = plan;
+  a.n = seeds->n; a.ld = seeds->n; a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.plan = plan;
   a.track_hits = track_hits; a.max_plan_len = max_plan_len;
   a.par_out = out->par; a.cov_out = out->cov; a.chi2 = chi2; a.nfit = nfit; a.status = status;
-  const int grid = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
-  if (backward) {
-    mkf_fit_backward_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
-    MKF_LAUNCHED(c, "mkf_fit_backward_kernel");
-  } else {
-    mkf_fit_kernel<<<grid, FIT_BLOCK, 0, (cudaStream_t)stream>>>(c->g, c->p, a);
-    MKF_LAUNCHED(c, "mkf_fit_kernel");
-  }
-  return MKF_OK;
+  return fit_launch(c, backward, a, (cudaStream_t)stream);
 }

@@ -6,12 +6,24 @@
 #include "../../include/mkf.h"
 #include "mkf_dev.cuh"
 
+// State of the host-buffer entry points (mkf_host.cu): a grow-only device arena, three streams (copy in, kernels,
+// copy out) and a pool of events, all created at the first host call and kept until mkf_destroy, so that repeated
+// calls allocate nothing ("a memory pool to pay the allocation overhead only at the beginning and end of job").
+struct mkf_host_state {
+  char* base = nullptr; size_t cap = 0;
+  cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
+  cudaEvent_t ev[128] = {};
+  int n_ev = 0;
+};
+
 struct mkf_ctx {
   mkf::GeomDev g;
   mkf::ParamsDev p;
   int max_plan_len;
   long long launches;
   char err[256];
+  mkf_host_state* host;
+  unsigned long long* build_counters;      // device, or null (mkf_set_build_counters)
 };
 
 namespace mkf {
@@ -33,6 +45,6 @@ inline int cuda_fail(mkf_ctx* c, cudaError_t e, const char* where) {
 inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 inline HitsDev hits_dev(const mkf_hits* h) {
   HitsDev d; d.n_events = h->n_events; d.n_hits = h->n_hits; d.layer_off = h->layer_off;
-  d.x = h->x; d.y = h->y; d.z = h->z; d.V = h->V; return d;
+  d.x = h->x; d.y = h->y; d.z = h->z; d.V = h->V; d.rec = (const float4*)h->rec; return d;
 }
 }  // namespace mkf

@@ -20,7 +20,7 @@ struct ParamsDev {
   float score_hit, score_miss, graze_cos_min; int material_flags; float dup_frac;
 };
 
-struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; };
+struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; const float4* rec; };
 
 // Parameters of a caller's state; the covariance is read separately by the first propagation (commit_first).
 MKF_HD void load_params(KState& S, const float* par, size_t n, size_t i) {
@@ -73,6 +73,14 @@ MKF_HD unsigned step_to_layer(KState& S, bool first, const float* cov, size_t n,
 }
 
 MKF_HD void load_hit(Hit& H, const HitsDev& h, int id) {
+#ifdef __CUDA_ARCH__
+  if (h.rec) {                                                   // 48-byte record: 2 sectors instead of 9 for a scattered id
+    const float4* r = h.rec + (size_t)3 * id;
+    const float4 a = __ldg(r), b = __ldg(r + 1), c = __ldg(r + 2);
+    H.x = a.x; H.y = a.y; H.z = a.z; H.v[0] = a.w; H.v[1] = b.x; H.v[2] = b.y; H.v[3] = b.z; H.v[4] = b.w; H.v[5] = c.x;
+    return;
+  }
+#endif
   const size_t nh = (size_t)h.n_hits;
   H.x = h.x[id]; H.y = h.y[id]; H.z = h.z[id];
 #pragma unroll
@@ -82,7 +90,9 @@ MKF_HD void load_hit(Hit& H, const HitsDev& h, int id) {
 // ---- fit of one track (C7) ------------------------------------------------------------------------------
 struct FitArgs {
   HitsDev hits;
-  int n; const float* par; const float* cov; const signed char* q; const signed char* plan;
+  int n;                       // tracks of this launch
+  int ld;                      // plane stride of every per-track array (>= n; the host entry points launch on track ranges)
+  const float* par; const float* cov; const signed char* q; const signed char* plan;
   const int* track_hits; int max_plan_len;
   float* par_out; float* cov_out; float* chi2; int* nfit; unsigned* status;
 };
@@ -91,8 +101,13 @@ struct FitArgs {
 // (unreachable, grazing, energy exhausted) leave the state as it was; the two that can only be seen after the
 // update (S not positive definite, non-finite result) re-run the track from its seed up to the failing step.
 MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
-  const size_t n = (size_t)a.n;
+  const size_t n = (size_t)a.ld;
   const int pl = a.plan[i];
+  if ((unsigned)pl >= (unsigned)g.n_plans) {                     // not a plan of this geometry: the seed goes out, flagged
+    copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
+    a.chi2[i] = 0.f; a.nfit[i] = 0; a.status[i] = ST_TRUNC;
+    return;
+  }
   const int p0 = g.plan_off[pl];
   int plen = g.plan_off[pl + 1] - p0;
   if (plen > a.max_plan_len) plen = a.max_plan_len;
@@ -125,6 +140,7 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
       th += n;
       hid_next = s + 1 < stop_at_loop ? *th : -1;
       if (hid < 0 || stopped) continue;
+      if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; continue; }    // not a hit of this call
       const LayerDev L = g.layers[g.plan_layers[p0 + s]];
       Hit H; load_hit(H, a.hits, hid);
       const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
@@ -152,8 +168,13 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
 // layer's material is given back too (done on the covariance at the output boundary), so the result is the state
 // before it. A failing step stops the track, which keeps the state after its last good update.
 MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
-  const size_t n = (size_t)a.n;
+  const size_t n = (size_t)a.ld;
   const int pl = a.plan[i];
+  if ((unsigned)pl >= (unsigned)g.n_plans) {
+    copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
+    a.chi2[i] = 0.f; a.nfit[i] = 0; a.status[i] = ST_TRUNC;
+    return;
+  }
   const int p0 = g.plan_off[pl];
   int plen = g.plan_off[pl + 1] - p0;
   if (plen > a.max_plan_len) plen = a.max_plan_len;
@@ -173,6 +194,7 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     for (int s = plen - 1; s > stop_at; s--) {
       const int hid = a.track_hits[(size_t)s * n + i];
       if (hid >= 0 && !stopped) do {
+        if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; break; }
         const int li = g.plan_layers[p0 + s];
         const LayerDev L = g.layers[li];
         Hit H; load_hit(H, a.hits, hid);

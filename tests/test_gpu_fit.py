@@ -187,3 +187,89 @@ def test_fit_backward_barrel_endcap_with_curling_tracks():
     ev, prm = datagen.config(3, scale=0.01)           # disks and cylinders, soft tracks that come back in radius
     r, h = check_backward(ev, prm)
     assert (r["status"] != 0).sum() >= 1
+
+
+def test_fit_on_shuffled_hits_with_48_byte_records_is_bit_identical():
+    """mkf_hits.rec (mkf_pack_hits): the same hits gathered from 48-byte records instead of the nine SoA planes, on hit
+    ids in random order; the result must not change by a bit, forward and backward, and equals the id-ordered fit."""
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    from workloads import assemble
+    ev, prm = datagen.config(1, scale=0.01)           # 40 000 helices, 17 layers
+    s = {k: ev["seeds"][k] for k in ("par", "cov", "q", "plan", "track_hits")}
+    h2, s2 = assemble.shuffle_hit_order(ev["hits"], s, 5)
+    assert not np.array_equal(s2["track_hits"], s["track_hits"])
+    from gpu_helpers import gpu_fit
+    base = gpu_fit(ev, prm, s)
+    ctx = B.Context(ev["geom"], prm)
+    dh = B.hits_to_device(h2)
+    sd = B.to_device(s2, ["par", "cov", "q", "plan", "track_hits"])
+    n = s["par"].shape[1]
+    for backward in (False, True):
+        outs = []
+        for use_rec in (False, True):
+            if use_rec:
+                dh["rec"] = torch.empty(12 * h2["x"].shape[0], dtype=torch.float32, device="cuda")
+                ctx.pack_hits(dh, dh["rec"])
+            else:
+                dh.pop("rec", None)
+            out = B.alloc_fit_out(n)
+            ctx.fit(dh, sd, sd["plan"], sd["track_hits"], out, out["chi2"], out["nfit"], out["status"], backward=backward)
+            torch.cuda.synchronize()
+            outs.append({k: v.cpu().numpy() for k, v in out.items()})
+        for k in ("par", "cov", "chi2", "nfit", "status"):
+            assert np.array_equal(outs[0][k], outs[1][k]), (backward, k)
+            if not backward:
+                assert np.array_equal(outs[1][k].view(np.uint32) if k == "status" else outs[1][k], base[k]), k
+    rec = dh["rec"].cpu().numpy().reshape(-1, 12)
+    assert np.array_equal(rec[:, 0], h2["x"]) and np.array_equal(rec[:, 3:9], h2["V"].T) and not rec[:, 9:].any()
+    ctx.close()
+
+
+def test_fit_host_pipeline_over_several_track_ranges():
+    """mkf_fit_host / mkf_fit_backward_host work on ranges of 256 k tracks on three streams: 600 k tracks (3 ranges, the
+    last one ragged) must give exactly the device path's result; a second call reuses the context's arena."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    from gpu_helpers import gpu_fit
+    from paper_2002_06295_b200 import binding as B
+    geom, prm, hits, seeds, _ = bench.make_fit_workload(9, 0.15)
+    n = seeds["par"].shape[1]
+    assert n == 600000
+    h = gpu_fit(dict(geom=geom, hits=hits), prm, seeds)
+    ctx = B.Context(geom, prm)
+    for rep in range(2):
+        r = ctx.fit_host(hits, seeds, seeds["plan"], seeds["track_hits"])
+        for k in ("par", "cov", "chi2", "nfit"):
+            assert np.array_equal(r[k], h[k]), k
+        assert np.array_equal(r["status"], h["status"])
+        assert r["d2h_bytes"] == n * (27 * 4 + 12)
+        assert r["h2d_bytes"] == hits["x"].shape[0] * 36 + 4 * len(hits["layer_off"]) + n * (27 * 4 + 2 + 4 * seeds["track_hits"].shape[0])
+    hb = gpu_fit(dict(geom=geom, hits=hits), prm, seeds, backward=True)
+    rb = ctx.fit_host(hits, seeds, seeds["plan"], seeds["track_hits"], backward=True)
+    for k in ("par", "cov", "chi2", "nfit"):
+        assert np.array_equal(rb[k], hb[k]), k
+    ctx.close()
+
+
+def test_fit_flags_indices_outside_the_call():
+    """A plan id that is no plan of the geometry, or a hit id >= n_hits: the track is flagged (TRUNCATED) instead of
+    reading out of bounds; its neighbours are not disturbed."""
+    from gpu_helpers import gpu_fit
+    ev, prm = datagen.config(0, scale=0.02)
+    s = {k: ev["seeds"][k].copy() for k in ("par", "cov", "q", "plan", "track_hits")}
+    base = gpu_fit(ev, prm, s)
+    s["plan"][3] = 5
+    s["plan"][4] = -1
+    nh = ev["hits"]["x"].shape[0]
+    s["track_hits"][6, 10] = nh + 7
+    h = gpu_fit(ev, prm, s)
+    for i in (3, 4):
+        assert h["status"][i] == 32 and h["nfit"][i] == 0 and np.array_equal(h["par"][:, i], s["par"][:, i])
+    assert (h["status"][10] & 32) and h["nfit"][10] == 6 and base["nfit"][10] == 10
+    others = np.ones(len(h["nfit"]), bool); others[[3, 4, 10]] = False
+    for k in ("par", "cov", "chi2", "nfit", "status"):
+        assert np.array_equal(h[k][..., others], base[k][..., others]), k
+    hb = gpu_fit(ev, prm, s, backward=True)                         # the backward kernel flags the plan ids the same way
+    assert hb["status"][3] == 32 and hb["status"][4] == 32 and hb["nfit"][3] == 0

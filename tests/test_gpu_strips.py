@@ -23,7 +23,7 @@ def check(d, sp, capacity=None):
 
 
 def test_strips_default_rules_bit_exact():
-    # 3000 modules of 512 / 256 strips: ~1.4 M strips = 700 tiles, modules straddle tile boundaries, ragged tail
+    # 3000 modules of 512 / 256 strips: ~1.4 M strips = 176 tiles of 8192, modules straddle tile boundaries, ragged tail
     d = datagen.make_strips(11, 3000)
     ref = check(d, datagen.default_strip_params())
     assert len(ref["module"]) > 3000
@@ -40,22 +40,25 @@ def test_strips_degenerate_inputs():
     sp = datagen.default_strip_params()
     d = datagen.make_strips(13, 64, strips_per_module=37)                 # tiny modules, length not a multiple of 8
     check(d, sp)
-    # every strip passes: one cluster per module, walked across tiles
-    n = 3 * 2048 + 5
-    off = np.array([0, 1000, 1000, 5000, n], np.int32)                   # an empty module, modules longer than a tile
+    # every strip passes: one cluster per module, walked across tiles (TILE = SC_TILE of csrc/mkf_strips.cu)
+    TILE = 8192
+    n = 3 * TILE + 5
+    off = np.array([0, 9000, 9000, 20000, n], np.int32)                  # an empty module, modules longer than a tile
     full = dict(module_off=off, adc=np.full(n, 100, np.uint16), noise=np.full(n, 4, np.float32), bad=np.zeros(n, np.uint8))
     ref = check(full, sp)
-    assert ref["module"].tolist() == [0, 2, 3] and ref["last"].tolist() == [999, 3999, n - 5001]
-    # alternating strips: the largest number of clusters a tile can hold
+    assert ref["module"].tolist() == [0, 2, 3] and ref["last"].tolist() == [8999, 10999, n - 20001]
+    # alternating strips: the largest number of clusters a tile can hold (TILE / 2 starts per tile)
     alt = dict(full, adc=np.where(np.arange(n) % 2 == 0, 100, 0).astype(np.uint16))
     ref = check(alt, sp)
     assert len(ref["module"]) == (n + 1) // 2
-    # all bad, all quiet, one-strip modules
+    # all bad, all quiet
     check(dict(full, bad=np.ones(n, np.uint8)), sp)
     check(dict(full, adc=np.zeros(n, np.uint16)), sp)
-    one = dict(module_off=np.arange(4097, dtype=np.int32), adc=np.full(4096, 100, np.uint16), noise=np.full(4096, 4, np.float32),
-               bad=np.zeros(4096, np.uint8))
-    assert len(check(one, sp)["module"]) == 4096
+    # one-strip modules over more than two tiles: every tile meets thousands of modules (the global module_of path)
+    m1 = 2 * TILE + 77
+    one = dict(module_off=np.arange(m1 + 1, dtype=np.int32), adc=np.full(m1, 100, np.uint16), noise=np.full(m1, 4, np.float32),
+               bad=np.zeros(m1, np.uint8))
+    assert len(check(one, sp)["module"]) == m1
     # capacity smaller than the number found: the count is still exact (the records are then incomplete)
     check(alt, sp, capacity=100)
     # saturated counts: 16-bit ADC at full scale over a long cluster (sums beyond 32 bits)
