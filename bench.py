@@ -356,11 +356,13 @@ def run_fit(R, w, seed, workload=None):
         hits_p = R.pin(hits, ["layer_off", "x", "y", "z", "V"]); hits_p["n_events"] = hits["n_events"]
         seeds_p = R.pin(seeds, ["par", "cov", "q", "plan", "track_hits"])
 
+        out_p = B.alloc_fit_out_host(n)
+
         def e2e_step():
-            r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"], backward=backward)
+            r = ctx.fit_host(hits_p, seeds_p, seeds_p["plan"], seeds_p["track_hits"], backward=backward, out=out_p)
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
         rec["e2e"] = R.e2e(e2e_step, METRIC["fit"][1])
-        del hits_p, seeds_p
+        del hits_p, seeds_p, out_p
     if R.rank != 0:
         return rec
     # ---- roofline of the kernel (the step is one launch) ---------------------------------------------------------
@@ -451,8 +453,10 @@ def run_build(R, w, seed):
         hits_p = R.pin(hits, ["layer_off", "x", "y", "z", "V"]); hits_p["n_events"] = hits["n_events"]
         seeds_p = R.pin(seeds, list(seeds.keys()))
 
+        out_p = B.alloc_build_out_host(n, ctx.max_plan_len)
+
         def e2e_step():
-            r = ctx.build_host(hits_p, seeds_p, seeds_p["event"], seeds_p["hits"], seeds_p["plan"], dedup=dedup)
+            r = ctx.build_host(hits_p, seeds_p, seeds_p["event"], seeds_p["hits"], seeds_p["plan"], dedup=dedup, out=out_p)
             return float(nev), r["h2d_bytes"], r["d2h_bytes"]
         rec["e2e"] = R.e2e(e2e_step, METRIC["build"][1])
         del hits_p, seeds_p

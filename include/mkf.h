@@ -139,8 +139,14 @@ int mkf_fit_backward(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const s
 
 /* a12 / C9. seeds: n states at their first hit; seed_event[n]; seed_hits[3][n] global hit ids;
  * plan[n]. Each seed is first fitted through its own three hits, then followed through the rest of its plan.
+ * max_plan_len must be mkf_max_plan_len(ctx). ws: mkf_workspace_bytes(ctx, MKF_CALL_BUILD_TRACKS, n_events, n_hits,
+ * n_seeds) bytes (the seeds' fitted states, their processing order and the hit-list trellis live there).
  * out: state of the winning candidate; chi2, score, nhits (incl. seed hits), nmiss;
- * hit_ids[max_plan_len][n]: hit id | -1 missed layer | -2 layer not crossed; status. */
+ * hit_ids[max_plan_len][n]: hit id | -1 missed layer | -2 layer not crossed; status (a seed whose plan or event id
+ * is out of range, or whose hits are not on its plan in plan order, comes back unchanged with MKF_TRUNCATED).
+ * Limits: n_hits <= 2^28 - 2, at most 255 phi and 255 eta bins (MKF_UNSUPPORTED otherwise).
+ * Any scoring parameters are valid: the children of a layer are ranked by the total order U14 whatever the relation of
+ * score_hit, score_miss and chi2_cut. */
 int mkf_build_tracks(mkf_ctx*, const mkf_hits*, const mkf_hit_index*, const mkf_states* seeds,
             const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
             mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status,

@@ -245,6 +245,11 @@ class Context:
         ix = HitIndex(_dev(idx["bin_off"], torch.int32), _dev(idx["sorted_id"], torch.int32), _dev(idx["vmax"], torch.float32),
                       _dev(packed, torch.float32) if packed is not None else None)
         n = int(seeds["par"].shape[1])
+        if ws is None:                                          # scratch for the call (kept for the next one of the same size)
+            need = max(self.workspace_bytes(CALL_BUILD_TRACKS, int(hits["n_events"]), int(hits["x"].shape[0]), n), 256)
+            if getattr(self, "_build_ws", None) is None or self._build_ws.numel() < need:
+                self._build_ws = torch.empty(need, dtype=torch.uint8, device=seeds["par"].device)
+            ws = self._build_ws
         s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
         o = States(n, _dev(out["par"], torch.float32), _dev(out["cov"], torch.float32), _dev(seeds["q"], torch.int8))
         rc = self.L.mkf_build_tracks(self.h, C.byref(hs), C.byref(ix), C.byref(s), _dev(seed_event, torch.int32),
@@ -296,13 +301,13 @@ class Context:
         return out
 
     # ---- host-buffer entry points -------------------------------------------------------------------------
-    def fit_host(self, hits, seeds, plan, track_hits, backward=False):
-        """All arguments numpy / CPU tensors; returns dict of numpy arrays plus the bytes copied each way."""
+    def fit_host(self, hits, seeds, plan, track_hits, backward=False, out=None):
+        """All arguments numpy / CPU tensors; returns dict of numpy arrays plus the bytes copied each way.
+        out (optional): preallocated result arrays (alloc_fit_out_host; pinned memory keeps the copies asynchronous)."""
         f32, i32, i8 = np.float32, np.int32, np.int8
         hs = self.hits_struct(hits, _host, i32, f32)
         n = int(seeds["par"].shape[1])
-        out = dict(par=np.empty((6, n), f32), cov=np.empty((21, n), f32), chi2=np.empty(n, f32), nfit=np.empty(n, i32),
-                   status=np.empty(n, np.uint32))
+        out = dict(out) if out is not None else alloc_fit_out_host(n, pinned=False)
         s = States(n, _host(seeds["par"], f32), _host(seeds["cov"], f32), _host(seeds["q"], i8))
         o = States(n, out["par"].ctypes.data, out["cov"].ctypes.data, _host(seeds["q"], i8))
         h2d, d2h = C.c_longlong(0), C.c_longlong(0)
@@ -314,15 +319,14 @@ class Context:
         out["h2d_bytes"], out["d2h_bytes"] = h2d.value, d2h.value
         return out
 
-    def build_host(self, hits, seeds, seed_event, seed_hits, plan, dedup=False):
+    def build_host(self, hits, seeds, seed_event, seed_hits, plan, dedup=False, out=None):
         f32, i32, i8 = np.float32, np.int32, np.int8
         hs = self.hits_struct(hits, _host, i32, f32)
         n = int(seeds["par"].shape[1])
         mpl = self.max_plan_len
-        out = dict(par=np.empty((6, n), f32), cov=np.empty((21, n), f32), chi2=np.empty(n, f32), score=np.empty(n, f32),
-                   nhits=np.empty(n, i32), nmiss=np.empty(n, i32), hit_ids=np.empty((mpl, n), i32),
-                   status=np.empty(n, np.uint32))
-        keep = np.empty(n, np.uint8) if dedup else None
+        out = dict(out) if out is not None else alloc_build_out_host(n, mpl, pinned=False)
+        keep = out.pop("keep") if dedup else None
+        out.pop("keep", None)
         s = States(n, _host(seeds["par"], f32), _host(seeds["cov"], f32), _host(seeds["q"], i8))
         o = States(n, out["par"].ctypes.data, out["cov"].ctypes.data, _host(seeds["q"], i8))
         h2d, d2h = C.c_longlong(0), C.c_longlong(0)
@@ -374,6 +378,28 @@ def alloc_hit_index(ctx, n_events, n_hits, packed=True, device="cuda"):
                packed=torch.empty(n_hits * 12, dtype=torch.float32, device=device) if packed else None)
     ws = torch.empty(max(ctx.workspace_bytes(CALL_BUILD_HIT_INDEX, n_events, n_hits, 0), 256), dtype=torch.uint8, device=device)
     return out, ws
+
+
+def _host_array(shape, dtype, pinned):
+    if not pinned:
+        return np.empty(shape, dtype)
+    tdt = {np.float32: torch.float32, np.int32: torch.int32, np.uint8: torch.uint8}[dtype if dtype is not np.uint32 else np.int32]
+    a = torch.empty(shape, dtype=tdt).pin_memory().numpy()
+    return a.view(np.uint32) if dtype is np.uint32 else a
+
+
+def alloc_fit_out_host(n, pinned=True):
+    """Result arrays of fit_host in (pinned) host memory."""
+    f32, i32 = np.float32, np.int32
+    return dict(par=_host_array((6, n), f32, pinned), cov=_host_array((21, n), f32, pinned), chi2=_host_array(n, f32, pinned),
+                nfit=_host_array(n, i32, pinned), status=_host_array(n, np.uint32, pinned))
+
+
+def alloc_build_out_host(n, mpl, pinned=True):
+    f32, i32 = np.float32, np.int32
+    return dict(par=_host_array((6, n), f32, pinned), cov=_host_array((21, n), f32, pinned), chi2=_host_array(n, f32, pinned),
+                score=_host_array(n, f32, pinned), nhits=_host_array(n, i32, pinned), nmiss=_host_array(n, i32, pinned),
+                hit_ids=_host_array((mpl, n), i32, pinned), status=_host_array(n, np.uint32, pinned), keep=_host_array(n, np.uint8, pinned))
 
 
 def alloc_build_ws(ctx, n_events, n_hits, n_seeds, device="cuda"):

@@ -2,27 +2,53 @@
 // innermost layers, proceeding outwards", "only the best ranking ones are cloned at each layer (with
 // a per-seed cap)", PAPER.md:5 short-track preservation).
 //
-// Mapping: 8 lanes of a warp own one seed (4 seeds per warp); lane k holds live candidate k (rank order) with its
-// state and covariance in registers. Per layer: every live lane propagates its candidate (a2-a4), scans the
-// phi/eta bins of its window (a5) reading the packed hit records (16-byte positions first: most are rejected before
-// their covariance is read), keeps its own best MAX_CAND hits by chi2 in a sorted list in shared memory (a6); the group then picks the top max_cand children of the whole seed
-// with 8-lane shuffle tournaments under the total order U14 (a8), the winners fetch their parent's state with
-// shuffles and update it (a7). The hit lists are a trellis in shared memory (per step and slot: hit id and
-// parent slot), so cloning a candidate costs one 4-byte entry; the winner's list is read back at the end.
-// Stopped candidates are offered to the seed's `best short` slot (a9), whose state lives in the output arrays.
+// Three kernels:
+//   bs_seed_kernel   one thread per seed: the seed is fitted through its own three hits (U18b); its factored state
+//                    goes to the workspace, its key (event, plan, eta, phi) to a counting sort;
+//   (counting sort)  seeds ordered by that key, so that the seeds of a CTA walk the same layers and hit bins;
+//   mkf_build_kernel one CTA = NS seeds x 8 candidate slots, candidate states in SHARED memory; per plan step the CTA
+//                    goes through phases, each with every lane busy:
+//       P  propagate + material + window (a2-a5): the live candidates of all seeds, compacted, one thread each;
+//       S  chi2 scan (a6): the eta rows of all windows flattened into one list, SCAN_G lanes walk one row together
+//          (16-byte positions of a row are contiguous; survivors of the position test read their 32-byte covariance);
+//          accepted hits are appended to the candidate's short list;
+//       T  top-N per seed (a8): 8 lanes of a seed (lane = parent slot) offer the head of their sorted list or their
+//          miss / pass-through child, whichever ranks first under U14; shuffle tournaments pick max_cand children;
+//       U  update (a7): one thread per chosen child takes its parent's propagated state from shared memory, updates
+//          it with the hit, and writes the new live set back (non-finite children are dropped, R1).
+//   Hit lists are a trellis in the workspace (per step and slot: hit id and parent slot); the winner's list is read
+//   back at the end. Stopped candidates are offered to the seed's `best short` slot (a9), whose state lives in the
+//   output arrays.
 #include "mkf_ctx.h"
+#include "mkf_scan.cuh"
 
 using namespace mkf;
 
 namespace {
 
-constexpr int G = 8;                 // lanes per seed == MAX_CAND
-#ifndef MKF_BUILD_BLOCK
-#define MKF_BUILD_BLOCK 64
+constexpr int G = 8;                 // candidate slots per seed == MAX_CAND
+#ifndef MKF_BUILD_NS
+#define MKF_BUILD_NS 16
 #endif
-constexpr int BUILD_BLOCK = MKF_BUILD_BLOCK;     // 8 seeds per CTA (64 threads: 2193 events/s on configs[4]; 128: 2108, 32: 2178)
+constexpr int NS = MKF_BUILD_NS;     // seeds per CTA
+constexpr int SL = NS * G;           // candidate slots per CTA
+constexpr int BT = SL;               // threads per CTA: one per slot
+constexpr int LC = 8;                // accepted hits kept per candidate and layer (a seed keeps at most MAX_CAND children)
+#ifndef MKF_BUILD_SCAN_G
+#define MKF_BUILD_SCAN_G 4
+#endif
+constexpr int SCAN_G = MKF_BUILD_SCAN_G;   // lanes that walk one eta row of a window together
 constexpr int HIT_NONE = 0x7fffffff; // "hit id" of miss / pass-through children in the order U14
-static_assert(G == MAX_CAND, "one lane per candidate slot");
+static_assert(G == MAX_CAND, "one slot per candidate");
+static_assert(BT % 32 == 0 && BT <= 1024, "CTA size");
+
+// fields of a candidate state in shared memory, [field][slot]
+enum { F_X, F_Y, F_Z, F_XL, F_YL, F_ZL, F_IPT, F_PHI, F_TH, F_CPH, F_SPH, F_CTH, F_STH, F_FK, F_FCB, F_FSB, F_U0,
+       F_D0 = F_U0 + 10, NF = F_D0 + 5 };
+// per-seed record of the seed kernel in the workspace, [field][seed]
+enum { W_CHI2 = NF, W_NH, W_LAST, W_STAT, W_OK, NW };
+
+enum : int { FL_SCAN = 1, FL_PASS = 2, FL_MISS = 4, FL_OFFER = 8, FL_OFFER_MISS = 16 };
 
 struct BuildArgs {
   HitsDev hits;
@@ -30,6 +56,28 @@ struct BuildArgs {
   int n; const float* par; const float* cov; const signed char* q; const int* seed_event; const int* seed_hits;
   const signed char* plan; int max_plan_len;
   float* par_out; float* cov_out; float* chi2; float* score; int* nhits; int* nmiss; int* hit_ids; unsigned* status;
+  float* wseed;             // [NW][n]   seed kernel -> build kernel
+  unsigned* trellis;        // [n][mpl][G]
+  const int* order;         // [n] seed processed at position k
+  unsigned* key; unsigned* bucket; int n_buckets;      // counting sort of the seeds
+  unsigned long long* counters;
+};
+
+struct Smem {
+  float A[NF][SL];          // live candidates as they stand before this layer
+  float B[NF][SL];          // the same candidates propagated to this layer (material applied)
+  float chi2[SL]; int cnt[SL];                     // cnt = nhits | nmiss << 8 | consec << 16
+  float tt[SL], tz[SL], zz[SL], lim1[SL], lim2[SL];
+  int wrow[SL], wphi[SL];   // window: e0 | n_rows << 8 ; w0 | wn << 8
+  int flag[SL]; unsigned ostat[SL];
+  int rowpre[SL + 1];
+  int lcount[SL];
+  unsigned long long lkey[LC][SL];                 // chi2 bits << 32 | hit id: ascending = the order U14 within a parent
+  int lt[LC][SL];                                  // position of the hit in the packed arrays
+  int plist[SL]; int nP;
+  int wsum[BT / 32];
+  int n_live[NS], p0[NS], plen[NS], ev[NS], last[NS], seed[NS];
+  float aq[NS];
 };
 
 __device__ __forceinline__ float score_of(const ParamsDev& p, int nh, int nm, float chi2) {
@@ -44,10 +92,25 @@ __device__ __forceinline__ bool before(float sa, float ca, int pa, int ha, float
   return ha < hb;
 }
 
-__device__ __forceinline__ void load_packed(Hit& H, int& id, const float4 a, const float4* __restrict__ cov) {
-  const float4 b = __ldg(cov), c = __ldg(cov + 1);
-  H.x = a.x; H.y = a.y; H.z = a.z; id = __float_as_int(a.w);
-  H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = c.x; H.v[5] = c.y;
+__device__ __forceinline__ void st_state(float (*M)[SL], int slot, const KState& S) {
+  M[F_X][slot] = S.x; M[F_Y][slot] = S.y; M[F_Z][slot] = S.z; M[F_XL][slot] = S.xl; M[F_YL][slot] = S.yl; M[F_ZL][slot] = S.zl;
+  M[F_IPT][slot] = S.ipt; M[F_PHI][slot] = S.phi; M[F_TH][slot] = S.th;
+  M[F_CPH][slot] = S.cph; M[F_SPH][slot] = S.sph; M[F_CTH][slot] = S.cth; M[F_STH][slot] = S.sth;
+  M[F_FK][slot] = __int_as_float(S.f.kind); M[F_FCB][slot] = S.f.cb; M[F_FSB][slot] = S.f.sb;
+#pragma unroll
+  for (int k = 0; k < 10; k++) M[F_U0 + k][slot] = S.u[k];
+#pragma unroll
+  for (int k = 0; k < 5; k++) M[F_D0 + k][slot] = S.d[k];
+}
+__device__ __forceinline__ void ld_state(const float (*M)[SL], int slot, KState& S) {
+  S.x = M[F_X][slot]; S.y = M[F_Y][slot]; S.z = M[F_Z][slot]; S.xl = M[F_XL][slot]; S.yl = M[F_YL][slot]; S.zl = M[F_ZL][slot];
+  S.ipt = M[F_IPT][slot]; S.phi = M[F_PHI][slot]; S.th = M[F_TH][slot];
+  S.cph = M[F_CPH][slot]; S.sph = M[F_SPH][slot]; S.cth = M[F_CTH][slot]; S.sth = M[F_STH][slot];
+  S.f.kind = __float_as_int(M[F_FK][slot]); S.f.cb = M[F_FCB][slot]; S.f.sb = M[F_FSB][slot];
+#pragma unroll
+  for (int k = 0; k < 10; k++) S.u[k] = M[F_U0 + k][slot];
+#pragma unroll
+  for (int k = 0; k < 5; k++) S.d[k] = M[F_D0 + k][slot];
 }
 
 // asinh to ~1e-6 absolute for |x| up to e^4 (one lg2.approx, one rsqrt-based sqrt): the eta edges of the window carry
@@ -95,177 +158,345 @@ __device__ __forceinline__ void window(const GeomDev& g, const LayerDev& L, floa
   p0 = a < 0 ? a + g.n_phi : (a >= g.n_phi ? a - g.n_phi : a); np = cnt;          // dphi < pi: a in (-n_phi, 2 n_phi)
 }
 
-#define SHFL_STATE(S, src, gm)                                           \
-  do {                                                                   \
-    S.x = __shfl_sync(gm, S.x, src); S.y = __shfl_sync(gm, S.y, src); S.z = __shfl_sync(gm, S.z, src);       \
-    S.xl = __shfl_sync(gm, S.xl, src); S.yl = __shfl_sync(gm, S.yl, src); S.zl = __shfl_sync(gm, S.zl, src); \
-    S.ipt = __shfl_sync(gm, S.ipt, src); S.phi = __shfl_sync(gm, S.phi, src); S.th = __shfl_sync(gm, S.th, src); \
-    S.cph = __shfl_sync(gm, S.cph, src); S.sph = __shfl_sync(gm, S.sph, src);                                 \
-    S.cth = __shfl_sync(gm, S.cth, src); S.sth = __shfl_sync(gm, S.sth, src);                                 \
-    S.f.kind = __shfl_sync(gm, S.f.kind, src); S.f.cb = __shfl_sync(gm, S.f.cb, src); S.f.sb = __shfl_sync(gm, S.f.sb, src); \
-    _Pragma("unroll") for (int k_ = 0; k_ < 10; k_++) S.u[k_] = __shfl_sync(gm, S.u[k_], src);             \
-    _Pragma("unroll") for (int k_ = 0; k_ < 5; k_++) S.d[k_] = __shfl_sync(gm, S.d[k_], src);              \
-  } while (0)
-
-#ifndef MKF_BUILD_MIN_BLOCKS
-#define MKF_BUILD_MIN_BLOCKS 16
-#endif
-__global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
-                                                                const __grid_constant__ ParamsDev p,
-                                                                const __grid_constant__ BuildArgs a) {
-  extern __shared__ unsigned trellis_all[];                  // [seed in CTA][step][slot]
-  const int lane = threadIdx.x & 31;
-  const int sub = lane & (G - 1);                            // candidate slot
-  const int gbase = lane & ~(G - 1);
-  const unsigned gm = 0xffu << gbase;
-  const int seed_in_cta = threadIdx.x / G;
-  const int i = blockIdx.x * (BUILD_BLOCK / G) + seed_in_cta;
-  const bool have_seed = i < a.n;
+// ---- seed phase -----------------------------------------------------------------------------------------------
+// One thread per seed: fit through its own three hits (U18b). Writes the factored state and the bookkeeping to the
+// workspace, the fallback output (the seed candidate itself, C9 last line) to the output arrays, the seed's hits to
+// slot 0 of its trellis, and its sort key.
+__global__ void __launch_bounds__(128) bs_seed_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ ParamsDev p,
+                                                      const __grid_constant__ BuildArgs a) {
+  const int i = blockIdx.x * 128 + threadIdx.x;
+  if (i >= a.n) return;
   const size_t n = (size_t)a.n;
   const int mpl = a.max_plan_len;
-  unsigned* trellis = trellis_all + (size_t)seed_in_cta * mpl * G;
-  // per-thread list of accepted hits of the current layer, [k][thread] (bank-conflict free): chi2, hit id
-  float* hc2 = reinterpret_cast<float*>(trellis_all + (size_t)(BUILD_BLOCK / G) * mpl * G) + threadIdx.x;
-  int* hid = reinterpret_cast<int*>(hc2 - threadIdx.x + G * BUILD_BLOCK) + threadIdx.x;
-  const int nb = g.n_phi * g.n_eta;
-
-  // ---- seed phase: slot 0 fits the seed through its own three hits (U18b) --------------------------------
+  unsigned* tr = a.trellis + (size_t)i * mpl * G;
+  const int pl = a.plan[i], ev = a.seed_event[i];
+  float chi2 = 0.f; int nh = 0, last_step = -1; unsigned stat = 0; bool ok = true;
   KState S;
-  float chi2 = 0.f; int nh = 0, nm = 0, consec = 0; unsigned stat = 0;
-  bool live = false;
-  int p0 = 0, plen = 0, ev = 0, last_step = -1;
-  float aq = 0.f;
-  bool seed_ok = false;
-  if (have_seed) {
-    const int pl = a.plan[i];
+  load_params(S, a.par, n, (size_t)i);
+  bool has_ud = false;
+  int p0 = 0, plen = 0;
+  if ((unsigned)pl >= (unsigned)g.n_plans || (unsigned)ev >= (unsigned)a.hits.n_events) { stat |= ST_TRUNC; ok = false; }
+  else {
     p0 = g.plan_off[pl];
     plen = min(g.plan_off[pl + 1] - p0, mpl);
-    ev = a.seed_event[i];
-    aq = -(float)a.q[i] * KAPPA * g.bz;
-    for (int s = sub; s < mpl; s += G) trellis[s * G + 0] = 0u;          // hit code 0 == -2 (not crossed), parent 0
-  }
-  __syncwarp(gm);
-  if (have_seed && sub == 0) {
-    load_params(S, a.par, n, (size_t)i);
-    bool has_ud = false;
+    const float aq = -(float)a.q[i] * KAPPA * g.bz;
     const int* loff = a.hits.layer_off + (size_t)ev * (g.n_layers + 1);
-    seed_ok = true;
-    for (int k = 0; k < 3 && seed_ok; k++) {
+    for (int k = 0; k < 3 && ok; k++) {
       const int hid = a.seed_hits[(size_t)k * n + i];
       int lay = -1;
       for (int l = 0; l < g.n_layers; l++) if (hid >= loff[l] && hid < loff[l + 1]) { lay = l; break; }
       int step = -1;
-      for (int s = last_step + 1; s < plen; s++) if ((int)g.plan_layers[p0 + s] == lay) { step = s; break; }
-      if (step < 0) { stat |= ST_TRUNC; seed_ok = false; break; }
+      if (lay >= 0) for (int s = last_step + 1; s < plen; s++) if ((int)g.plan_layers[p0 + s] == lay) { step = s; break; }
+      if (step < 0) { stat |= ST_TRUNC; ok = false; break; }
       const LayerDev L = g.layers[lay];
       const unsigned rc = step_to_layer(S, !has_ud, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
-      if (rc) { stat |= rc; seed_ok = false; break; }
+      if (rc) { stat |= rc; ok = false; break; }
       has_ud = true;
       Hit H; load_hit(H, a.hits, hid);
       SInv o; float c2;
       hit_to_local(S, H, o);
-      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; seed_ok = false; break; }
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
+      for (int s = last_step + 1; s < step; s++) tr[s * G] = 0u;            // hit code 0 == -2 (not crossed), parent 0
       chi2 += c2; nh++; last_step = step;
-      trellis[step * G + 0] = (unsigned)(hid + 2);
+      tr[step * G] = (unsigned)(hid + 2);
     }
-    // fallback output: the seed candidate itself (C9 last line); overwritten by best_short / the final winner
-    if (has_ud) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
-    else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
-    live = seed_ok;
   }
-  seed_ok = __shfl_sync(gm, (int)seed_ok, gbase) != 0;
-  last_step = __shfl_sync(gm, last_step, gbase);
-  const float seed_chi2 = __shfl_sync(gm, chi2, gbase);
-  const int seed_nh = __shfl_sync(gm, nh, gbase);
-  const unsigned seed_stat = __shfl_sync(gm, stat, gbase);
+  if (has_ud) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+  else copy_seed(a.par, a.cov, a.par_out, a.cov_out, n, (size_t)i);
+  float* w = a.wseed + i;
+  w[(size_t)F_X * n] = S.x; w[(size_t)F_Y * n] = S.y; w[(size_t)F_Z * n] = S.z;
+  w[(size_t)F_XL * n] = S.xl; w[(size_t)F_YL * n] = S.yl; w[(size_t)F_ZL * n] = S.zl;
+  w[(size_t)F_IPT * n] = S.ipt; w[(size_t)F_PHI * n] = S.phi; w[(size_t)F_TH * n] = S.th;
+  w[(size_t)F_CPH * n] = S.cph; w[(size_t)F_SPH * n] = S.sph; w[(size_t)F_CTH * n] = S.cth; w[(size_t)F_STH * n] = S.sth;
+  w[(size_t)F_FK * n] = __int_as_float(S.f.kind); w[(size_t)F_FCB * n] = S.f.cb; w[(size_t)F_FSB * n] = S.f.sb;
+#pragma unroll
+  for (int k = 0; k < 10; k++) w[(size_t)(F_U0 + k) * n] = S.u[k];
+#pragma unroll
+  for (int k = 0; k < 5; k++) w[(size_t)(F_D0 + k) * n] = S.d[k];
+  w[(size_t)W_CHI2 * n] = chi2; w[(size_t)W_NH * n] = __int_as_float(nh); w[(size_t)W_LAST * n] = __int_as_float(last_step);
+  w[(size_t)W_STAT * n] = __int_as_float((int)stat); w[(size_t)W_OK * n] = __int_as_float(ok ? 1 : 0);
+  // sort key: seeds that will walk the same layers and bins next to each other (any order gives the same tracks)
+  const float x = S.x + S.xl, y = S.y + S.yl;
+  int ip = (int)((atan2f(y, x) + PI_F) * (16.f / (2.f * PI_F))); ip = min(max(ip, 0), 15);
+  int ie = (int)((S.cth + 1.f) * 8.f); ie = min(max(ie, 0), 15);          // cos(theta) is monotone in eta
+  const int pe = ok ? ((ev * g.n_plans + pl) * 16 + ie) * 16 + ip : a.n_buckets - 1;       // failed seeds last
+  a.key[i] = (unsigned)pe;
+  atomicAdd(&a.bucket[pe], 1u);
+}
 
-  // best short candidate of the seed (replicated in every lane of the group)
-  bool bs_have = false; float bs_score = 0.f, bs_chi2 = 0.f; int bs_nh = 0, bs_nm = 0, bs_step = 0, bs_parent = 0, bs_last = -2;
-  unsigned bs_stat = 0;
-  int t_last = last_step;                                    // last step at which the live set was rewritten
-  int n_live = seed_ok ? 1 : 0;
+__global__ void __launch_bounds__(256) bs_order_kernel(int n, const unsigned* __restrict__ key, unsigned* cursor, int* order) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  order[atomicAdd(&cursor[key[i]], 1u)] = i;
+}
 
-  for (int s = 0; s < mpl; s++) {
-    const bool active = have_seed && seed_ok && s > last_step && s < plen && n_live > 0;   // uniform in the group
-    if (!active) continue;
-    const int lay = g.plan_layers[p0 + s];
-    const LayerDev L = g.layers[lay];
-    const size_t seg = (size_t)ev * g.n_layers + lay;
+// ---- the chi2 of one hit against one propagated candidate; appends accepted hits to the candidate's list ---------
+struct ScanCand { float x, y, z, xl, yl, zl, cb, sb, tt, tz, zz, lim1, lim2; int kind; };
 
-    // ---- each live lane: propagate, scan its window, keep its own best hits ------------------------------
-    int n_hitc = 0, head = 0;             // accepted hits in hc2/hid (sorted), next one to offer
-    bool miss_avail = false, pass_avail = false;
-    bool offer = false; int offer_phase = 0; float offer_score = 0.f; int offer_nm = 0;
-    if (live) {
-      const unsigned rc = step_to_layer(S, false, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, true);
-      if (rc & (ST_UNREACH | ST_SKIP_ACC)) {
-        pass_avail = true;                                   // silent skip: competes unchanged (C9.1)
-      } else if (rc) {                                       // grazing / energy exhausted: the candidate stops
-        stat |= rc;
-        if (nh >= p.min_hits_keep) { offer = true; offer_phase = 0; offer_nm = nm; offer_score = score_of(p, nh, nm, chi2); }
-      } else {
-        float tt, tz, zz;
-        cov_aa(S, tt, tz, zz);
-        int e0, e1, w0, wn;
-        window(g, L, p.chi2_cut, S, tt, zz, a.vmax[2 * seg], a.vmax[2 * seg + 1], e0, e1, w0, wn);
-        const float lim1 = p.chi2_cut * (tt + a.vmax[2 * seg]) * 1.0001f;
-        const float lim2 = p.chi2_cut * (zz + (L.kind == 0 ? a.vmax[2 * seg + 1] : a.vmax[2 * seg])) * 1.0001f;
-        const unsigned* boff = a.bin_off + seg * (size_t)nb;
-        for (int ie = e0; ie <= e1; ie++) {
-          const unsigned* row = boff + ie * g.n_phi;
-#pragma unroll 1
-          for (int part = 0; part < 2; part++) {
-            unsigned tb, te;
-            if (part == 0) { tb = row[w0]; te = row[min(w0 + wn, g.n_phi)]; }
-            else { if (w0 + wn <= g.n_phi) break; tb = row[0]; te = row[w0 + wn - g.n_phi]; }
-            float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (a.packed && tb < te) qn = __ldg(a.packed + tb);
-            for (unsigned t = tb; t < te; t++) {
-              Hit H; int id;
-              if (a.packed) {
-                // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11),
-                // so most hits of the padded bins are rejected before their covariance is read; the next record's
-                // position is already in flight
-                const float4 q0 = qn;
-                if (t + 1 < te) qn = __ldg(a.packed + t + 1);
-                const float rx = (q0.x - S.x) - S.xl, ry = (q0.y - S.y) - S.yl, rz = (q0.z - S.z) - S.zl;
-                const float r1 = S.f.kind == 0 ? S.f.cb * ry - S.f.sb * rx : rx, r2 = S.f.kind == 0 ? rz : ry;
-                if (r1 * r1 > lim1 || r2 * r2 > lim2) continue;
-                load_packed(H, id, q0, a.packed + (size_t)a.hits.n_hits + (size_t)2 * t);
-              } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
-              SInv o; float c2;
-              if (!chi2_local(S, tt, tz, zz, H, o, c2)) continue;
-              if (c2 < p.chi2_cut) {
-                // kept sorted by (chi2, id) in shared memory: lists are short (1-2 entries on average), so the
-                // insertion is a handful of divergent instructions and no register array is needed
-                int k = n_hitc;
-                if (n_hitc == G) {
-                  const float wv = hc2[(G - 1) * BUILD_BLOCK]; const int wi = hid[(G - 1) * BUILD_BLOCK];
-                  k = (c2 < wv || (c2 == wv && id < wi)) ? G - 1 : -1;
-                } else n_hitc++;
-                if (k >= 0) {
-                  while (k > 0) {
-                    const float pv = hc2[(k - 1) * BUILD_BLOCK]; const int pi = hid[(k - 1) * BUILD_BLOCK];
-                    if (!(c2 < pv || (c2 == pv && id < pi))) break;
-                    hc2[k * BUILD_BLOCK] = pv; hid[k * BUILD_BLOCK] = pi; k--;
-                  }
-                  hc2[k * BUILD_BLOCK] = c2; hid[k * BUILD_BLOCK] = id;
-                }
-              }
-            }
-          }
-        }
-        // miss child (C9.5): stopped if it reaches the consecutive-miss limit
-        if (consec + 1 >= p.max_consec_miss) {
-          if (nh >= p.min_hits_keep) { offer = true; offer_phase = 1; offer_nm = nm + 1; offer_score = score_of(p, nh, nm + 1, chi2); }
-        } else miss_avail = true;
+template <bool COUNT>
+__device__ __forceinline__ void scan_range(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const ScanCand& c,
+                                           unsigned tb, unsigned te, int lane, int stride, unsigned& n_pos, unsigned& n_c2, unsigned& n_acc) {
+  KState S;                                                        // only what hit_to_local / chi2_local read
+  S.x = c.x; S.y = c.y; S.z = c.z; S.xl = c.xl; S.yl = c.yl; S.zl = c.zl; S.f.kind = c.kind; S.f.cb = c.cb; S.f.sb = c.sb;
+  for (unsigned t = tb + lane; t < te; t += stride) {
+    Hit H; int id;
+    if (COUNT) n_pos++;
+    if (a.packed) {
+      // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11), so most
+      // hits of the padded bins are rejected before their covariance is read
+      const float4 q0 = __ldg(a.packed + t);
+      const float rx = (q0.x - c.x) - c.xl, ry = (q0.y - c.y) - c.yl, rz = (q0.z - c.z) - c.zl;
+      const float r1 = c.kind == 0 ? c.cb * ry - c.sb * rx : rx, r2 = c.kind == 0 ? rz : ry;
+      if (r1 * r1 > c.lim1 || r2 * r2 > c.lim2) continue;
+      const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
+      const float4 b = __ldg(cv), d = __ldg(cv + 1);
+      H.x = q0.x; H.y = q0.y; H.z = q0.z; id = __float_as_int(q0.w);
+      H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
+    } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
+    if (COUNT) n_c2++;
+    SInv o; float c2;
+    if (!chi2_local(S, c.tt, c.tz, c.zz, H, o, c2)) continue;
+    if (c2 < p.chi2_cut) {
+      if (COUNT) n_acc++;
+      const int k = atomicAdd(&sm.lcount[slot], 1);
+      if (k < LC) {
+        sm.lkey[k][slot] = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
+        sm.lt[k][slot] = (int)t;
       }
     }
+  }
+}
 
-    // ---- offers to best_short (C9.6): best offer of this layer, then strict comparison with the holder ------
+__device__ __forceinline__ void load_scan_cand(const Smem& sm, int slot, ScanCand& c) {
+  c.x = sm.B[F_X][slot]; c.y = sm.B[F_Y][slot]; c.z = sm.B[F_Z][slot];
+  c.xl = sm.B[F_XL][slot]; c.yl = sm.B[F_YL][slot]; c.zl = sm.B[F_ZL][slot];
+  c.kind = __float_as_int(sm.B[F_FK][slot]); c.cb = sm.B[F_FCB][slot]; c.sb = sm.B[F_FSB][slot];
+  c.tt = sm.tt[slot]; c.tz = sm.tz[slot]; c.zz = sm.zz[slot]; c.lim1 = sm.lim1[slot]; c.lim2 = sm.lim2[slot];
+}
+
+// More than LC hits of a window passed the cut (a crowded region): the owner of the slot walks its window again and
+// keeps the LC best under (chi2, id). Rare; not inlined so that it stays out of the hot loop's instruction stream.
+__device__ __noinline__ void rescan_slot(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const unsigned* boff, int n_phi) {
+  ScanCand c; load_scan_cand(sm, slot, c);
+  KState S;
+  S.x = c.x; S.y = c.y; S.z = c.z; S.xl = c.xl; S.yl = c.yl; S.zl = c.zl; S.f.kind = c.kind; S.f.cb = c.cb; S.f.sb = c.sb;
+  const int e0 = sm.wrow[slot] & 0xff, nr = sm.wrow[slot] >> 8, w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
+  int cntk = 0;
+  for (int ie = e0; ie < e0 + nr; ie++) {
+    const unsigned* row = boff + ie * n_phi;
+    for (int part = 0; part < 2; part++) {
+      unsigned tb, te;
+      if (part == 0) { tb = row[w0]; te = row[min(w0 + wn, n_phi)]; }
+      else { if (w0 + wn <= n_phi) break; tb = row[0]; te = row[w0 + wn - n_phi]; }
+      for (unsigned t = tb; t < te; t++) {
+        Hit H; int id;
+        if (a.packed) {
+          const float4 q0 = __ldg(a.packed + t);
+          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
+          const float4 b = __ldg(cv), d = __ldg(cv + 1);
+          H.x = q0.x; H.y = q0.y; H.z = q0.z; id = __float_as_int(q0.w);
+          H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
+        } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
+        SInv o; float c2;
+        if (!chi2_local(S, c.tt, c.tz, c.zz, H, o, c2)) continue;
+        if (!(c2 < p.chi2_cut)) continue;
+        const unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
+        int k = cntk;
+        if (cntk == LC) { if (key < sm.lkey[LC - 1][slot]) k = LC - 1; else continue; }
+        else cntk++;
+        while (k > 0 && key < sm.lkey[k - 1][slot]) { sm.lkey[k][slot] = sm.lkey[k - 1][slot]; sm.lt[k][slot] = sm.lt[k - 1][slot]; k--; }
+        sm.lkey[k][slot] = key; sm.lt[k][slot] = (int)t;
+      }
+    }
+  }
+  sm.lcount[slot] = cntk;
+}
+
+#ifndef MKF_BUILD_MIN_BLOCKS
+#define MKF_BUILD_MIN_BLOCKS 4
+#endif
+template <bool COUNT>
+__global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
+                                                                const __grid_constant__ ParamsDev p,
+                                                                const __grid_constant__ BuildArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int sl = tid >> 3;                                   // seed of this thread's slot (phases T, U)
+  const int sub = tid & (G - 1);                             // candidate slot inside the seed
+  const int gbase = lane & ~(G - 1);
+  const unsigned gm = 0xffu << gbase;
+  const size_t n = (size_t)a.n;
+  const int mpl = a.max_plan_len;
+  const int nb = g.n_phi * g.n_eta;
+  unsigned n_steps = 0, n_pos = 0, n_c2 = 0, n_acc = 0, n_upd = 0;        // COUNT only
+
+  // ---- load the seeds of this CTA ------------------------------------------------------------------------------
+  const int pos = blockIdx.x * NS + sl;
+  const int i = pos < a.n ? a.order[pos] : -1;                // the seed of this thread's group
+  float seed_chi2 = 0.f; int seed_nh = 0, seed_last = -1; unsigned seed_stat = 0; bool seed_ok = false;
+  if (i >= 0) {
+    const float* w = a.wseed + i;
+    seed_chi2 = w[(size_t)W_CHI2 * n]; seed_nh = __float_as_int(w[(size_t)W_NH * n]); seed_last = __float_as_int(w[(size_t)W_LAST * n]);
+    seed_stat = (unsigned)__float_as_int(w[(size_t)W_STAT * n]); seed_ok = __float_as_int(w[(size_t)W_OK * n]) != 0;
+    if (sub == 0) {
+      int p0 = 0, plen = 0;
+      if (seed_ok) { const int pl = a.plan[i]; p0 = g.plan_off[pl]; plen = min(g.plan_off[pl + 1] - p0, mpl); }
+      sm.p0[sl] = p0; sm.plen[sl] = plen; sm.ev[sl] = seed_ok ? a.seed_event[i] : 0; sm.last[sl] = seed_last; sm.seed[sl] = i;
+      sm.aq[sl] = -(float)a.q[i] * KAPPA * g.bz;
+      sm.n_live[sl] = seed_ok ? 1 : 0;
+      if (seed_ok) {
+#pragma unroll
+        for (int k = 0; k < NF; k++) sm.A[k][tid] = w[(size_t)k * n];
+        sm.chi2[tid] = seed_chi2; sm.cnt[tid] = seed_nh;
+      }
+    }
+  } else if (sub == 0) { sm.n_live[sl] = 0; sm.plen[sl] = 0; sm.last[sl] = -1; sm.seed[sl] = -1; sm.p0[sl] = 0; sm.ev[sl] = 0; sm.aq[sl] = 0.f; }
+  unsigned* trellis = a.trellis + (size_t)(i >= 0 ? i : 0) * mpl * G;
+
+  // best short candidate of the seed (replicated in the 8 lanes of the group)
+  bool bs_have = false; float bs_score = 0.f, bs_chi2 = 0.f; int bs_nh = 0, bs_nm = 0, bs_step = 0, bs_parent = 0, bs_last = -2;
+  unsigned bs_stat = 0;
+  int t_last = seed_last;                                    // last step at which the live set was rewritten
+  __syncthreads();
+
+  for (int s = 0; s < mpl; s++) {
+    // ---- which slots propagate at this step: compacted list over the CTA ------------------------------------------
+    const int nl_prev = sm.n_live[sl];
+    const bool seed_act = i >= 0 && seed_ok && s > seed_last && s < sm.plen[sl] && nl_prev > 0;     // uniform in the group
+    const bool act = seed_act && sub < nl_prev;
     {
-      float os = offer ? offer_score : -INFINITY, oc = chi2; int ok = offer_phase * G + sub;
-      int ol = sub;
+      const unsigned bal = __ballot_sync(0xffffffffu, act);
+      if (lane == 0) sm.wsum[warp] = __popc(bal);
+      sm.flag[tid] = 0; sm.lcount[tid] = 0; sm.rowpre[tid] = 0;
+      __syncthreads();
+      int base = 0, tot = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < BT / 32; w2++) { const int c = sm.wsum[w2]; if (w2 < warp) base += c; tot += c; }
+      if (tot == 0) {                                         // no seed of this CTA is active at this step
+        __syncthreads();
+        continue;
+      }
+      if (act) sm.plist[base + __popc(bal & ((1u << lane) - 1u))] = tid;
+      if (tid == 0) sm.nP = tot;
+      __syncthreads();
+    }
+
+    // ---- phase P: propagate, material, window ---------------------------------------------------------------------
+    if (tid < sm.nP) {
+      const int slot = sm.plist[tid];
+      const int ssl = slot >> 3;
+      const int lay = g.plan_layers[sm.p0[ssl] + s];
+      const LayerDev L = g.layers[lay];
+      KState S; ld_state(sm.A, slot, S);
+      Prop P;
+      const unsigned rc = propagate_geom(S, L, sm.aq[ssl], p.graze_cos_min, p.material_flags, true, P);
+      const int cn = sm.cnt[slot];
+      const int nh = cn & 0xff, nm = (cn >> 8) & 0xff, consec = cn >> 16;
+      if (rc & (ST_UNREACH | ST_SKIP_ACC)) {
+        sm.flag[slot] = FL_PASS;                              // silent skip: competes unchanged (C9.1)
+      } else if (rc) {                                        // grazing / energy exhausted: the candidate stops
+        if (nh >= p.min_hits_keep) { sm.flag[slot] = FL_OFFER; sm.ostat[slot] = rc; }
+      } else {
+        commit_step(S, P, p.material_flags);
+        if (COUNT) n_steps++;
+        st_state(sm.B, slot, S);
+        float tt, tz, zz;
+        cov_aa(S, tt, tz, zz);
+        const size_t seg = (size_t)sm.ev[ssl] * g.n_layers + lay;
+        const float vxy = a.vmax[2 * seg], vzz = a.vmax[2 * seg + 1];
+        int e0, e1, w0, wn;
+        window(g, L, p.chi2_cut, S, tt, zz, vxy, vzz, e0, e1, w0, wn);
+        sm.tt[slot] = tt; sm.tz[slot] = tz; sm.zz[slot] = zz;
+        sm.lim1[slot] = p.chi2_cut * (tt + vxy) * 1.0001f;
+        sm.lim2[slot] = p.chi2_cut * (zz + (L.kind == 0 ? vzz : vxy)) * 1.0001f;
+        sm.wrow[slot] = e0 | ((e1 - e0 + 1) << 8); sm.wphi[slot] = w0 | (wn << 8);
+        sm.rowpre[slot] = e1 - e0 + 1;
+        int fl = FL_SCAN;
+        // miss child (C9.5): stopped if it reaches the consecutive-miss limit
+        if (consec + 1 >= p.max_consec_miss) { if (nh >= p.min_hits_keep) { fl |= FL_OFFER_MISS; sm.ostat[slot] = 0; } }
+        else fl |= FL_MISS;
+        sm.flag[slot] = fl;
+      }
+    }
+    __syncthreads();
+
+    // ---- exclusive prefix of the windows' row counts: the rows of all candidates as one list -----------------------
+    {
+      const int v = sm.rowpre[tid];
+      int inc = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
+      if (lane == 31) sm.wsum[warp] = inc;
+      __syncthreads();
+      int base = 0, tot = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < BT / 32; w2++) { const int c = sm.wsum[w2]; if (w2 < warp) base += c; tot += c; }
+      sm.rowpre[tid] = base + inc - v;
+      if (tid == 0) sm.rowpre[SL] = tot;
+      __syncthreads();
+    }
+
+    // ---- phase S: SCAN_G lanes per (candidate, eta row) --------------------------------------------------------------
+    {
+      const int NR = sm.rowpre[SL];
+      const int gl = tid & (SCAN_G - 1);
+      for (int j = tid / SCAN_G; j < NR; j += BT / SCAN_G) {
+        int lo = 0, hi = SL;
+#pragma unroll
+        for (int it = 0; it < 8; it++) {                      // last slot with rowpre[slot] <= j  (SL <= 256)
+          const int mid = (lo + hi) >> 1;
+          if (hi - lo > 1) { if (sm.rowpre[mid] <= j) lo = mid; else hi = mid; }
+        }
+        const int slot = lo;
+        const int ssl = slot >> 3;
+        ScanCand c; load_scan_cand(sm, slot, c);
+        const int ie = (sm.wrow[slot] & 0xff) + (j - sm.rowpre[slot]);
+        const int w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
+        const int lay = g.plan_layers[sm.p0[ssl] + s];
+        const unsigned* row = a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb + ie * g.n_phi;
+        const unsigned tb0 = __ldg(row + w0), te0 = __ldg(row + min(w0 + wn, g.n_phi));
+        unsigned tb1 = 0, te1 = 0;
+        if (w0 + wn > g.n_phi) { tb1 = __ldg(row); te1 = __ldg(row + w0 + wn - g.n_phi); }
+        scan_range<COUNT>(a, p, sm, slot, c, tb0, te0, gl, SCAN_G, n_pos, n_c2, n_acc);
+        if (te1 > tb1) scan_range<COUNT>(a, p, sm, slot, c, tb1, te1, gl, SCAN_G, n_pos, n_c2, n_acc);
+      }
+    }
+    __syncthreads();
+
+    // ---- phase L: each slot orders its accepted hits by (chi2, id) ---------------------------------------------------
+    const int fl = sm.flag[tid];
+    int n_hitc = 0;
+    if (fl & FL_SCAN) {
+      n_hitc = sm.lcount[tid];
+      if (n_hitc > LC) {
+        const int ssl = tid >> 3;
+        const int lay = g.plan_layers[sm.p0[ssl] + s];
+        rescan_slot(a, p, sm, tid, a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb, g.n_phi);
+        n_hitc = sm.lcount[tid];
+      } else {
+        for (int k = 1; k < n_hitc; k++) {
+          const unsigned long long key = sm.lkey[k][tid]; const int tk = sm.lt[k][tid];
+          int m = k;
+          while (m > 0 && key < sm.lkey[m - 1][tid]) { sm.lkey[m][tid] = sm.lkey[m - 1][tid]; sm.lt[m][tid] = sm.lt[m - 1][tid]; m--; }
+          sm.lkey[m][tid] = key; sm.lt[m][tid] = tk;
+        }
+      }
+    }
+    __syncwarp();
+
+    // ---- phases T and U work per seed group: lane = parent slot (T) / new rank (U) ----------------------------------
+    const float chi2 = sm.chi2[tid];
+    const int cn = sm.cnt[tid];
+    const int nh = cn & 0xff, nm = (cn >> 8) & 0xff;
+    const bool parent_live = seed_act && sub < nl_prev;
+
+    // offers to best_short (C9.6): first the stops found while propagating (state before the layer), then the
+    // stopped miss children (propagated state), each in rank order; strict comparison with the holder
+    if (seed_act) {
+      const bool off0 = parent_live && (fl & FL_OFFER), off1 = parent_live && (fl & FL_OFFER_MISS);
+      const int onm = off1 ? nm + 1 : nm;
+      float os = (off0 || off1) ? score_of(p, nh, onm, chi2) : -INFINITY, oc = chi2; int ok = (off1 ? G : 0) + sub, ol = sub;
 #pragma unroll
       for (int d = 1; d < G; d <<= 1) {
         const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
@@ -275,117 +506,167 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
       }
       if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
         const int src = gbase + ol;
-        if (sub == ol) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
+        if (sub == ol) { KState S; ld_state(ok >= G ? sm.B : sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
         bs_have = true; bs_score = os; bs_chi2 = oc;
-        bs_nh = __shfl_sync(gm, nh, src); bs_nm = __shfl_sync(gm, offer_nm, src);
-        bs_stat = __shfl_sync(gm, stat, src);
+        bs_nh = __shfl_sync(gm, nh, src); bs_nm = __shfl_sync(gm, onm, src);
+        bs_stat = __shfl_sync(gm, (fl & (FL_OFFER | FL_OFFER_MISS)) ? sm.ostat[tid] : 0u, src);
         bs_step = s; bs_parent = ol; bs_last = (ok >= G) ? -1 : -2;
       }
     }
 
-    // ---- top max_cand children of the seed (U14) --------------------------------------------------------
-    const float base_hit = score_of(p, nh + 1, nm, chi2);     // hit child: base_hit - c2_hit
-    const float sc_miss = score_of(p, nh, nm + 1, chi2), sc_pass = score_of(p, nh, nm, chi2);
-    int my_parent = sub, my_hit = -2, my_kind = -1;           // what this slot becomes
-    int n_new = 0;
-    for (int r = 0; r < p.max_cand; r++) {
-      float hs, hc; int hh, hk;                               // head child of this lane
-      if (head < n_hitc) { const float c2h = hc2[head * BUILD_BLOCK]; hs = base_hit - c2h; hc = chi2 + c2h; hh = hid[head * BUILD_BLOCK]; hk = 0; }
-      else if (miss_avail) { hs = sc_miss; hc = chi2; hh = HIT_NONE; hk = 1; }
-      else if (pass_avail) { hs = sc_pass; hc = chi2; hh = HIT_NONE; hk = 2; }
-      else { hs = -INFINITY; hc = INFINITY; hh = HIT_NONE; hk = 3; }
-      float ws = hs, wc = hc; int wp = sub, wh = hh, wk = hk;
+    // ---- phase T: top max_cand children of the seed (U14) -----------------------------------------------------------
+    int my_parent = sub, my_hit = -2, my_kind = -1, my_t = 0, n_new = 0;
+    if (seed_act) {
+      const float base_hit = score_of(p, nh + 1, nm, chi2);   // hit child: base_hit - c2_hit
+      const bool alt_avail0 = parent_live && (fl & (FL_MISS | FL_PASS));
+      const int alt_kind = (fl & FL_MISS) ? 1 : 2;
+      const float alt_score = (fl & FL_MISS) ? score_of(p, nh, nm + 1, chi2) : score_of(p, nh, nm, chi2);
+      bool alt_avail = alt_avail0;
+      if (!parent_live) n_hitc = 0;
+      int head = 0;
+      for (int r = 0; r < p.max_cand; r++) {
+        // head child of this lane: its next hit or its miss / pass-through child, whichever ranks first (U14)
+        float hs = -INFINITY, hc = INFINITY; int hh = HIT_NONE, hk = 3, ht = 0;
+        if (head < n_hitc) {
+          const unsigned long long key = sm.lkey[head][tid];
+          const float c2h = __uint_as_float((unsigned)(key >> 32));
+          hs = base_hit - c2h; hc = chi2 + c2h; hh = (int)(unsigned)key; hk = 0; ht = sm.lt[head][tid];
+        }
+        if (alt_avail && (hk == 3 || before(alt_score, chi2, sub, HIT_NONE, hs, hc, sub, hh))) { hs = alt_score; hc = chi2; hh = HIT_NONE; hk = alt_kind; }
+        float ws = hs, wc = hc; int wp = sub, wh = hh, wk = hk, wt = ht;
 #pragma unroll
-      for (int d = 1; d < G; d <<= 1) {
-        const float s2 = __shfl_xor_sync(gm, ws, d), c2 = __shfl_xor_sync(gm, wc, d);
-        const int p2 = __shfl_xor_sync(gm, wp, d), h2 = __shfl_xor_sync(gm, wh, d), k2 = __shfl_xor_sync(gm, wk, d);
-        if (before(s2, c2, p2, h2, ws, wc, wp, wh)) { ws = s2; wc = c2; wp = p2; wh = h2; wk = k2; }
+        for (int d = 1; d < G; d <<= 1) {
+          const float s2 = __shfl_xor_sync(gm, ws, d), c2 = __shfl_xor_sync(gm, wc, d);
+          const int p2 = __shfl_xor_sync(gm, wp, d), h2 = __shfl_xor_sync(gm, wh, d), k2 = __shfl_xor_sync(gm, wk, d), t2 = __shfl_xor_sync(gm, wt, d);
+          if (before(s2, c2, p2, h2, ws, wc, wp, wh)) { ws = s2; wc = c2; wp = p2; wh = h2; wk = k2; wt = t2; }
+        }
+        if (!(ws > -INFINITY)) break;                         // pool exhausted (uniform in the group)
+        if (sub == wp) { if (wk == 0) head++; else alt_avail = false; }      // the winner lane pops its head
+        if (sub == r) { my_parent = wp; my_kind = wk; my_hit = wk == 0 ? wh : (wk == 1 ? -1 : -2); my_t = wt; }
+        n_new = r + 1;
       }
-      if (!(ws > -INFINITY)) break;                           // pool exhausted (uniform in the group)
-      if (sub == wp) {                                        // the winner lane pops its head
-        if (wk == 0) {
-          head++;
-        } else if (wk == 1) miss_avail = false;
-        else pass_avail = false;
-      }
-      if (sub == r) { my_parent = wp; my_kind = wk; my_hit = wk == 0 ? wh : (wk == 1 ? -1 : -2); }
-      n_new = r + 1;
     }
 
-    // ---- the new live set: fetch the parent's state, update with the hit -----------------------------------
-    {
-      const int src = gbase + my_parent;
-      SHFL_STATE(S, src, gm);
-      chi2 = __shfl_sync(gm, chi2, src);
-      nh = __shfl_sync(gm, nh, src); nm = __shfl_sync(gm, nm, src); consec = __shfl_sync(gm, consec, src);
-      stat = __shfl_sync(gm, stat, src);
-    }
-    live = sub < n_new;
+    // ---- phase U: the new live set: the parent's state, updated with the hit ---------------------------------------
+    KState S;
+    float c_chi2 = 0.f; int c_nh = 0, c_nm = 0, c_consec = 0;
+    bool live = seed_act && sub < n_new;
+    bool nan_child = false;
     if (live) {
-      if (my_kind == 1) { nm++; consec++; }
+      const int ps = (tid & ~(G - 1)) + my_parent;            // parent's slot
+      const int pcn = sm.cnt[ps];
+      c_chi2 = sm.chi2[ps]; c_nh = pcn & 0xff; c_nm = (pcn >> 8) & 0xff; c_consec = pcn >> 16;
+      if (my_kind == 2) ld_state(sm.A, ps, S);                // pass-through: the state does not move
+      else ld_state(sm.B, ps, S);
+      if (my_kind == 1) { c_nm++; c_consec++; }
       else if (my_kind == 0) {
-        Hit H; load_hit(H, a.hits, my_hit);
+        Hit H;
+        if (a.packed) {
+          const float4 q0 = __ldg(a.packed + my_t);
+          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * my_t;
+          const float4 b = __ldg(cv), d = __ldg(cv + 1);
+          H.x = q0.x; H.y = q0.y; H.z = q0.z;
+          H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
+        } else load_hit(H, a.hits, my_hit);
         SInv o; float c2;
         hit_to_local(S, H, o);
-        if (kalman_update(S, o, c2)) {
-          chi2 += c2; nh++; consec = 0;
-          if (!state_finite(S)) live = false;                 // dropped (C9: NaN child)
-        } else live = false;
+        if (COUNT) n_upd++;
+        if (kalman_update(S, o, c2) && state_finite(S) && fabsf(c2) <= 3.0e38f) { c_chi2 += c2; c_nh++; c_consec = 0; }
+        else { live = false; nan_child = true; }              // dropped (C9 / R1)
       }
     }
-    // keep the live lanes contiguous in rank order (only needed after a dropped child)
-    const unsigned alive = (__ballot_sync(gm, live) >> gbase) & 0xffu;
-    if (alive != ((1u << n_new) - 1u)) {
-      const int cnt = __popc(alive);
-      const int pick = sub < cnt ? (int)__fns(alive, 0, sub + 1) : sub;
-      const int src = gbase + pick;
-      SHFL_STATE(S, src, gm);
-      chi2 = __shfl_sync(gm, chi2, src);
-      nh = __shfl_sync(gm, nh, src); nm = __shfl_sync(gm, nm, src); consec = __shfl_sync(gm, consec, src);
-      stat = __shfl_sync(gm, stat, src);
-      my_parent = __shfl_sync(gm, my_parent, src); my_hit = __shfl_sync(gm, my_hit, src);
-      n_new = cnt; live = sub < cnt;
+    const bool any_nan = __syncthreads_or(nan_child);         // also: every read of A and B of this step is done
+    if (any_nan) {
+     if (seed_act) {
+      // R1: the parent of a dropped child, as it stood before the layer, is offered to best_short (after the offers
+      // above, in child rank order; strict comparison with the holder)
+      const int ps = (tid & ~(G - 1)) + my_parent;
+      const int pcn = sm.cnt[ps];
+      const int pnh = pcn & 0xff, pnm = (pcn >> 8) & 0xff;
+      const float pchi2 = sm.chi2[ps];
+      float os = (nan_child && pnh >= p.min_hits_keep) ? score_of(p, pnh, pnm, pchi2) : -INFINITY, oc = pchi2; int ol = sub;
+#pragma unroll
+      for (int d = 1; d < G; d <<= 1) {
+        const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
+        const int l2 = __shfl_xor_sync(gm, ol, d);
+        const bool take = (s2 != os) ? (s2 > os) : ((c2 != oc) ? (c2 < oc) : (l2 < ol));
+        if (take) { os = s2; oc = c2; ol = l2; }
+      }
+      if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
+        const int src = gbase + ol;
+        if (sub == ol) { KState Sp; ld_state(sm.A, ps, Sp); store_state(Sp, a.par_out, a.cov_out, n, (size_t)i); }
+        bs_have = true; bs_score = os; bs_chi2 = oc;
+        bs_nh = __shfl_sync(gm, pnh, src); bs_nm = __shfl_sync(gm, pnm, src);
+        bs_stat = 0;
+        bs_step = s; bs_parent = __shfl_sync(gm, my_parent, src); bs_last = -2;
+      }
+     }
+      __syncthreads();                                        // the parents' states have been read
     }
-    if (live) trellis[s * G + sub] = (unsigned)(my_hit + 2) | ((unsigned)my_parent << 28);
-    n_live = n_new;
-    t_last = s;
-    __syncwarp(gm);
+    if (seed_act) {
+      // the live children, contiguous in rank order
+      const unsigned alive = (__ballot_sync(gm, live) >> gbase) & 0xffu;
+      if (live) {
+        const int dst = (tid & ~(G - 1)) + __popc(alive & ((1u << sub) - 1u));
+        st_state(sm.A, dst, S);
+        sm.chi2[dst] = c_chi2; sm.cnt[dst] = c_nh | (c_nm << 8) | (c_consec << 16);
+        trellis[(size_t)s * G + (dst & (G - 1))] = (unsigned)(my_hit + 2) | ((unsigned)my_parent << 28);
+      }
+      if (sub == 0) sm.n_live[sl] = __popc(alive);
+      t_last = s;
+    }
+    __syncthreads();
   }
 
-  if (!have_seed) return;
-  // ---- final choice: best of live U {best_short} (C9) -------------------------------------------------------
-  float fs = (live && nh >= p.min_hits_keep) ? score_of(p, nh, nm, chi2) : -INFINITY, fc = chi2; int fl = sub;
+  // ---- final choice: best of live U {best_short} (C9) -----------------------------------------------------------
+  if (i >= 0) {
+    const int nl = sm.n_live[sl];
+    const float chi2 = sm.chi2[tid];
+    const int cn = sm.cnt[tid];
+    const int nh = cn & 0xff, nm = (cn >> 8) & 0xff;
+    const bool live = seed_ok && sub < nl;
+    float fs = (live && nh >= p.min_hits_keep) ? score_of(p, nh, nm, chi2) : -INFINITY, fc = chi2; int fl2 = sub;
 #pragma unroll
-  for (int d = 1; d < G; d <<= 1) {
-    const float s2 = __shfl_xor_sync(gm, fs, d), c2 = __shfl_xor_sync(gm, fc, d);
-    const int l2 = __shfl_xor_sync(gm, fl, d);
-    const bool take = (s2 != fs) ? (s2 > fs) : ((c2 != fc) ? (c2 < fc) : (l2 < fl));
-    if (take) { fs = s2; fc = c2; fl = l2; }
+    for (int d = 1; d < G; d <<= 1) {
+      const float s2 = __shfl_xor_sync(gm, fs, d), c2 = __shfl_xor_sync(gm, fc, d);
+      const int l2 = __shfl_xor_sync(gm, fl2, d);
+      const bool take = (s2 != fs) ? (s2 > fs) : ((c2 != fc) ? (c2 < fc) : (l2 < fl2));
+      if (take) { fs = s2; fc = c2; fl2 = l2; }
+    }
+    const bool live_wins = fs > -INFINITY && !(bs_have && (bs_score > fs || (bs_score == fs && bs_chi2 < fc)));
+    float o_chi2, o_score; int o_nh, o_nm, bt_step, bt_slot, tail_step = -1, tail_val = -2; unsigned o_stat;
+    if (live_wins) {
+      const int src = gbase + fl2;
+      if (sub == fl2) { KState S; ld_state(sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
+      o_chi2 = fc; o_score = fs;
+      o_nh = __shfl_sync(gm, nh, src); o_nm = __shfl_sync(gm, nm, src); o_stat = 0;
+      bt_step = t_last; bt_slot = fl2;
+    } else if (bs_have) {
+      o_chi2 = bs_chi2; o_score = bs_score; o_nh = bs_nh; o_nm = bs_nm; o_stat = bs_stat;
+      bt_step = bs_step - 1; bt_slot = bs_parent; tail_step = bs_step; tail_val = bs_last;
+    } else {                                                    // nothing qualifies: the seed itself, TRUNCATED
+      o_chi2 = seed_chi2; o_nh = seed_nh; o_nm = 0; o_stat = seed_stat | ST_TRUNC; o_score = score_of(p, seed_nh, 0, seed_chi2);
+      bt_step = seed_last; bt_slot = 0;
+    }
+    if (sub == 0) {
+      a.chi2[i] = o_chi2; a.score[i] = o_score; a.nhits[i] = o_nh; a.nmiss[i] = o_nm; a.status[i] = o_stat;
+      int slot = bt_slot;
+      for (int s = mpl - 1; s >= 0; s--) {
+        int v = -2;
+        if (s == tail_step) v = tail_val;
+        else if (s <= bt_step) { const unsigned e = trellis[(size_t)s * G + slot]; v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28); }
+        a.hit_ids[(size_t)s * n + i] = v;
+      }
+    }
   }
-  const bool live_wins = fs > -INFINITY && !(bs_have && (bs_score > fs || (bs_score == fs && bs_chi2 < fc)));
-  float o_chi2, o_score; int o_nh, o_nm, bt_step, bt_slot, tail_step = -1, tail_val = -2; unsigned o_stat;
-  if (live_wins) {
-    const int src = gbase + fl;
-    if (sub == fl) store_state(S, a.par_out, a.cov_out, n, (size_t)i);
-    o_chi2 = fc; o_score = fs;
-    o_nh = __shfl_sync(gm, nh, src); o_nm = __shfl_sync(gm, nm, src); o_stat = __shfl_sync(gm, stat, src);
-    bt_step = t_last; bt_slot = fl;
-  } else if (bs_have) {
-    o_chi2 = bs_chi2; o_score = bs_score; o_nh = bs_nh; o_nm = bs_nm; o_stat = bs_stat;
-    bt_step = bs_step - 1; bt_slot = bs_parent; tail_step = bs_step; tail_val = bs_last;
-  } else {                                                    // nothing qualifies: the seed itself, TRUNCATED
-    o_chi2 = seed_chi2; o_nh = seed_nh; o_nm = 0; o_stat = seed_stat | ST_TRUNC; o_score = score_of(p, seed_nh, 0, seed_chi2);
-    bt_step = last_step; bt_slot = 0;
-  }
-  __syncwarp(gm);
-  if (sub == 0) {
-    a.chi2[i] = o_chi2; a.score[i] = o_score; a.nhits[i] = o_nh; a.nmiss[i] = o_nm; a.status[i] = o_stat;
-    int slot = bt_slot;
-    for (int s = mpl - 1; s >= 0; s--) {
-      int v = -2;
-      if (s == tail_step) v = tail_val;
-      else if (s <= bt_step) { const unsigned e = trellis[s * G + slot]; v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28); }
-      a.hit_ids[(size_t)s * n + i] = v;
+  if (COUNT) {
+    unsigned v[5] = {n_steps, n_pos, n_c2, n_acc, n_upd};
+#pragma unroll
+    for (int k = 0; k < 5; k++) {
+      unsigned x = v[k];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+      if (lane == 0 && x) atomicAdd(&a.counters[k], (unsigned long long)x);
     }
   }
 }
@@ -393,32 +674,36 @@ __global__ void __launch_bounds__(BUILD_BLOCK, MKF_BUILD_MIN_BLOCKS) mkf_build_k
 }  // namespace
 
 namespace mkf {
-size_t build_smem_bytes(int max_plan_len) {
-  return (size_t)(BUILD_BLOCK / G) * max_plan_len * G * sizeof(unsigned) + (size_t)2 * G * BUILD_BLOCK * sizeof(float);
+// workspace of mkf_build_tracks: seed records, trellis, seed order, sort keys, bucket counts + scan partials
+static size_t n_buckets_of(const mkf_ctx* c, int n_events) { return (size_t)n_events * c->g.n_plans * 256 + 1; }
+size_t build_ws_bytes(const mkf_ctx* c, int n_events, int n_seeds) {
+  const size_t n = (size_t)n_seeds, nbk = n_buckets_of(c, n_events);
+  return align256(n * NW * 4) + align256(n * c->max_plan_len * G * 4) + 2 * align256(n * 4) + 2 * align256((nbk + 1) * 4) + scan_partial_bytes(nbk);
 }
-}
+}  // namespace mkf
 
 extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
                                 const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
                                 mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids,
                                 unsigned* status, void* ws, size_t ws_bytes, void* stream) {
-  (void)ws; (void)ws_bytes;
   if (!c) return MKF_INVALID_ARG;
   if (!h || !idx || !seeds || !out) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
   if (seeds->n < 0 || out->n != seeds->n || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: bad sizes");
-  if (h->n_hits >= (1 << 28)) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: n_hits >= 2^28");
+  if (max_plan_len != c->max_plan_len) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: max_plan_len is not mkf_max_plan_len(ctx)");
+  if (h->n_hits > (1 << 28) - 2) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: n_hits > 2^28 - 2");
   if (seeds->n == 0) return MKF_OK;                      // nothing to do; array pointers may be null
   if (!seed_event || !seed_hits || !plan || !chi2 || !score || !nhits || !nmiss || !hit_ids || !status)
     return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
   if (!idx->bin_off || !idx->sorted_id || !idx->vmax || !h->layer_off || !h->x || !h->y || !h->z || !h->V ||
       !seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov)
     return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null array");
-  const size_t smem = build_smem_bytes(max_plan_len);
-  if (smem > 200 * 1024) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: plan too long for the shared-memory trellis");
-  if (smem > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(mkf_build_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
-  }
+  if (h->n_events < 1) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: no events");
+  if (c->g.n_phi > 255 || c->g.n_eta > 255) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: more than 255 phi or eta bins");
+  const size_t need = build_ws_bytes(c, h->n_events, seeds->n);
+  if (ws_bytes < need || !ws) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_build_tracks: workspace too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t n = (size_t)seeds->n, nbk = n_buckets_of(c, h->n_events);
+  char* w = (char*)ws;
   BuildArgs a;
   a.hits = hits_dev(h);
   a.bin_off = idx->bin_off; a.sorted_id = idx->sorted_id; a.vmax = idx->vmax; a.packed = (const float4*)idx->packed;
@@ -426,9 +711,34 @@ extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_ind
   a.plan = plan; a.max_plan_len = max_plan_len;
   a.par_out = out->par; a.cov_out = out->cov; a.chi2 = chi2; a.score = score; a.nhits = nhits; a.nmiss = nmiss;
   a.hit_ids = hit_ids; a.status = status;
-  const int seeds_per_cta = BUILD_BLOCK / G;
-  const int grid = (a.n + seeds_per_cta - 1) / seeds_per_cta;
-  mkf_build_kernel<<<grid, BUILD_BLOCK, smem, (cudaStream_t)stream>>>(c->g, c->p, a);
+  a.wseed = (float*)w; w += align256(n * NW * 4);
+  a.trellis = (unsigned*)w; w += align256(n * max_plan_len * G * 4);
+  int* order = (int*)w; w += align256(n * 4);
+  a.order = order;
+  a.key = (unsigned*)w; w += align256(n * 4);
+  a.bucket = (unsigned*)w; w += align256((nbk + 1) * 4);
+  unsigned* bucket_off = (unsigned*)w; w += align256((nbk + 1) * 4);
+  unsigned* partial = (unsigned*)w;
+  a.n_buckets = (int)nbk;
+  a.counters = c->build_counters;
+  cudaError_t e = cudaMemsetAsync(a.bucket, 0, nbk * 4, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: memset");
+  bs_seed_kernel<<<(a.n + 127) / 128, 128, 0, st>>>(c->g, c->p, a);
+  MKF_LAUNCHED(c, "bs_seed_kernel");
+  { const int rc = exclusive_scan_u32(c, a.bucket, nbk, partial, bucket_off, (unsigned)a.n, st); if (rc) return rc; }
+  bs_order_kernel<<<(a.n + 255) / 256, 256, 0, st>>>(a.n, a.key, a.bucket, order);
+  MKF_LAUNCHED(c, "bs_order_kernel");
+  const size_t smem = sizeof(Smem);
+  const int grid = (a.n + NS - 1) / NS;
+  if (a.counters) {
+    e = cudaFuncSetAttribute(mkf_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
+    mkf_build_kernel<true><<<grid, BT, smem, st>>>(c->g, c->p, a);
+  } else {
+    e = cudaFuncSetAttribute(mkf_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
+    mkf_build_kernel<false><<<grid, BT, smem, st>>>(c->g, c->p, a);
+  }
   MKF_LAUNCHED(c, "mkf_build_kernel");
   return MKF_OK;
 }

@@ -13,6 +13,7 @@ namespace mkf {
 size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits);
 size_t dedup_ws_bytes(int n_hits, int n, int mpl);
 size_t strips_ws_bytes(int n_strips, int capacity);
+size_t build_ws_bytes(const mkf_ctx* c, int n_events, int n_seeds);
 int fit_launch(mkf_ctx* c, bool backward, const FitArgs& a, cudaStream_t st);
 }
 using namespace mkf;
@@ -23,7 +24,8 @@ extern "C" size_t mkf_workspace_bytes(const mkf_ctx* c, int call_id, int n_event
     case MKF_CALL_BUILD_HIT_INDEX: return hit_index_ws_bytes(c, n_events, n_hits);
     case MKF_CALL_REMOVE_DUPLICATES: return dedup_ws_bytes(n_hits, n_seeds, c->max_plan_len);
     case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits, n_seeds);
-    default: return 0;      // fit and build keep everything in registers / shared memory
+    case MKF_CALL_BUILD_TRACKS: return build_ws_bytes(c, n_events, n_seeds);
+    default: return 0;      // the fit keeps everything in registers
   }
 }
 

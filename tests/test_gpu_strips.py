@@ -58,7 +58,7 @@ def test_strips_degenerate_inputs():
     m1 = 2 * TILE + 77
     one = dict(module_off=np.arange(m1 + 1, dtype=np.int32), adc=np.full(m1, 100, np.uint16), noise=np.full(m1, 4, np.float32),
                bad=np.zeros(m1, np.uint8))
-    assert len(check(one, sp)["module"]) == m1
+    assert len(check(one, sp, capacity=m1)["module"]) == m1
     # capacity smaller than the number found: the count is still exact (the records are then incomplete)
     check(alt, sp, capacity=100)
     # saturated counts: 16-bit ADC at full scale over a long cluster (sums beyond 32 bits)
