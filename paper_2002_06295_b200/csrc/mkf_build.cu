@@ -63,6 +63,8 @@ struct BuildArgs {
   unsigned long long* counters;
 };
 
+constexpr int OVC = 256;             // CTA-wide overflow list of accepted hits beyond a candidate's LC entries
+
 struct Smem {
   float A[NF][SL];          // live candidates as they stand before this layer
   float B[NF][SL];          // the same candidates propagated to this layer (material applied)
@@ -74,6 +76,8 @@ struct Smem {
   int lcount[SL];
   unsigned long long lkey[LC][SL];                 // chi2 bits << 32 | hit id: ascending = the order U14 within a parent
   int lt[LC][SL];                                  // position of the hit in the packed arrays
+  unsigned long long ovf_key[OVC]; int ovf_t[OVC]; int ovf_slot[OVC]; int ovf_n;
+  int sel[SL], sel_t[SL], sel_hit[SL];             // the children picked for the new live set: parent | kind << 3 | dead << 8
   int plist[SL]; int nP;
   int wsum[BT / 32];
   int n_live[NS], p0[NS], plen[NS], ev[NS], last[NS], seed[NS];
@@ -82,14 +86,6 @@ struct Smem {
 
 __device__ __forceinline__ float score_of(const ParamsDev& p, int nh, int nm, float chi2) {
   return p.score_hit * (float)nh - p.score_miss * (float)nm - chi2;
-}
-
-// U14: does child a rank before child b?
-__device__ __forceinline__ bool before(float sa, float ca, int pa, int ha, float sb, float cb, int pb, int hb) {
-  if (sa != sb) return sa > sb;
-  if (ca != cb) return ca < cb;
-  if (pa != pb) return pa < pb;
-  return ha < hb;
 }
 
 __device__ __forceinline__ void st_state(float (*M)[SL], int slot, const KState& S) {
@@ -233,35 +229,58 @@ __global__ void __launch_bounds__(256) bs_order_kernel(int n, const unsigned* __
 // ---- the chi2 of one hit against one propagated candidate; appends accepted hits to the candidate's list ---------
 struct ScanCand { float x, y, z, xl, yl, zl, cb, sb, tt, tz, zz, lim1, lim2; int kind; };
 
+__device__ __forceinline__ void accept_hit(Smem& sm, int slot, float c2, int id, unsigned t) {
+  const unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
+  const int k = atomicAdd(&sm.lcount[slot], 1);
+  if (k < LC) { sm.lkey[k][slot] = key; sm.lt[k][slot] = (int)t; }
+  else {                                                           // a crowded window: the CTA-wide overflow list
+    const int e = atomicAdd(&sm.ovf_n, 1);
+    if (e < OVC) { sm.ovf_key[e] = key; sm.ovf_t[e] = (int)t; sm.ovf_slot[e] = slot; }
+  }
+}
+
 template <bool COUNT>
 __device__ __forceinline__ void scan_range(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const ScanCand& c,
                                            unsigned tb, unsigned te, int lane, int stride, unsigned& n_pos, unsigned& n_c2, unsigned& n_acc) {
   KState S;                                                        // only what hit_to_local / chi2_local read
   S.x = c.x; S.y = c.y; S.z = c.z; S.xl = c.xl; S.yl = c.yl; S.zl = c.zl; S.f.kind = c.kind; S.f.cb = c.cb; S.f.sb = c.sb;
-  for (unsigned t = tb + lane; t < te; t += stride) {
-    Hit H; int id;
-    if (COUNT) n_pos++;
-    if (a.packed) {
+  unsigned t = tb + lane;
+  if (a.packed) {
+    float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (t < te) qn = __ldg(a.packed + t);
+    while (t < te) {
       // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11), so most
-      // hits of the padded bins are rejected before their covariance is read
-      const float4 q0 = __ldg(a.packed + t);
+      // hits of the padded bins are rejected before their covariance is read; the next position is already in flight
+      const float4 q0 = qn;
+      const unsigned tn = t + stride;
+      if (tn < te) qn = __ldg(a.packed + tn);
+      if (COUNT) n_pos++;
       const float rx = (q0.x - c.x) - c.xl, ry = (q0.y - c.y) - c.yl, rz = (q0.z - c.z) - c.zl;
       const float r1 = c.kind == 0 ? c.cb * ry - c.sb * rx : rx, r2 = c.kind == 0 ? rz : ry;
-      if (r1 * r1 > c.lim1 || r2 * r2 > c.lim2) continue;
-      const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
-      const float4 b = __ldg(cv), d = __ldg(cv + 1);
-      H.x = q0.x; H.y = q0.y; H.z = q0.z; id = __float_as_int(q0.w);
-      H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-    } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
-    if (COUNT) n_c2++;
-    SInv o; float c2;
-    if (!chi2_local(S, c.tt, c.tz, c.zz, H, o, c2)) continue;
-    if (c2 < p.chi2_cut) {
-      if (COUNT) n_acc++;
-      const int k = atomicAdd(&sm.lcount[slot], 1);
-      if (k < LC) {
-        sm.lkey[k][slot] = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
-        sm.lt[k][slot] = (int)t;
+      if (!(r1 * r1 > c.lim1 || r2 * r2 > c.lim2)) {
+        const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
+        const float4 b = __ldg(cv), d = __ldg(cv + 1);
+        Hit H;
+        H.x = q0.x; H.y = q0.y; H.z = q0.z;
+        H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
+        if (COUNT) n_c2++;
+        SInv o; float c2;
+        if (chi2_local(S, c.tt, c.tz, c.zz, H, o, c2) && c2 < p.chi2_cut) {
+          if (COUNT) n_acc++;
+          accept_hit(sm, slot, c2, __float_as_int(q0.w), t);
+        }
+      }
+      t = tn;
+    }
+  } else {
+    for (; t < te; t += stride) {
+      const int id = a.sorted_id[t];
+      Hit H; load_hit(H, a.hits, id);
+      if (COUNT) { n_pos++; n_c2++; }
+      SInv o; float c2;
+      if (chi2_local(S, c.tt, c.tz, c.zz, H, o, c2) && c2 < p.chi2_cut) {
+        if (COUNT) n_acc++;
+        accept_hit(sm, slot, c2, id, t);
       }
     }
   }
@@ -274,8 +293,17 @@ __device__ __forceinline__ void load_scan_cand(const Smem& sm, int slot, ScanCan
   c.tt = sm.tt[slot]; c.tz = sm.tz[slot]; c.zz = sm.zz[slot]; c.lim1 = sm.lim1[slot]; c.lim2 = sm.lim2[slot];
 }
 
-// More than LC hits of a window passed the cut (a crowded region): the owner of the slot walks its window again and
-// keeps the LC best under (chi2, id). Rare; not inlined so that it stays out of the hot loop's instruction stream.
+// sorted insertion of (key, t) into the first `cnt` (<= LC) entries of a slot's list, keeping the LC smallest keys
+__device__ __forceinline__ void list_insert(Smem& sm, int slot, int& cnt, unsigned long long key, int t) {
+  int k = cnt;
+  if (cnt == LC) { if (key < sm.lkey[LC - 1][slot]) k = LC - 1; else return; }
+  else cnt++;
+  while (k > 0 && key < sm.lkey[k - 1][slot]) { sm.lkey[k][slot] = sm.lkey[k - 1][slot]; sm.lt[k][slot] = sm.lt[k - 1][slot]; k--; }
+  sm.lkey[k][slot] = key; sm.lt[k][slot] = t;
+}
+
+// Last resort (the CTA-wide overflow list itself overflowed): the owner of the slot walks its window again and keeps
+// the LC best under (chi2, id). Not inlined so that it stays out of the hot loop's instruction stream.
 __device__ __noinline__ void rescan_slot(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const unsigned* boff, int n_phi) {
   ScanCand c; load_scan_cand(sm, slot, c);
   KState S;
@@ -300,17 +328,21 @@ __device__ __noinline__ void rescan_slot(const BuildArgs& a, const ParamsDev& p,
         SInv o; float c2;
         if (!chi2_local(S, c.tt, c.tz, c.zz, H, o, c2)) continue;
         if (!(c2 < p.chi2_cut)) continue;
-        const unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
-        int k = cntk;
-        if (cntk == LC) { if (key < sm.lkey[LC - 1][slot]) k = LC - 1; else continue; }
-        else cntk++;
-        while (k > 0 && key < sm.lkey[k - 1][slot]) { sm.lkey[k][slot] = sm.lkey[k - 1][slot]; sm.lt[k][slot] = sm.lt[k - 1][slot]; k--; }
-        sm.lkey[k][slot] = key; sm.lt[k][slot] = (int)t;
+        list_insert(sm, slot, cntk, ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id, (int)t);
       }
     }
   }
   sm.lcount[slot] = cntk;
 }
+
+// U14 as two integer keys, smaller = ranks first: k1 = (score descending, chi2 ascending), k2 = (parent, hit id)
+__device__ __forceinline__ unsigned long long rank_key1(float score, float chi2) {
+  unsigned su = __float_as_uint(score);
+  su = (su & 0x80000000u) ? ~su : (su | 0x80000000u);            // ascending in the float order
+  return ((unsigned long long)(~su) << 32) | __float_as_uint(chi2);
+}
+__device__ __forceinline__ unsigned rank_key2(int parent, int hit) { return ((unsigned)parent << 28) | ((unsigned)hit & 0x0fffffffu); }
+constexpr unsigned long long KEY_NONE = ~0ull;
 
 #ifndef MKF_BUILD_MIN_BLOCKS
 #define MKF_BUILD_MIN_BLOCKS 4
@@ -322,7 +354,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int sl = tid >> 3;                                   // seed of this thread's slot (phases T, U)
+  const int sl = tid >> 3;                                   // seed of this thread's group (phases T, offers)
   const int sub = tid & (G - 1);                             // candidate slot inside the seed
   const int gbase = lane & ~(G - 1);
   const unsigned gm = 0xffu << gbase;
@@ -364,11 +396,12 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     // ---- which slots propagate at this step: compacted list over the CTA ------------------------------------------
     const int nl_prev = sm.n_live[sl];
     const bool seed_act = i >= 0 && seed_ok && s > seed_last && s < sm.plen[sl] && nl_prev > 0;     // uniform in the group
-    const bool act = seed_act && sub < nl_prev;
+    const bool parent_live = seed_act && sub < nl_prev;
     {
-      const unsigned bal = __ballot_sync(0xffffffffu, act);
+      const unsigned bal = __ballot_sync(0xffffffffu, parent_live);
       if (lane == 0) sm.wsum[warp] = __popc(bal);
       sm.flag[tid] = 0; sm.lcount[tid] = 0; sm.rowpre[tid] = 0;
+      if (tid == 0) sm.ovf_n = 0;
       __syncthreads();
       int base = 0, tot = 0;
 #pragma unroll
@@ -377,7 +410,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         __syncthreads();
         continue;
       }
-      if (act) sm.plist[base + __popc(bal & ((1u << lane) - 1u))] = tid;
+      if (parent_live) sm.plist[base + __popc(bal & ((1u << lane) - 1u))] = tid;
       if (tid == 0) sm.nP = tot;
       __syncthreads();
     }
@@ -392,7 +425,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       Prop P;
       const unsigned rc = propagate_geom(S, L, sm.aq[ssl], p.graze_cos_min, p.material_flags, true, P);
       const int cn = sm.cnt[slot];
-      const int nh = cn & 0xff, nm = (cn >> 8) & 0xff, consec = cn >> 16;
+      const int nh = cn & 0xff, consec = cn >> 16;
       if (rc & (ST_UNREACH | ST_SKIP_ACC)) {
         sm.flag[slot] = FL_PASS;                              // silent skip: competes unchanged (C9.1)
       } else if (rc) {                                        // grazing / energy exhausted: the candidate stops
@@ -437,183 +470,244 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       __syncthreads();
     }
 
-    // ---- phase S: SCAN_G lanes per (candidate, eta row) --------------------------------------------------------------
-    {
-      const int NR = sm.rowpre[SL];
+    // ---- phase S: SCAN_G lanes per (candidate, eta row); the next row's bin offsets are fetched ahead ---------------
+    const int NR = sm.rowpre[SL];
+    if (NR > 0) {
       const int gl = tid & (SCAN_G - 1);
-      for (int j = tid / SCAN_G; j < NR; j += BT / SCAN_G) {
+      auto item = [&](int j, int& slot, unsigned& tb0, unsigned& te0, unsigned& tb1, unsigned& te1) {
         int lo = 0, hi = SL;
 #pragma unroll
         for (int it = 0; it < 8; it++) {                      // last slot with rowpre[slot] <= j  (SL <= 256)
           const int mid = (lo + hi) >> 1;
           if (hi - lo > 1) { if (sm.rowpre[mid] <= j) lo = mid; else hi = mid; }
         }
-        const int slot = lo;
+        slot = lo;
         const int ssl = slot >> 3;
-        ScanCand c; load_scan_cand(sm, slot, c);
         const int ie = (sm.wrow[slot] & 0xff) + (j - sm.rowpre[slot]);
         const int w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
         const int lay = g.plan_layers[sm.p0[ssl] + s];
         const unsigned* row = a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb + ie * g.n_phi;
-        const unsigned tb0 = __ldg(row + w0), te0 = __ldg(row + min(w0 + wn, g.n_phi));
-        unsigned tb1 = 0, te1 = 0;
+        tb0 = __ldg(row + w0); te0 = __ldg(row + min(w0 + wn, g.n_phi));
+        tb1 = 0; te1 = 0;
         if (w0 + wn > g.n_phi) { tb1 = __ldg(row); te1 = __ldg(row + w0 + wn - g.n_phi); }
+      };
+      int j = tid / SCAN_G;
+      int slot_n = 0; unsigned ntb0 = 0, nte0 = 0, ntb1 = 0, nte1 = 0;
+      if (j < NR) item(j, slot_n, ntb0, nte0, ntb1, nte1);
+      while (j < NR) {
+        const int slot = slot_n; const unsigned tb0 = ntb0, te0 = nte0, tb1 = ntb1, te1 = nte1;
+        const int jn = j + BT / SCAN_G;
+        if (jn < NR) item(jn, slot_n, ntb0, nte0, ntb1, nte1);
+        ScanCand c; load_scan_cand(sm, slot, c);
         scan_range<COUNT>(a, p, sm, slot, c, tb0, te0, gl, SCAN_G, n_pos, n_c2, n_acc);
         if (te1 > tb1) scan_range<COUNT>(a, p, sm, slot, c, tb1, te1, gl, SCAN_G, n_pos, n_c2, n_acc);
+        j = jn;
       }
+      __syncthreads();
     }
-    __syncthreads();
 
     // ---- phase L: each slot orders its accepted hits by (chi2, id) ---------------------------------------------------
     const int fl = sm.flag[tid];
     int n_hitc = 0;
     if (fl & FL_SCAN) {
-      n_hitc = sm.lcount[tid];
-      if (n_hitc > LC) {
-        const int ssl = tid >> 3;
-        const int lay = g.plan_layers[sm.p0[ssl] + s];
-        rescan_slot(a, p, sm, tid, a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb, g.n_phi);
-        n_hitc = sm.lcount[tid];
-      } else {
-        for (int k = 1; k < n_hitc; k++) {
-          const unsigned long long key = sm.lkey[k][tid]; const int tk = sm.lt[k][tid];
-          int m = k;
-          while (m > 0 && key < sm.lkey[m - 1][tid]) { sm.lkey[m][tid] = sm.lkey[m - 1][tid]; sm.lt[m][tid] = sm.lt[m - 1][tid]; m--; }
-          sm.lkey[m][tid] = key; sm.lt[m][tid] = tk;
+      const int nacc = sm.lcount[tid];
+      n_hitc = min(nacc, LC);
+      for (int k = 1; k < n_hitc; k++) {
+        const unsigned long long key = sm.lkey[k][tid]; const int tk = sm.lt[k][tid];
+        int m = k;
+        while (m > 0 && key < sm.lkey[m - 1][tid]) { sm.lkey[m][tid] = sm.lkey[m - 1][tid]; sm.lt[m][tid] = sm.lt[m - 1][tid]; m--; }
+        sm.lkey[m][tid] = key; sm.lt[m][tid] = tk;
+      }
+      if (nacc > LC) {
+        const int nov = sm.ovf_n;
+        if (nov <= OVC) {
+          for (int e = 0; e < nov; e++) if (sm.ovf_slot[e] == tid) list_insert(sm, tid, n_hitc, sm.ovf_key[e], sm.ovf_t[e]);
+        } else {
+          const int ssl = tid >> 3;
+          const int lay = g.plan_layers[sm.p0[ssl] + s];
+          rescan_slot(a, p, sm, tid, a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb, g.n_phi);
+          n_hitc = sm.lcount[tid];
         }
       }
     }
     __syncwarp();
 
-    // ---- phases T and U work per seed group: lane = parent slot (T) / new rank (U) ----------------------------------
+    // ---- per seed group: lane = parent slot -------------------------------------------------------------------------
     const float chi2 = sm.chi2[tid];
     const int cn = sm.cnt[tid];
     const int nh = cn & 0xff, nm = (cn >> 8) & 0xff;
-    const bool parent_live = seed_act && sub < nl_prev;
+    // a seed all of whose candidates pass this layer by (not crossed) keeps its live set as it is
+    const bool noop = seed_act && (__ballot_sync(gm, parent_live && fl != FL_PASS) & gm) == 0u;
 
     // offers to best_short (C9.6): first the stops found while propagating (state before the layer), then the
     // stopped miss children (propagated state), each in rank order; strict comparison with the holder
-    if (seed_act) {
+    if (seed_act && !noop) {
       const bool off0 = parent_live && (fl & FL_OFFER), off1 = parent_live && (fl & FL_OFFER_MISS);
-      const int onm = off1 ? nm + 1 : nm;
-      float os = (off0 || off1) ? score_of(p, nh, onm, chi2) : -INFINITY, oc = chi2; int ok = (off1 ? G : 0) + sub, ol = sub;
+      if (__ballot_sync(gm, off0 || off1) & gm) {
+        const int onm = off1 ? nm + 1 : nm;
+        float os = (off0 || off1) ? score_of(p, nh, onm, chi2) : -INFINITY, oc = chi2; int ok = (off1 ? G : 0) + sub, ol = sub;
 #pragma unroll
-      for (int d = 1; d < G; d <<= 1) {
-        const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
-        const int k2 = __shfl_xor_sync(gm, ok, d), l2 = __shfl_xor_sync(gm, ol, d);
-        const bool take = (s2 != os) ? (s2 > os) : ((c2 != oc) ? (c2 < oc) : (k2 < ok));
-        if (take) { os = s2; oc = c2; ok = k2; ol = l2; }
-      }
-      if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
-        const int src = gbase + ol;
-        if (sub == ol) { KState S; ld_state(ok >= G ? sm.B : sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
-        bs_have = true; bs_score = os; bs_chi2 = oc;
-        bs_nh = __shfl_sync(gm, nh, src); bs_nm = __shfl_sync(gm, onm, src);
-        bs_stat = __shfl_sync(gm, (fl & (FL_OFFER | FL_OFFER_MISS)) ? sm.ostat[tid] : 0u, src);
-        bs_step = s; bs_parent = ol; bs_last = (ok >= G) ? -1 : -2;
+        for (int d = 1; d < G; d <<= 1) {
+          const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
+          const int k2 = __shfl_xor_sync(gm, ok, d), l2 = __shfl_xor_sync(gm, ol, d);
+          const bool take = (s2 != os) ? (s2 > os) : ((c2 != oc) ? (c2 < oc) : (k2 < ok));
+          if (take) { os = s2; oc = c2; ok = k2; ol = l2; }
+        }
+        if (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2)) {
+          const int src = gbase + ol;
+          if (sub == ol) { KState S; ld_state(ok >= G ? sm.B : sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
+          bs_have = true; bs_score = os; bs_chi2 = oc;
+          bs_nh = __shfl_sync(gm, nh, src); bs_nm = __shfl_sync(gm, onm, src);
+          bs_stat = __shfl_sync(gm, (fl & (FL_OFFER | FL_OFFER_MISS)) ? sm.ostat[tid] : 0u, src);
+          bs_step = s; bs_parent = ol; bs_last = (ok >= G) ? -1 : -2;
+        }
       }
     }
 
-    // ---- phase T: top max_cand children of the seed (U14) -----------------------------------------------------------
-    int my_parent = sub, my_hit = -2, my_kind = -1, my_t = 0, n_new = 0;
-    if (seed_act) {
+    // ---- phase T: top max_cand children of the seed (U14), 8-lane tournaments on integer keys -----------------------
+    int my_parent = sub, n_new = 0;
+    if (seed_act && !noop) {
       const float base_hit = score_of(p, nh + 1, nm, chi2);   // hit child: base_hit - c2_hit
-      const bool alt_avail0 = parent_live && (fl & (FL_MISS | FL_PASS));
+      bool alt_avail = parent_live && (fl & (FL_MISS | FL_PASS));
       const int alt_kind = (fl & FL_MISS) ? 1 : 2;
-      const float alt_score = (fl & FL_MISS) ? score_of(p, nh, nm + 1, chi2) : score_of(p, nh, nm, chi2);
-      bool alt_avail = alt_avail0;
+      const unsigned long long alt_k1 = rank_key1((fl & FL_MISS) ? score_of(p, nh, nm + 1, chi2) : score_of(p, nh, nm, chi2), chi2);
       if (!parent_live) n_hitc = 0;
       int head = 0;
+      int my_kind = -1, my_hit = -2, my_t = 0;
       for (int r = 0; r < p.max_cand; r++) {
         // head child of this lane: its next hit or its miss / pass-through child, whichever ranks first (U14)
-        float hs = -INFINITY, hc = INFINITY; int hh = HIT_NONE, hk = 3, ht = 0;
+        unsigned long long k1 = KEY_NONE; int hh = HIT_NONE, hk = 3, ht = 0;
         if (head < n_hitc) {
           const unsigned long long key = sm.lkey[head][tid];
           const float c2h = __uint_as_float((unsigned)(key >> 32));
-          hs = base_hit - c2h; hc = chi2 + c2h; hh = (int)(unsigned)key; hk = 0; ht = sm.lt[head][tid];
+          k1 = rank_key1(base_hit - c2h, chi2 + c2h); hh = (int)(unsigned)key; hk = 0; ht = sm.lt[head][tid];
         }
-        if (alt_avail && (hk == 3 || before(alt_score, chi2, sub, HIT_NONE, hs, hc, sub, hh))) { hs = alt_score; hc = chi2; hh = HIT_NONE; hk = alt_kind; }
-        float ws = hs, wc = hc; int wp = sub, wh = hh, wk = hk, wt = ht;
+        if (alt_avail && alt_k1 < k1) { k1 = alt_k1; hh = HIT_NONE; hk = alt_kind; }     // same parent: a tie in k1 goes to the hit
+        unsigned k2 = rank_key2(sub, hh);
+        unsigned long long w1 = k1; unsigned w2 = k2;
 #pragma unroll
         for (int d = 1; d < G; d <<= 1) {
-          const float s2 = __shfl_xor_sync(gm, ws, d), c2 = __shfl_xor_sync(gm, wc, d);
-          const int p2 = __shfl_xor_sync(gm, wp, d), h2 = __shfl_xor_sync(gm, wh, d), k2 = __shfl_xor_sync(gm, wk, d), t2 = __shfl_xor_sync(gm, wt, d);
-          if (before(s2, c2, p2, h2, ws, wc, wp, wh)) { ws = s2; wc = c2; wp = p2; wh = h2; wk = k2; wt = t2; }
+          const unsigned long long o1 = __shfl_xor_sync(gm, w1, d); const unsigned o2 = __shfl_xor_sync(gm, w2, d);
+          if (o1 < w1 || (o1 == w1 && o2 < w2)) { w1 = o1; w2 = o2; }
         }
-        if (!(ws > -INFINITY)) break;                         // pool exhausted (uniform in the group)
+        if (w1 == KEY_NONE) break;                            // pool exhausted (uniform in the group)
+        const int wp = (int)(w2 >> 28);
+        const int src = gbase + wp;
+        const int wk = __shfl_sync(gm, hk, src), wh = __shfl_sync(gm, hh, src), wt = __shfl_sync(gm, ht, src);
         if (sub == wp) { if (wk == 0) head++; else alt_avail = false; }      // the winner lane pops its head
         if (sub == r) { my_parent = wp; my_kind = wk; my_hit = wk == 0 ? wh : (wk == 1 ? -1 : -2); my_t = wt; }
         n_new = r + 1;
       }
+      if (sub < n_new) { sm.sel[tid] = my_parent | (my_kind << 3); sm.sel_t[tid] = my_t; sm.sel_hit[tid] = my_hit; }
     }
 
-    // ---- phase U: the new live set: the parent's state, updated with the hit ---------------------------------------
+    // ---- phase U: the chosen children, compacted over the CTA: the parent's state, updated with the hit --------------
+    const bool is_child = seed_act && !noop && sub < n_new;
+    {
+      const unsigned bal = __ballot_sync(0xffffffffu, is_child);
+      if (lane == 0) sm.wsum[warp] = __popc(bal);
+      __syncthreads();
+      int base = 0, tot = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < BT / 32; w2++) { const int c = sm.wsum[w2]; if (w2 < warp) base += c; tot += c; }
+      if (is_child) sm.plist[base + __popc(bal & ((1u << lane) - 1u))] = tid;
+      if (tid == 0) sm.nP = tot;
+      __syncthreads();
+    }
     KState S;
-    float c_chi2 = 0.f; int c_nh = 0, c_nm = 0, c_consec = 0;
-    bool live = seed_act && sub < n_new;
+    float c_chi2 = 0.f; int c_cnt = 0, cslot = -1, c_sel = 0, c_hit = 0;
     bool nan_child = false;
-    if (live) {
-      const int ps = (tid & ~(G - 1)) + my_parent;            // parent's slot
-      const int pcn = sm.cnt[ps];
-      c_chi2 = sm.chi2[ps]; c_nh = pcn & 0xff; c_nm = (pcn >> 8) & 0xff; c_consec = pcn >> 16;
-      if (my_kind == 2) ld_state(sm.A, ps, S);                // pass-through: the state does not move
-      else ld_state(sm.B, ps, S);
-      if (my_kind == 1) { c_nm++; c_consec++; }
-      else if (my_kind == 0) {
-        Hit H;
+    if (tid < sm.nP) {
+      cslot = sm.plist[tid];
+      c_sel = sm.sel[cslot]; c_hit = sm.sel_hit[cslot];
+      const int kind = (c_sel >> 3) & 3;
+      const int ps = (cslot & ~(G - 1)) + (c_sel & 7);        // parent's slot
+      Hit H;
+      if (kind == 0) {                                        // the hit's record first: its latency overlaps the state loads
         if (a.packed) {
-          const float4 q0 = __ldg(a.packed + my_t);
-          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * my_t;
+          const int t = sm.sel_t[cslot];
+          const float4 q0 = __ldg(a.packed + t);
+          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
           const float4 b = __ldg(cv), d = __ldg(cv + 1);
           H.x = q0.x; H.y = q0.y; H.z = q0.z;
           H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-        } else load_hit(H, a.hits, my_hit);
+        } else load_hit(H, a.hits, c_hit);
+      }
+      const int pcn = sm.cnt[ps];
+      c_chi2 = sm.chi2[ps];
+      int c_nh = pcn & 0xff, c_nm = (pcn >> 8) & 0xff, c_consec = pcn >> 16;
+      if (kind == 2) ld_state(sm.A, ps, S);                   // pass-through: the state does not move
+      else ld_state(sm.B, ps, S);
+      if (kind == 1) { c_nm++; c_consec++; }
+      else if (kind == 0) {
         SInv o; float c2;
         hit_to_local(S, H, o);
         if (COUNT) n_upd++;
         if (kalman_update(S, o, c2) && state_finite(S) && fabsf(c2) <= 3.0e38f) { c_chi2 += c2; c_nh++; c_consec = 0; }
-        else { live = false; nan_child = true; }              // dropped (C9 / R1)
+        else { nan_child = true; sm.sel[cslot] = c_sel | 256; }        // dropped (C9 / R1)
       }
+      c_cnt = c_nh | (c_nm << 8) | (c_consec << 16);
     }
     const bool any_nan = __syncthreads_or(nan_child);         // also: every read of A and B of this step is done
     if (any_nan) {
-     if (seed_act) {
       // R1: the parent of a dropped child, as it stood before the layer, is offered to best_short (after the offers
       // above, in child rank order; strict comparison with the holder)
-      const int ps = (tid & ~(G - 1)) + my_parent;
-      const int pcn = sm.cnt[ps];
-      const int pnh = pcn & 0xff, pnm = (pcn >> 8) & 0xff;
-      const float pchi2 = sm.chi2[ps];
-      float os = (nan_child && pnh >= p.min_hits_keep) ? score_of(p, pnh, pnm, pchi2) : -INFINITY, oc = pchi2; int ol = sub;
+      if (seed_act && !noop) {
+        const bool dead = sub < n_new && (sm.sel[tid] & 256);
+        const int ps = (tid & ~(G - 1)) + my_parent;
+        const int pcn = sm.cnt[ps];
+        const int pnh = pcn & 0xff, pnm = (pcn >> 8) & 0xff;
+        const float pchi2 = sm.chi2[ps];
+        float os = (dead && pnh >= p.min_hits_keep) ? score_of(p, pnh, pnm, pchi2) : -INFINITY, oc = pchi2; int ol = sub;
 #pragma unroll
-      for (int d = 1; d < G; d <<= 1) {
-        const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
-        const int l2 = __shfl_xor_sync(gm, ol, d);
-        const bool take = (s2 != os) ? (s2 > os) : ((c2 != oc) ? (c2 < oc) : (l2 < ol));
-        if (take) { os = s2; oc = c2; ol = l2; }
+        for (int d = 1; d < G; d <<= 1) {
+          const float s2 = __shfl_xor_sync(gm, os, d), c2 = __shfl_xor_sync(gm, oc, d);
+          const int l2 = __shfl_xor_sync(gm, ol, d);
+          const bool take = (s2 != os) ? (s2 > os) : ((c2 != oc) ? (c2 < oc) : (l2 < ol));
+          if (take) { os = s2; oc = c2; ol = l2; }
+        }
+        if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
+          const int src = gbase + ol;
+          if (sub == ol) { KState Sp; ld_state(sm.A, ps, Sp); store_state(Sp, a.par_out, a.cov_out, n, (size_t)i); }
+          bs_have = true; bs_score = os; bs_chi2 = oc;
+          bs_nh = __shfl_sync(gm, pnh, src); bs_nm = __shfl_sync(gm, pnm, src);
+          bs_stat = 0;
+          bs_step = s; bs_parent = __shfl_sync(gm, my_parent, src); bs_last = -2;
+        }
       }
-      if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
-        const int src = gbase + ol;
-        if (sub == ol) { KState Sp; ld_state(sm.A, ps, Sp); store_state(Sp, a.par_out, a.cov_out, n, (size_t)i); }
-        bs_have = true; bs_score = os; bs_chi2 = oc;
-        bs_nh = __shfl_sync(gm, pnh, src); bs_nm = __shfl_sync(gm, pnm, src);
-        bs_stat = 0;
-        bs_step = s; bs_parent = __shfl_sync(gm, my_parent, src); bs_last = -2;
-      }
-     }
       __syncthreads();                                        // the parents' states have been read
     }
+    if (cslot >= 0 && !nan_child) {                           // the child becomes live candidate `rank` of its seed
+      st_state(sm.A, cslot, S);
+      sm.chi2[cslot] = c_chi2; sm.cnt[cslot] = c_cnt;
+      const int si = sm.seed[cslot >> 3];
+      a.trellis[((size_t)si * mpl + s) * G + (cslot & (G - 1))] = (unsigned)(c_hit + 2) | ((unsigned)(c_sel & 7) << 28);
+    }
     if (seed_act) {
-      // the live children, contiguous in rank order
-      const unsigned alive = (__ballot_sync(gm, live) >> gbase) & 0xffu;
-      if (live) {
-        const int dst = (tid & ~(G - 1)) + __popc(alive & ((1u << sub) - 1u));
-        st_state(sm.A, dst, S);
-        sm.chi2[dst] = c_chi2; sm.cnt[dst] = c_nh | (c_nm << 8) | (c_consec << 16);
-        trellis[(size_t)s * G + (dst & (G - 1))] = (unsigned)(my_hit + 2) | ((unsigned)my_parent << 28);
-      }
-      if (sub == 0) sm.n_live[sl] = __popc(alive);
+      if (noop) { if (parent_live) trellis[(size_t)s * G + sub] = (unsigned)sub << 28; }        // hit code 0 == -2 (not crossed)
+      else if (sub == 0) sm.n_live[sl] = n_new;
       t_last = s;
+    }
+    if (any_nan) {
+      // dropped children leave holes in the new live set: close them, keeping the rank order (rare)
+      __syncthreads();
+      if (seed_act && !noop) {
+        const unsigned alive = (__ballot_sync(gm, sub < n_new && !(sm.sel[tid] & 256)) >> gbase) & 0xffu;
+        if (alive != ((1u << n_new) - 1u)) {
+          const int cntl = __popc(alive);
+          const int srcl = sub < cntl ? (int)__fns(alive, 0, sub + 1) : sub;
+          const int from = (tid & ~(G - 1)) + srcl;
+          KState Sm; ld_state(sm.A, from, Sm);
+          const float mchi2 = sm.chi2[from]; const int mcnt = sm.cnt[from];
+          const unsigned ent = (unsigned)(sm.sel_hit[from] + 2) | ((unsigned)(sm.sel[from] & 7) << 28);
+          __syncwarp(gm);
+          if (sub < cntl) {
+            st_state(sm.A, tid, Sm); sm.chi2[tid] = mchi2; sm.cnt[tid] = mcnt;
+            trellis[(size_t)s * G + sub] = ent;
+          }
+          if (sub == 0) sm.n_live[sl] = cntl;
+        }
+      }
     }
     __syncthreads();
   }
@@ -637,7 +731,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     float o_chi2, o_score; int o_nh, o_nm, bt_step, bt_slot, tail_step = -1, tail_val = -2; unsigned o_stat;
     if (live_wins) {
       const int src = gbase + fl2;
-      if (sub == fl2) { KState S; ld_state(sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
+      if (sub == fl2) { KState Sf; ld_state(sm.A, tid, Sf); store_state(Sf, a.par_out, a.cov_out, n, (size_t)i); }
       o_chi2 = fc; o_score = fs;
       o_nh = __shfl_sync(gm, nh, src); o_nm = __shfl_sync(gm, nm, src); o_stat = 0;
       bt_step = t_last; bt_slot = fl2;
@@ -650,13 +744,30 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     }
     if (sub == 0) {
       a.chi2[i] = o_chi2; a.score[i] = o_score; a.nhits[i] = o_nh; a.nmiss[i] = o_nm; a.status[i] = o_stat;
-      int slot = bt_slot;
-      for (int s = mpl - 1; s >= 0; s--) {
-        int v = -2;
-        if (s == tail_step) v = tail_val;
-        else if (s <= bt_step) { const unsigned e = trellis[(size_t)s * G + slot]; v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28); }
-        a.hit_ids[(size_t)s * n + i] = v;
+    }
+    // the winner's hit list: the 8 lanes bring the seed's trellis into shared memory (the propagated states are dead by
+    // now), lane 0 walks it backwards, the 8 lanes write the plan steps
+    const bool staged = (size_t)mpl * G * NS <= (size_t)NF * SL;
+    unsigned* tsm = reinterpret_cast<unsigned*>(&sm.B[0][0]) + (size_t)sl * mpl * G;
+    if (staged) {
+      for (int s = 0; s <= max(bt_step, 0) && s < mpl; s++) tsm[s * G + sub] = trellis[(size_t)s * G + sub];
+      __syncwarp(gm);
+    }
+    int slot = bt_slot;
+    for (int s0 = ((mpl - 1) / G) * G; s0 >= 0; s0 -= G) {
+      int mine = -2;
+      if (sub == 0) {
+        for (int s = min(s0 + G, mpl) - 1; s >= s0; s--) {
+          int v = -2;
+          if (s == tail_step) v = tail_val;
+          else if (s <= bt_step) { const unsigned e = staged ? tsm[s * G + slot] : trellis[(size_t)s * G + slot]; v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28); }
+          sm.sel_t[(tid & ~(G - 1)) + (s - s0)] = v;
+        }
       }
+      __syncwarp(gm);
+      if (s0 + sub < mpl) mine = sm.sel_t[(tid & ~(G - 1)) + sub];
+      __syncwarp(gm);
+      if (s0 + sub < mpl) a.hit_ids[(size_t)(s0 + sub) * n + i] = mine;
     }
   }
   if (COUNT) {

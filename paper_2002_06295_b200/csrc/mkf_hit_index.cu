@@ -9,6 +9,12 @@
 //                     order the atomics ran in;
 //   5. hi_pack      : the hits in sorted order, positions (16 B) and covariances (32 B) in two contiguous blocks,
 //                     so that a bin scan reads contiguous memory.
+// That five-kernel path serves the masked index (R9) and bin grids too large for shared memory. The plain index runs
+// as ONE kernel, hi_fused_kernel (one CTA per segment): the hits of a segment occupy the same range of positions before
+// and after sorting, so its bin offsets are layer_off + a prefix over the segment's own bins, computed in shared
+// memory; each warp owns a contiguous range of the segment's ids, counts its keys per bin, and after the prefix places
+// its hits with a warp-local rank (match.any), which makes the order inside a bin ascending in id without a sort;
+// the packed records are written in the same pass, so every hit is read once from HBM (the second pass hits L2).
 // HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
 #include "mkf_ctx.h"
 #include "mkf_scan.cuh"
@@ -136,6 +142,121 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
   o[1] = make_float4(V[4 * nh + id], V[5 * nh + id], 0.f, 0.f);
 }
 
+
+// ---- the plain index in one kernel ------------------------------------------------------------------------------------
+constexpr int HF_BLOCK = 128, HF_WARPS = HF_BLOCK / 32;
+
+// Bin key of a hit, identical to the fp64 evaluation of C8 (U12): fp32 first; the fp64 formulas only when the fp32
+// value lies within 1e-3 bin widths of a bin edge (fp32 atan2f / asinhf are good to a few 1e-7 in value, 2e-5 in bin
+// units, so outside that margin both evaluations floor to the same bin).
+__device__ __forceinline__ int bin_key(float xf, float yf, float zf, float elo_f, float ehi_f, int n_phi, int n_eta) {
+  const float PI = 3.14159265358979323846f;
+  const float bp = (atan2f(yf, xf) + PI) * ((float)n_phi * (1.f / (2.f * PI)));
+  const float be = (asinhf(zf * rsqrtf(fmaf(xf, xf, yf * yf))) - elo_f) * ((float)n_eta / (ehi_f - elo_f));
+  int ip, ie;
+  if (fabsf(bp - rintf(bp)) > 1e-3f && bp > 0.f && bp < (float)n_phi) ip = (int)bp;
+  else ip = phi_bin_d(atan2((double)yf, (double)xf), n_phi);
+  if (fabsf(be - rintf(be)) > 1e-3f && be > 0.f && be < (float)n_eta) ie = (int)be;
+  else if (be < -1.f) ie = 0;
+  else if (be > (float)n_eta + 1.f) ie = n_eta - 1;
+  else {
+    const double x = (double)xf, y = (double)yf, z = (double)zf;
+    ie = eta_bin_d(asinh(z / sqrt(x * x + y * y)), (double)elo_f, (double)ehi_f, n_eta);
+  }
+  return ie * n_phi + ip;
+}
+
+__global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
+  extern __shared__ unsigned hf_sm[];                         // cntw[HF_WARPS][nb], tot[nb]
+  __shared__ float s_xy[HF_WARPS], s_zz[HF_WARPS];
+  __shared__ unsigned s_ws[HF_WARPS];
+  const int seg = blockIdx.x;
+  const int nb = a.n_phi * a.n_eta;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
+  const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
+  unsigned* cntw = hf_sm + (size_t)w * nb;
+  unsigned* tot = hf_sm + (size_t)HF_WARPS * nb;
+  for (int k = tid; k < (HF_WARPS + 1) * nb; k += HF_BLOCK) hf_sm[k] = 0u;
+  __syncthreads();
+  const float elo = g.layers[l].eta_lo, ehi = g.layers[l].eta_hi;
+  const size_t nh = (size_t)a.hits.n_hits;
+  // each warp owns a contiguous range of the segment's ids (a multiple of 32 long, so that its loads stay aligned)
+  const int per = ((e - b + HF_WARPS - 1) / HF_WARPS + 31) & ~31;
+  const int wb = min(b + w * per, e), we = min(wb + per, e);
+  float vxy = 0.f, vzz = 0.f;
+  for (int i = wb + lane; i < we; i += 32) {
+    const int key = bin_key(a.hits.x[i], a.hits.y[i], a.hits.z[i], elo, ehi, a.n_phi, a.n_eta);
+    a.key[i] = key;
+    atomicAdd(&cntw[key], 1u);
+    // larger eigenvalue of the xy block of V in round-to-nearest fp32 without contraction (bit-exact with C8)
+    const float vxx = a.hits.V[i], vxyv = a.hits.V[nh + i], vyy = a.hits.V[2 * nh + i];
+    const float hs = __fmul_rn(0.5f, __fadd_rn(vxx, vyy)), hd = __fmul_rn(0.5f, __fsub_rn(vxx, vyy));
+    const float ev1 = __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(vxyv, vxyv))));
+    vxy = fmaxf(vxy, ev1);
+    vzz = fmaxf(vzz, a.hits.V[5 * nh + i]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    vxy = fmaxf(vxy, __shfl_xor_sync(0xffffffffu, vxy, o));
+    vzz = fmaxf(vzz, __shfl_xor_sync(0xffffffffu, vzz, o));
+  }
+  if (lane == 0) { s_xy[w] = vxy; s_zz[w] = vzz; }
+  __syncthreads();
+  if (tid == 0) {
+    for (int k = 1; k < HF_WARPS; k++) { vxy = fmaxf(vxy, s_xy[k]); vzz = fmaxf(vzz, s_zz[k]); }
+    a.vmax[2 * (size_t)seg] = vxy; a.vmax[2 * (size_t)seg + 1] = vzz;
+  }
+  // per bin: the warps' counts become their offsets inside the bin; tot = hits of the bin
+  for (int k = tid; k < nb; k += HF_BLOCK) {
+    unsigned run = 0;
+#pragma unroll
+    for (int q = 0; q < HF_WARPS; q++) { const unsigned c = hf_sm[(size_t)q * nb + k]; hf_sm[(size_t)q * nb + k] = run; run += c; }
+    tot[k] = run;
+  }
+  __syncthreads();
+  // exclusive prefix of tot over the bins (blocked: thread t owns bins [t * pb, (t + 1) * pb))
+  {
+    const int pb = (nb + HF_BLOCK - 1) / HF_BLOCK;
+    const int k0 = min(tid * pb, nb), k1 = min(k0 + pb, nb);
+    unsigned sum = 0;
+    for (int k = k0; k < k1; k++) sum += tot[k];
+    unsigned inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
+    if (lane == 31) s_ws[w] = inc;
+    __syncthreads();
+    unsigned base = 0;
+    for (int q = 0; q < w; q++) base += s_ws[q];
+    unsigned run = base + inc - sum;
+    unsigned* bo = a.bin_off + (size_t)seg * nb;
+    for (int k = k0; k < k1; k++) { const unsigned c = tot[k]; tot[k] = run; bo[k] = (unsigned)b + run; run += c; }
+    if (seg == gridDim.x - 1 && tid == 0) a.bin_off[a.n_bins] = (unsigned)a.hits.n_hits;
+  }
+  __syncthreads();
+  // placement: ids of a warp ascend with the lane and with the iteration, warps own ascending ranges -> stable
+  const float* V = a.hits.V;
+  for (int i0 = wb; i0 < we; i0 += 32) {
+    const int i = i0 + lane;
+    const bool valid = i < we;
+    const int key = valid ? a.key[i] : -1 - lane;
+    const unsigned m = __match_any_sync(0xffffffffu, key);
+    const int leader = __ffs(m) - 1;
+    unsigned base = 0;
+    if (valid && lane == leader) { base = cntw[key]; cntw[key] = base + __popc(m); }
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (!valid) continue;
+    const unsigned t = (unsigned)b + tot[key] + base + __popc(m & ((1u << lane) - 1u));
+    a.sorted_id[t] = i;
+    if (a.packed) {
+      a.packed[t] = make_float4(a.hits.x[i], a.hits.y[i], a.hits.z[i], __int_as_float(i));
+      float4* o = a.packed + nh + (size_t)2 * t;
+      o[0] = make_float4(V[i], V[nh + i], V[2 * nh + i], V[3 * nh + i]);
+      o[1] = make_float4(V[4 * nh + i], V[5 * nh + i], 0.f, 0.f);
+    }
+  }
+}
+
 }  // namespace
 
 namespace mkf {
@@ -170,6 +291,22 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
   unsigned* partial = (unsigned*)w;
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
   a.mask = mask; a.n_bins = nbins;
+  const size_t fused_smem = (size_t)(HF_WARPS + 1) * c->g.n_phi * c->g.n_eta * 4;
+  if (!mask && fused_smem <= 200 * 1024) {
+    if (h->n_hits == 0) {                                      // nothing to place: all offsets are zero
+      cudaError_t e0 = cudaMemsetAsync(a.bin_off, 0, (nbins + 1) * 4, st);
+      if (e0 == cudaSuccess) e0 = cudaMemsetAsync(a.vmax, 0, (size_t)nseg * 8, st);
+      if (e0 != cudaSuccess) return cuda_fail(c, e0, "mkf_build_hit_index: memset");
+      return MKF_OK;
+    }
+    if (fused_smem > 48 * 1024) {
+      cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
+      if (e1 != cudaSuccess) return cuda_fail(c, e1, "mkf_build_hit_index: shared memory attribute");
+    }
+    hi_fused_kernel<<<nseg, HF_BLOCK, fused_smem, st>>>(c->g, a);
+    MKF_LAUNCHED(c, "hi_fused_kernel");
+    return MKF_OK;
+  }
   cudaError_t e = cudaMemsetAsync(a.cnt, 0, nbins * 4, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_hit_index: memset");
   hi_key_count<<<nseg, HI_BLOCK, 0, st>>>(c->g, a);
