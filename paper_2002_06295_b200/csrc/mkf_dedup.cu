@@ -33,21 +33,19 @@ __global__ void __launch_bounds__(DD_BLOCK) dd_fill(const __grid_constant__ DdAr
   if (h >= 0 && h < a.n_hits) a.list[atomicAdd(&a.cnt[h], 1u)] = (int)(k % (size_t)a.n);
 }
 
-__global__ void __launch_bounds__(DD_BLOCK) dd_mark(const __grid_constant__ DdArgs a) {
-  const int i = blockIdx.x * DD_BLOCK + threadIdx.x;
-  if (i >= a.n) return;
-  // event of track i: last ev with track_off[ev] <= i
-  int lo = 0, hi = a.n_events;
-  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (a.track_off[mid] <= i) lo = mid; else hi = mid; }
-  const int eb = a.track_off[lo], ee = a.track_off[lo + 1];
+// |ids_i ∩ ids_j| is the number of times j appears in the lists filed under the hits of i (a hit appears at most once
+// in a track), so one warp per track gathers those lists into shared memory and counts multiplicities: with at most 32
+// entries one match.any does it. Tracks whose lists hold more than DD_CAP entries take the plain loop (lane 0).
+constexpr int DD_CAP = 128, DD_WARPS = DD_BLOCK / 32;
+
+__device__ bool dd_dominated_slow(const DdArgs& a, int i, int eb, int ee) {
   const size_t n = (size_t)a.n;
   const int nhi = a.nhits[i];
   const float si = a.score[i];
-  bool removed = false;
-  for (int s = 0; s < a.mpl && !removed; s++) {
+  for (int s = 0; s < a.mpl; s++) {
     const int h = a.hit_ids[(size_t)s * n + i];
     if (h < 0 || h >= a.n_hits) continue;
-    for (unsigned t = a.off[h]; t < a.off[h + 1] && !removed; t++) {
+    for (unsigned t = a.off[h]; t < a.off[h + 1]; t++) {
       const int j = a.list[t];
       if (j == i || j < eb || j >= ee) continue;
       const float sj = a.score[j];
@@ -60,10 +58,65 @@ __global__ void __launch_bounds__(DD_BLOCK) dd_mark(const __grid_constant__ DdAr
         if (hc < 0) continue;
         for (int d = 0; d < a.mpl; d++) if (a.hit_ids[(size_t)d * n + i] == hc) { shared++; break; }
       }
-      if ((double)shared > (double)a.dup_frac * (double)mn) removed = true;
+      if ((double)shared > (double)a.dup_frac * (double)mn) return true;
     }
   }
-  a.keep[i] = removed ? 0 : 1;
+  return false;
+}
+
+__global__ void __launch_bounds__(DD_BLOCK) dd_mark(const __grid_constant__ DdArgs a) {
+  __shared__ int s_e[DD_WARPS][DD_CAP];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int i = blockIdx.x * DD_WARPS + w;
+  if (i >= a.n) return;                                       // whole warp
+  int* E = s_e[w];
+  // event of track i: last ev with track_off[ev] <= i
+  int lo = 0, hi = a.n_events;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (a.track_off[mid] <= i) lo = mid; else hi = mid; }
+  const int eb = a.track_off[lo], ee = a.track_off[lo + 1];
+  const size_t n = (size_t)a.n;
+  int total = 0;
+  for (int s0 = 0; s0 < a.mpl; s0 += 32) {
+    const int s = s0 + lane;
+    int h = -1;
+    if (s < a.mpl) h = a.hit_ids[(size_t)s * n + i];
+    unsigned b = 0; int len = 0;
+    if (h >= 0 && h < a.n_hits) { b = a.off[h]; len = (int)(a.off[h + 1] - b); }
+    int inc = len;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
+    const int pos = total + inc - len;
+    for (int k = 0; k < len; k++) if (pos + k < DD_CAP) E[pos + k] = a.list[b + k];
+    total += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  __syncwarp();
+  bool removed = false;
+  if (total > DD_CAP) { if (lane == 0) removed = dd_dominated_slow(a, i, eb, ee); }
+  else {
+    const int nhi = a.nhits[i];
+    const float si = a.score[i];
+    for (int e0 = 0; e0 < total; e0 += 32) {
+      const int e = e0 + lane;
+      const int j = e < total ? E[e] : -1 - lane;
+      int m; bool first;
+      if (total <= 32) {
+        const unsigned mm = __match_any_sync(0xffffffffu, j);
+        m = __popc(mm); first = (__ffs(mm) - 1) == lane;
+      } else {
+        m = 0; first = true;
+        for (int q = 0; q < total; q++) { const bool eq = E[q] == j; m += eq; if (eq && q < e) first = false; }
+      }
+      if (e < total && first && j != i && j >= eb && j < ee) {
+        const float sj = a.score[j];
+        if (sj > si || (sj == si && j < i)) {                 // j ranks higher
+          const int mn = min(nhi, a.nhits[j]);
+          if (mn > 0 && (double)m > (double)a.dup_frac * (double)mn) removed = true;
+        }
+      }
+    }
+  }
+  removed = __any_sync(0xffffffffu, removed);
+  if (lane == 0) a.keep[i] = removed ? 0 : 1;
 }
 
 __global__ void __launch_bounds__(DD_BLOCK) dd_count_kept(const __grid_constant__ DdArgs a) {
@@ -115,7 +168,7 @@ extern "C" int mkf_remove_duplicates(mkf_ctx* c, int n_events, int n, int n_hits
     { const int rc = exclusive_scan_u32(c, a.cnt, (size_t)n_hits + 1, partial, a.off, 0u, st); if (rc) return rc; }
     dd_fill<<<grid, DD_BLOCK, 0, st>>>(a);
     MKF_LAUNCHED(c, "dd_fill");
-    dd_mark<<<(n + DD_BLOCK - 1) / DD_BLOCK, DD_BLOCK, 0, st>>>(a);
+    dd_mark<<<(n + DD_WARPS - 1) / DD_WARPS, DD_BLOCK, 0, st>>>(a);
     MKF_LAUNCHED(c, "dd_mark");
   }
   dd_count_kept<<<n_events, DD_BLOCK, 0, st>>>(a);

@@ -12,9 +12,9 @@
 // That five-kernel path serves the masked index (R9) and bin grids too large for shared memory. The plain index runs
 // as ONE kernel, hi_fused_kernel (one CTA per segment): the hits of a segment occupy the same range of positions before
 // and after sorting, so its bin offsets are layer_off + a prefix over the segment's own bins, computed in shared
-// memory; each warp owns a contiguous range of the segment's ids, counts its keys per bin, and after the prefix places
-// its hits with a warp-local rank (match.any), which makes the order inside a bin ascending in id without a sort;
-// the packed records are written in the same pass, so every hit is read once from HBM (the second pass hits L2).
+// memory (10 KB for 63 x 40 bins: the occupancy is bounded by threads, not by shared memory); ids are scattered with
+// an atomic cursor, each bin's few ids are then put in ascending order, and every hit writes its packed record at the
+// place it finds for its id in its bin; the segment is read from HBM once (the later passes hit L2).
 // HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
 #include "mkf_ctx.h"
 #include "mkf_scan.cuh"
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
 
 
 // ---- the plain index in one kernel ------------------------------------------------------------------------------------
-constexpr int HF_BLOCK = 128, HF_WARPS = HF_BLOCK / 32;
+constexpr int HF_BLOCK = 256, HF_WARPS = HF_BLOCK / 32;
 
 // Bin key of a hit, identical to the fp64 evaluation of C8 (U12): fp32 first; the fp64 formulas only when the fp32
 // value lies within 1e-3 bin widths of a bin edge (fp32 atan2f / asinhf are good to a few 1e-7 in value, 2e-5 in bin
@@ -166,8 +166,14 @@ __device__ __forceinline__ int bin_key(float xf, float yf, float zf, float elo_f
   return ie * n_phi + ip;
 }
 
+// One CTA per segment, bin counts of the segment in shared memory:
+//   A  key per hit (kept in the workspace), count per bin, per-segment max hit variances;
+//   -  exclusive prefix over the segment's bins -> bin_off (= layer_off + prefix) and the scatter cursors;
+//   B  ids scattered to their bins (atomic cursor: any order inside a bin);
+//   -  each bin's ids sorted ascending: the unique stable order of C8;
+//   C  every hit finds its place in its bin and writes its packed record there (reads in id order: coalesced).
 __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
-  extern __shared__ unsigned hf_sm[];                         // cntw[HF_WARPS][nb], tot[nb]
+  extern __shared__ unsigned hf_cnt[];                        // [nb] counts, then cursors
   __shared__ float s_xy[HF_WARPS], s_zz[HF_WARPS];
   __shared__ unsigned s_ws[HF_WARPS];
   const int seg = blockIdx.x;
@@ -175,26 +181,22 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
   const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
-  unsigned* cntw = hf_sm + (size_t)w * nb;
-  unsigned* tot = hf_sm + (size_t)HF_WARPS * nb;
-  for (int k = tid; k < (HF_WARPS + 1) * nb; k += HF_BLOCK) hf_sm[k] = 0u;
+  for (int k = tid; k < nb; k += HF_BLOCK) hf_cnt[k] = 0u;
   __syncthreads();
   const float elo = g.layers[l].eta_lo, ehi = g.layers[l].eta_hi;
   const size_t nh = (size_t)a.hits.n_hits;
-  // each warp owns a contiguous range of the segment's ids (a multiple of 32 long, so that its loads stay aligned)
-  const int per = ((e - b + HF_WARPS - 1) / HF_WARPS + 31) & ~31;
-  const int wb = min(b + w * per, e), we = min(wb + per, e);
+  const float* V = a.hits.V;
   float vxy = 0.f, vzz = 0.f;
-  for (int i = wb + lane; i < we; i += 32) {
+  for (int i = b + tid; i < e; i += HF_BLOCK) {
     const int key = bin_key(a.hits.x[i], a.hits.y[i], a.hits.z[i], elo, ehi, a.n_phi, a.n_eta);
     a.key[i] = key;
-    atomicAdd(&cntw[key], 1u);
+    atomicAdd(&hf_cnt[key], 1u);
     // larger eigenvalue of the xy block of V in round-to-nearest fp32 without contraction (bit-exact with C8)
-    const float vxx = a.hits.V[i], vxyv = a.hits.V[nh + i], vyy = a.hits.V[2 * nh + i];
+    const float vxx = V[i], vxyv = V[nh + i], vyy = V[2 * nh + i];
     const float hs = __fmul_rn(0.5f, __fadd_rn(vxx, vyy)), hd = __fmul_rn(0.5f, __fsub_rn(vxx, vyy));
     const float ev1 = __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(vxyv, vxyv))));
     vxy = fmaxf(vxy, ev1);
-    vzz = fmaxf(vzz, a.hits.V[5 * nh + i]);
+    vzz = fmaxf(vzz, V[5 * nh + i]);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -207,20 +209,12 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
     for (int k = 1; k < HF_WARPS; k++) { vxy = fmaxf(vxy, s_xy[k]); vzz = fmaxf(vzz, s_zz[k]); }
     a.vmax[2 * (size_t)seg] = vxy; a.vmax[2 * (size_t)seg + 1] = vzz;
   }
-  // per bin: the warps' counts become their offsets inside the bin; tot = hits of the bin
-  for (int k = tid; k < nb; k += HF_BLOCK) {
-    unsigned run = 0;
-#pragma unroll
-    for (int q = 0; q < HF_WARPS; q++) { const unsigned c = hf_sm[(size_t)q * nb + k]; hf_sm[(size_t)q * nb + k] = run; run += c; }
-    tot[k] = run;
-  }
-  __syncthreads();
-  // exclusive prefix of tot over the bins (blocked: thread t owns bins [t * pb, (t + 1) * pb))
+  // exclusive prefix of the counts over the bins (blocked: thread t owns bins [t * pb, (t + 1) * pb))
   {
     const int pb = (nb + HF_BLOCK - 1) / HF_BLOCK;
     const int k0 = min(tid * pb, nb), k1 = min(k0 + pb, nb);
     unsigned sum = 0;
-    for (int k = k0; k < k1; k++) sum += tot[k];
+    for (int k = k0; k < k1; k++) sum += hf_cnt[k];
     unsigned inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const unsigned t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
@@ -228,32 +222,42 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
     __syncthreads();
     unsigned base = 0;
     for (int q = 0; q < w; q++) base += s_ws[q];
-    unsigned run = base + inc - sum;
+    unsigned run = (unsigned)b + base + inc - sum;
     unsigned* bo = a.bin_off + (size_t)seg * nb;
-    for (int k = k0; k < k1; k++) { const unsigned c = tot[k]; tot[k] = run; bo[k] = (unsigned)b + run; run += c; }
+    for (int k = k0; k < k1; k++) { const unsigned c = hf_cnt[k]; hf_cnt[k] = run; bo[k] = run; run += c; }
     if (seg == gridDim.x - 1 && tid == 0) a.bin_off[a.n_bins] = (unsigned)a.hits.n_hits;
   }
   __syncthreads();
-  // placement: ids of a warp ascend with the lane and with the iteration, warps own ascending ranges -> stable
-  const float* V = a.hits.V;
-  for (int i0 = wb; i0 < we; i0 += 32) {
-    const int i = i0 + lane;
-    const bool valid = i < we;
-    const int key = valid ? a.key[i] : -1 - lane;
-    const unsigned m = __match_any_sync(0xffffffffu, key);
-    const int leader = __ffs(m) - 1;
-    unsigned base = 0;
-    if (valid && lane == leader) { base = cntw[key]; cntw[key] = base + __popc(m); }
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (!valid) continue;
-    const unsigned t = (unsigned)b + tot[key] + base + __popc(m & ((1u << lane) - 1u));
-    a.sorted_id[t] = i;
-    if (a.packed) {
-      a.packed[t] = make_float4(a.hits.x[i], a.hits.y[i], a.hits.z[i], __int_as_float(i));
-      float4* o = a.packed + nh + (size_t)2 * t;
-      o[0] = make_float4(V[i], V[nh + i], V[2 * nh + i], V[3 * nh + i]);
-      o[1] = make_float4(V[4 * nh + i], V[5 * nh + i], 0.f, 0.f);
+  for (int i = b + tid; i < e; i += HF_BLOCK) a.sorted_id[atomicAdd(&hf_cnt[a.key[i]], 1u)] = i;
+  __syncthreads();                                            // cursor[k] is now the end of bin k
+  for (int k = tid; k < nb; k += HF_BLOCK) {
+    const unsigned kb = k == 0 ? (unsigned)b : hf_cnt[k - 1], ke = hf_cnt[k];
+    const int len = (int)(ke - kb);
+    if (len < 2) continue;
+    int* v = a.sorted_id + kb;
+    if (len == 2) { const int x0 = v[0], x1 = v[1]; if (x0 > x1) { v[0] = x1; v[1] = x0; } continue; }
+    for (int q = 1; q < len; q++) {                           // insertion sort (a handful of ids; crowded bins are O(len^2))
+      const int x = v[q];
+      int j = q - 1;
+      while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; j--; }
+      v[j + 1] = x;
     }
+  }
+  if (!a.packed) return;
+  __syncthreads();
+  for (int i = b + tid; i < e; i += HF_BLOCK) {
+    const int key = a.key[i];
+    unsigned t = key == 0 ? (unsigned)b : hf_cnt[key - 1];
+    const unsigned te = hf_cnt[key];
+    if (te - t > 8u) {                                        // crowded bin: binary search of the ascending ids
+      unsigned lo = t, hi = te;
+      while (hi - lo > 1u) { const unsigned mid = (lo + hi) >> 1; if (a.sorted_id[mid] <= i) lo = mid; else hi = mid; }
+      t = lo;
+    } else while (a.sorted_id[t] != i) t++;
+    a.packed[t] = make_float4(a.hits.x[i], a.hits.y[i], a.hits.z[i], __int_as_float(i));
+    float4* o = a.packed + nh + (size_t)2 * t;
+    o[0] = make_float4(V[i], V[nh + i], V[2 * nh + i], V[3 * nh + i]);
+    o[1] = make_float4(V[4 * nh + i], V[5 * nh + i], 0.f, 0.f);
   }
 }
 
@@ -291,7 +295,7 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
   unsigned* partial = (unsigned*)w;
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
   a.mask = mask; a.n_bins = nbins;
-  const size_t fused_smem = (size_t)(HF_WARPS + 1) * c->g.n_phi * c->g.n_eta * 4;
+  const size_t fused_smem = (size_t)c->g.n_phi * c->g.n_eta * 4;
   if (!mask && fused_smem <= 200 * 1024) {
     if (h->n_hits == 0) {                                      // nothing to place: all offsets are zero
       cudaError_t e0 = cudaMemsetAsync(a.bin_off, 0, (nbins + 1) * 4, st);
