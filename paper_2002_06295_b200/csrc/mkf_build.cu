@@ -34,10 +34,9 @@ constexpr int NS = MKF_BUILD_NS;     // seeds per CTA
 constexpr int SL = NS * G;           // candidate slots per CTA
 constexpr int BT = SL;               // threads per CTA: one per slot
 constexpr int LC = 8;                // accepted hits kept per candidate and layer (a seed keeps at most MAX_CAND children)
-#ifndef MKF_BUILD_SCAN_G
-#define MKF_BUILD_SCAN_G 4
-#endif
-constexpr int SCAN_G = MKF_BUILD_SCAN_G;   // lanes that walk one eta row of a window together
+constexpr int ROWCAP = 24 * NS;        // row parts (contiguous runs of hits) in the CTA's table per scan round
+constexpr int SQCAP = 48 * NS;        // survivors of the position test queued per scan pass (= hits looked at per pass)
+constexpr int RUN_MAX = (1 << 22) - 1; // longest run of hits in one table entry (queue entries hold run << 22 | offset)
 constexpr int HIT_NONE = 0x7fffffff; // "hit id" of miss / pass-through children in the order U14
 static_assert(G == MAX_CAND, "one slot per candidate");
 static_assert(BT % 32 == 0 && BT <= 1024, "CTA size");
@@ -63,26 +62,26 @@ struct BuildArgs {
   unsigned long long* counters;
 };
 
-constexpr int OVC = 256;             // CTA-wide overflow list of accepted hits beyond a candidate's LC entries
-
 struct Smem {
   float A[NF][SL];          // live candidates as they stand before this layer
   float B[NF][SL];          // the same candidates propagated to this layer (material applied)
   float chi2[SL]; int cnt[SL];                     // cnt = nhits | nmiss << 8 | consec << 16
-  float tt[SL], tz[SL], zz[SL], lim1[SL], lim2[SL];
-  int wrow[SL], wphi[SL];   // window: e0 | n_rows << 8 ; w0 | wn << 8
+  float tt[SL], tz[SL], zz[SL], lim1[SL], lim2[SL];          // lim = (variance bound of the residual) x 1.0001: r^2 > cut x lim rejects
   int flag[SL]; unsigned ostat[SL];
-  int rowpre[SL + 1];
-  int lcount[SL];
-  unsigned long long lkey[LC][SL];                 // chi2 bits << 32 | hit id: ascending = the order U14 within a parent
-  int lt[LC][SL];                                  // position of the hit in the packed arrays
-  unsigned long long ovf_key[OVC]; int ovf_t[OVC]; int ovf_slot[OVC]; int ovf_n;
+  uint2 rows[ROWCAP]; int n_rows, more;                       // runs of hits to scan: (slot | n << 8, first position); more: a window has rows left
+  int runpre[ROWCAP + 1];                                     // exclusive prefix of the runs' lengths: the hits of a round as one list
+  unsigned sq[SQCAP]; int sq_n;                               // survivors of the position test: run << 22 | offset in the run
+  int wrow[SL], wphi[SL];                                     // window: next row | end row << 8 ; w0 | wn << 8
+  unsigned long long lkey[LC][SL];                 // the LC best hits of the candidate on this layer, ascending:
+                                                   // chi2 bits << 32 | position t of the hit in the sorted index
   int sel[SL], sel_t[SL], sel_hit[SL];             // the children picked for the new live set: parent | kind << 3 | dead << 8
   int plist[SL]; int nP;
   int wsum[BT / 32];
   int n_live[NS], p0[NS], plen[NS], ev[NS], last[NS], seed[NS];
   float aq[NS];
 };
+
+static_assert((sizeof(Smem) + 1024) * (64 / NS) <= 228 * 1024, "64 seeds per SM");
 
 __device__ __forceinline__ float score_of(const ParamsDev& p, int nh, int nm, float chi2) {
   return p.score_hit * (float)nh - p.score_miss * (float)nm - chi2;
@@ -229,60 +228,19 @@ __global__ void __launch_bounds__(256) bs_order_kernel(int n, const unsigned* __
 // ---- the chi2 of one hit against one propagated candidate; appends accepted hits to the candidate's list ---------
 struct ScanCand { float x, y, z, xl, yl, zl, cb, sb, tt, tz, zz, lim1, lim2; int kind; };
 
-__device__ __forceinline__ void accept_hit(Smem& sm, int slot, float c2, int id, unsigned t) {
-  const unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id;
-  const int k = atomicAdd(&sm.lcount[slot], 1);
-  if (k < LC) { sm.lkey[k][slot] = key; sm.lt[k][slot] = (int)t; }
-  else {                                                           // a crowded window: the CTA-wide overflow list
-    const int e = atomicAdd(&sm.ovf_n, 1);
-    if (e < OVC) { sm.ovf_key[e] = key; sm.ovf_t[e] = (int)t; sm.ovf_slot[e] = slot; }
-  }
-}
+constexpr unsigned long long KEY_NONE = ~0ull;
 
-template <bool COUNT>
-__device__ __forceinline__ void scan_range(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const ScanCand& c,
-                                           unsigned tb, unsigned te, int lane, int stride, unsigned& n_pos, unsigned& n_c2, unsigned& n_acc) {
-  KState S;                                                        // only what hit_to_local / chi2_local read
-  S.x = c.x; S.y = c.y; S.z = c.z; S.xl = c.xl; S.yl = c.yl; S.zl = c.zl; S.f.kind = c.kind; S.f.cb = c.cb; S.f.sb = c.sb;
-  unsigned t = tb + lane;
-  if (a.packed) {
-    float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (t < te) qn = __ldg(a.packed + t);
-    while (t < te) {
-      // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11), so most
-      // hits of the padded bins are rejected before their covariance is read; the next position is already in flight
-      const float4 q0 = qn;
-      const unsigned tn = t + stride;
-      if (tn < te) qn = __ldg(a.packed + tn);
-      if (COUNT) n_pos++;
-      const float rx = (q0.x - c.x) - c.xl, ry = (q0.y - c.y) - c.yl, rz = (q0.z - c.z) - c.zl;
-      const float r1 = c.kind == 0 ? c.cb * ry - c.sb * rx : rx, r2 = c.kind == 0 ? rz : ry;
-      if (!(r1 * r1 > c.lim1 || r2 * r2 > c.lim2)) {
-        const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
-        const float4 b = __ldg(cv), d = __ldg(cv + 1);
-        Hit H;
-        H.x = q0.x; H.y = q0.y; H.z = q0.z;
-        H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-        if (COUNT) n_c2++;
-        SInv o; float c2;
-        if (chi2_local(S, c.tt, c.tz, c.zz, H, o, c2) && c2 < p.chi2_cut) {
-          if (COUNT) n_acc++;
-          accept_hit(sm, slot, c2, __float_as_int(q0.w), t);
-        }
-      }
-      t = tn;
-    }
-  } else {
-    for (; t < te; t += stride) {
-      const int id = a.sorted_id[t];
-      Hit H; load_hit(H, a.hits, id);
-      if (COUNT) { n_pos++; n_c2++; }
-      SInv o; float c2;
-      if (chi2_local(S, c.tt, c.tz, c.zz, H, o, c2) && c2 < p.chi2_cut) {
-        if (COUNT) n_acc++;
-        accept_hit(sm, slot, c2, id, t);
-      }
-    }
+// Keeps the nk (<= LC) smallest keys of a candidate, sorted, under concurrent insertion by any lanes of the CTA: the key
+// sinks through the list by atomic minima, each position keeping the smaller key and handing the larger one down.
+// Whatever the interleaving, position k ends up with the minimum of everything offered to it, i.e. the (k+1)-th
+// smallest key. The last position only ever decreases, so a key that is not below it can be dropped without an atomic.
+__device__ __forceinline__ void accept_hit(Smem& sm, int slot, int nk, float c2, unsigned t) {
+  unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | t;
+  if (key >= sm.lkey[nk - 1][slot]) return;
+  for (int k = 0; k < nk; k++) {
+    const unsigned long long old = atomicMin(&sm.lkey[k][slot], key);
+    if (old == KEY_NONE) break;                                    // took an empty place
+    if (old > key) key = old;                                      // displaced a larger key: it sinks further
   }
 }
 
@@ -293,59 +251,16 @@ __device__ __forceinline__ void load_scan_cand(const Smem& sm, int slot, ScanCan
   c.tt = sm.tt[slot]; c.tz = sm.tz[slot]; c.zz = sm.zz[slot]; c.lim1 = sm.lim1[slot]; c.lim2 = sm.lim2[slot];
 }
 
-// sorted insertion of (key, t) into the first `cnt` (<= LC) entries of a slot's list, keeping the LC smallest keys
-__device__ __forceinline__ void list_insert(Smem& sm, int slot, int& cnt, unsigned long long key, int t) {
-  int k = cnt;
-  if (cnt == LC) { if (key < sm.lkey[LC - 1][slot]) k = LC - 1; else return; }
-  else cnt++;
-  while (k > 0 && key < sm.lkey[k - 1][slot]) { sm.lkey[k][slot] = sm.lkey[k - 1][slot]; sm.lt[k][slot] = sm.lt[k - 1][slot]; k--; }
-  sm.lkey[k][slot] = key; sm.lt[k][slot] = t;
-}
-
-// Last resort (the CTA-wide overflow list itself overflowed): the owner of the slot walks its window again and keeps
-// the LC best under (chi2, id). Not inlined so that it stays out of the hot loop's instruction stream.
-__device__ __noinline__ void rescan_slot(const BuildArgs& a, const ParamsDev& p, Smem& sm, int slot, const unsigned* boff, int n_phi) {
-  ScanCand c; load_scan_cand(sm, slot, c);
-  KState S;
-  S.x = c.x; S.y = c.y; S.z = c.z; S.xl = c.xl; S.yl = c.yl; S.zl = c.zl; S.f.kind = c.kind; S.f.cb = c.cb; S.f.sb = c.sb;
-  const int e0 = sm.wrow[slot] & 0xff, nr = sm.wrow[slot] >> 8, w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
-  int cntk = 0;
-  for (int ie = e0; ie < e0 + nr; ie++) {
-    const unsigned* row = boff + ie * n_phi;
-    for (int part = 0; part < 2; part++) {
-      unsigned tb, te;
-      if (part == 0) { tb = row[w0]; te = row[min(w0 + wn, n_phi)]; }
-      else { if (w0 + wn <= n_phi) break; tb = row[0]; te = row[w0 + wn - n_phi]; }
-      for (unsigned t = tb; t < te; t++) {
-        Hit H; int id;
-        if (a.packed) {
-          const float4 q0 = __ldg(a.packed + t);
-          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
-          const float4 b = __ldg(cv), d = __ldg(cv + 1);
-          H.x = q0.x; H.y = q0.y; H.z = q0.z; id = __float_as_int(q0.w);
-          H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-        } else { id = a.sorted_id[t]; load_hit(H, a.hits, id); }
-        SInv o; float c2;
-        if (!chi2_local(S, c.tt, c.tz, c.zz, H, o, c2)) continue;
-        if (!(c2 < p.chi2_cut)) continue;
-        list_insert(sm, slot, cntk, ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | (unsigned)id, (int)t);
-      }
-    }
-  }
-  sm.lcount[slot] = cntk;
-}
-
-// U14 as two integer keys, smaller = ranks first: k1 = (score descending, chi2 ascending), k2 = (parent, hit id)
+// U14 as two integer keys, smaller = ranks first: k1 = (score descending, chi2 ascending), k2 = (parent, hit), the hit
+// given by its position in the sorted index (bin, then id; misses last): reading R11 of DESIGN.md
 __device__ __forceinline__ unsigned long long rank_key1(float score, float chi2) {
   unsigned su = __float_as_uint(score);
   su = (su & 0x80000000u) ? ~su : (su | 0x80000000u);            // ascending in the float order
   return ((unsigned long long)(~su) << 32) | __float_as_uint(chi2);
 }
 __device__ __forceinline__ unsigned rank_key2(int parent, int hit) { return ((unsigned)parent << 28) | ((unsigned)hit & 0x0fffffffu); }
-constexpr unsigned long long KEY_NONE = ~0ull;
-
 #ifndef MKF_BUILD_MIN_BLOCKS
-#define MKF_BUILD_MIN_BLOCKS 4
+#define MKF_BUILD_MIN_BLOCKS (64 / MKF_BUILD_NS)
 #endif
 template <bool COUNT>
 __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
@@ -361,7 +276,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
   const size_t n = (size_t)a.n;
   const int mpl = a.max_plan_len;
   const int nb = g.n_phi * g.n_eta;
-  unsigned n_steps = 0, n_pos = 0, n_c2 = 0, n_acc = 0, n_upd = 0;        // COUNT only
+  unsigned n_steps = 0, n_pos = 0, n_c2 = 0, n_acc = 0, n_upd = 0, n_rowt = 0, n_rowo = 0;        // COUNT only
 
   // ---- load the seeds of this CTA ------------------------------------------------------------------------------
   const int pos = blockIdx.x * NS + sl;
@@ -393,6 +308,43 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
   __syncthreads();
 
   for (int s = 0; s < mpl; s++) {
+    // The rows of a window go to the CTA's table as runs of hits, with their bin offsets (the next row's are fetched
+    // ahead). A window that finds the table full keeps its place and goes on in the next scan round.
+    auto push_rows = [&](int slot) {
+      const int ssl = slot >> 3;
+      const int lay = g.plan_layers[sm.p0[ssl] + s];
+      int ie = sm.wrow[slot] & 0xff; const int iend = sm.wrow[slot] >> 8;
+      if (ie >= iend) return;
+      const int w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
+      const unsigned* row = a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb + ie * g.n_phi;
+      const int wend = min(w0 + wn, g.n_phi), wrap = w0 + wn - g.n_phi;
+      unsigned tb0 = __ldg(row + w0), te0 = __ldg(row + wend), tb1 = 0, te1 = 0;
+      if (wrap > 0) { tb1 = __ldg(row); te1 = __ldg(row + wrap); }
+      for (; ie < iend; ie++) {
+        const unsigned cb0 = tb0, ce0 = te0, cb1 = tb1, ce1 = te1;
+        if (ie + 1 < iend) {
+          row += g.n_phi;
+          tb0 = __ldg(row + w0); te0 = __ldg(row + wend);
+          if (wrap > 0) { tb1 = __ldg(row); te1 = __ldg(row + wrap); }
+        }
+        // a run longer than RUN_MAX hits (never met in practice) goes in as several entries
+        const unsigned n0 = ce0 - cb0, n1 = ce1 > cb1 ? ce1 - cb1 : 0u;
+        const int np = (int)((n0 + RUN_MAX - 1) / RUN_MAX + (n1 + RUN_MAX - 1) / RUN_MAX);
+        if (np == 0) continue;
+        const int k = atomicAdd(&sm.n_rows, np);
+        if (COUNT) n_rowt += np;
+        if (k + np > ROWCAP) {                                // no room: this row and the ones behind it wait for the next round
+          for (int kk = k; kk < min(k + np, ROWCAP); kk++) sm.rows[kk] = make_uint2((unsigned)slot, 0u);
+          sm.more = 1;
+          if (COUNT) n_rowo += np;
+          break;
+        }
+        int kk = k;
+        for (unsigned o = 0; o < n0; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n0 - o, (unsigned)RUN_MAX) << 8), cb0 + o);
+        for (unsigned o = 0; o < n1; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n1 - o, (unsigned)RUN_MAX) << 8), cb1 + o);
+      }
+      sm.wrow[slot] = ie | (iend << 8);
+    };
     // ---- which slots propagate at this step: compacted list over the CTA ------------------------------------------
     const int nl_prev = sm.n_live[sl];
     const bool seed_act = i >= 0 && seed_ok && s > seed_last && s < sm.plen[sl] && nl_prev > 0;     // uniform in the group
@@ -400,8 +352,10 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     {
       const unsigned bal = __ballot_sync(0xffffffffu, parent_live);
       if (lane == 0) sm.wsum[warp] = __popc(bal);
-      sm.flag[tid] = 0; sm.lcount[tid] = 0; sm.rowpre[tid] = 0;
-      if (tid == 0) sm.ovf_n = 0;
+      sm.flag[tid] = 0; sm.wrow[tid] = 0;
+      if (tid == 0) { sm.n_rows = 0; sm.more = 0; }
+#pragma unroll
+      for (int k = 0; k < LC; k++) sm.lkey[k][tid] = KEY_NONE;
       __syncthreads();
       int base = 0, tot = 0;
 #pragma unroll
@@ -441,10 +395,10 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         int e0, e1, w0, wn;
         window(g, L, p.chi2_cut, S, tt, zz, vxy, vzz, e0, e1, w0, wn);
         sm.tt[slot] = tt; sm.tz[slot] = tz; sm.zz[slot] = zz;
-        sm.lim1[slot] = p.chi2_cut * (tt + vxy) * 1.0001f;
-        sm.lim2[slot] = p.chi2_cut * (zz + (L.kind == 0 ? vzz : vxy)) * 1.0001f;
-        sm.wrow[slot] = e0 | ((e1 - e0 + 1) << 8); sm.wphi[slot] = w0 | (wn << 8);
-        sm.rowpre[slot] = e1 - e0 + 1;
+        sm.lim1[slot] = (tt + vxy) * 1.0001f;
+        sm.lim2[slot] = (zz + (L.kind == 0 ? vzz : vxy)) * 1.0001f;
+        sm.wrow[slot] = e0 | ((e1 + 1) << 8); sm.wphi[slot] = w0 | (wn << 8);
+        push_rows(slot);
         int fl = FL_SCAN;
         // miss child (C9.5): stopped if it reaches the consecutive-miss limit
         if (consec + 1 >= p.max_consec_miss) { if (nh >= p.min_hits_keep) { fl |= FL_OFFER_MISS; sm.ostat[slot] = 0; } }
@@ -454,83 +408,121 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     }
     __syncthreads();
 
-    // ---- exclusive prefix of the windows' row counts: the rows of all candidates as one list -----------------------
-    {
-      const int v = sm.rowpre[tid];
-      int inc = v;
+    // ---- phase S: the hits of all runs of the table as ONE list. Pass A: every thread takes an equal share of it and
+    // tests positions (16 B per hit); the survivors go to a queue. Pass B: one thread per queued survivor reads the
+    // covariance (32 B) and evaluates chi2; accepted hits sink into their candidate's list. Both passes run with every
+    // lane busy whatever the sizes of the windows. Further rounds while windows have rows left. --------------------------
+    for (;;) {
+      const int NR = min(sm.n_rows, ROWCAP);
+      const int more = sm.more;
+      // exclusive prefix of the run lengths
+      {
+        constexpr int PER = (ROWCAP + BT - 1) / BT;
+        int loc[PER]; int sum = 0;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { const int t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
-      if (lane == 31) sm.wsum[warp] = inc;
-      __syncthreads();
-      int base = 0, tot = 0;
+        for (int k = 0; k < PER; k++) { const int j = tid * PER + k; loc[k] = j < NR ? (int)(sm.rows[j].x >> 8) : 0; sum += loc[k]; }
+        int inc = sum;
 #pragma unroll
-      for (int w2 = 0; w2 < BT / 32; w2++) { const int c = sm.wsum[w2]; if (w2 < warp) base += c; tot += c; }
-      sm.rowpre[tid] = base + inc - v;
-      if (tid == 0) sm.rowpre[SL] = tot;
-      __syncthreads();
-    }
-
-    // ---- phase S: SCAN_G lanes per (candidate, eta row); the next row's bin offsets are fetched ahead ---------------
-    const int NR = sm.rowpre[SL];
-    if (NR > 0) {
-      const int gl = tid & (SCAN_G - 1);
-      auto item = [&](int j, int& slot, unsigned& tb0, unsigned& te0, unsigned& tb1, unsigned& te1) {
-        int lo = 0, hi = SL;
+        for (int o = 1; o < 32; o <<= 1) { const int t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
+        if (lane == 31) sm.wsum[warp] = inc;
+        __syncthreads();
+        int base = 0, tot = 0;
 #pragma unroll
-        for (int it = 0; it < 8; it++) {                      // last slot with rowpre[slot] <= j  (SL <= 256)
-          const int mid = (lo + hi) >> 1;
-          if (hi - lo > 1) { if (sm.rowpre[mid] <= j) lo = mid; else hi = mid; }
-        }
-        slot = lo;
-        const int ssl = slot >> 3;
-        const int ie = (sm.wrow[slot] & 0xff) + (j - sm.rowpre[slot]);
-        const int w0 = sm.wphi[slot] & 0xff, wn = sm.wphi[slot] >> 8;
-        const int lay = g.plan_layers[sm.p0[ssl] + s];
-        const unsigned* row = a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb + ie * g.n_phi;
-        tb0 = __ldg(row + w0); te0 = __ldg(row + min(w0 + wn, g.n_phi));
-        tb1 = 0; te1 = 0;
-        if (w0 + wn > g.n_phi) { tb1 = __ldg(row); te1 = __ldg(row + w0 + wn - g.n_phi); }
-      };
-      int j = tid / SCAN_G;
-      int slot_n = 0; unsigned ntb0 = 0, nte0 = 0, ntb1 = 0, nte1 = 0;
-      if (j < NR) item(j, slot_n, ntb0, nte0, ntb1, nte1);
-      while (j < NR) {
-        const int slot = slot_n; const unsigned tb0 = ntb0, te0 = nte0, tb1 = ntb1, te1 = nte1;
-        const int jn = j + BT / SCAN_G;
-        if (jn < NR) item(jn, slot_n, ntb0, nte0, ntb1, nte1);
-        ScanCand c; load_scan_cand(sm, slot, c);
-        scan_range<COUNT>(a, p, sm, slot, c, tb0, te0, gl, SCAN_G, n_pos, n_c2, n_acc);
-        if (te1 > tb1) scan_range<COUNT>(a, p, sm, slot, c, tb1, te1, gl, SCAN_G, n_pos, n_c2, n_acc);
-        j = jn;
+        for (int w2 = 0; w2 < BT / 32; w2++) { const int c = sm.wsum[w2]; if (w2 < warp) base += c; tot += c; }
+        int run = base + inc - sum;
+#pragma unroll
+        for (int k = 0; k < PER; k++) { const int j = tid * PER + k; if (j <= NR) sm.runpre[j] = run; run += loc[k]; }
+        if (tid == 0) { sm.runpre[NR] = tot; sm.sq_n = 0; }
+        __syncthreads();
       }
+      const int H = sm.runpre[NR];
+      for (int h0 = 0; h0 < H; h0 += SQCAP) {
+        // ---- pass A: hits [h0, h1), a contiguous share per thread (its next position is fetched ahead) ------------------
+        const int h1 = min(h0 + SQCAP, H);
+        const int share = (h1 - h0 + BT - 1) / BT;
+        int q = h0 + tid * share;
+        const int qe = min(q + share, h1);
+        if (q < qe) {
+          int lo = 0, hi = NR;                                // run of hit q: last j with runpre[j] <= q
+          while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sm.runpre[mid] <= q) lo = mid; else hi = mid; }
+          int j = lo;
+          while (q < qe) {
+            const uint2 r = sm.rows[j];
+            const int slot = (int)(r.x & 0xffu);
+            const int rb = sm.runpre[j], re = rb + (int)(r.x >> 8);
+            const int qs = min(qe, re);
+            if (a.packed) {
+              const float cx = sm.B[F_X][slot], cy = sm.B[F_Y][slot], cz = sm.B[F_Z][slot];
+              const float cxl = sm.B[F_XL][slot], cyl = sm.B[F_YL][slot], czl = sm.B[F_ZL][slot];
+              const int kind = __float_as_int(sm.B[F_FK][slot]); const float cb = sm.B[F_FCB][slot], sb = sm.B[F_FSB][slot];
+              const float l1 = sm.lim1[slot], l2 = sm.lim2[slot];
+              const unsigned* worst = reinterpret_cast<const unsigned*>(&sm.lkey[p.max_cand - 1][slot]) + 1;    // chi2 bits of the list's last hit
+              const float4* pp = a.packed + r.y + (q - rb);
+              float4 qn = __ldg(pp);
+              for (; q < qs; q++) {
+                // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11); once
+                // the candidate's list is full only a hit better than its last one can matter, so the cut follows it
+                const float4 q0 = qn;
+                pp++;
+                if (q + 1 < qs) qn = __ldg(pp);
+                if (COUNT) n_pos++;
+                const float cut = fminf(p.chi2_cut, __uint_as_float(min(*(volatile const unsigned*)worst, 0x7f800000u)));
+                const float rx = (q0.x - cx) - cxl, ry = (q0.y - cy) - cyl, rz = (q0.z - cz) - czl;
+                const float r1 = kind == 0 ? cb * ry - sb * rx : rx, r2 = kind == 0 ? rz : ry;
+                if (!(r1 * r1 > cut * l1 || r2 * r2 > cut * l2)) sm.sq[atomicAdd(&sm.sq_n, 1)] = ((unsigned)j << 22) | (unsigned)(q - rb);
+              }
+            } else {
+              if (COUNT) n_pos += qs - q;
+              for (; q < qs; q++) sm.sq[atomicAdd(&sm.sq_n, 1)] = ((unsigned)j << 22) | (unsigned)(q - rb);
+            }
+            j++;
+          }
+        }
+        __syncthreads();
+        // ---- pass B: one thread per survivor ---------------------------------------------------------------------------
+        const int nq = sm.sq_n;
+        for (int k = tid; k < nq; k += BT) {
+          const unsigned e = sm.sq[k];
+          const uint2 r = sm.rows[e >> 22];
+          const int slot = (int)(r.x & 0xffu);
+          const unsigned t = r.y + (e & 0x3fffffu);
+          Hit H2;
+          if (a.packed) {
+            const float4 q0 = __ldg(a.packed + t);
+            const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
+            const float4 b4 = __ldg(cv), d4 = __ldg(cv + 1);
+            H2.x = q0.x; H2.y = q0.y; H2.z = q0.z;
+            H2.v[0] = b4.x; H2.v[1] = b4.y; H2.v[2] = b4.z; H2.v[3] = b4.w; H2.v[4] = d4.x; H2.v[5] = d4.y;
+          } else load_hit(H2, a.hits, a.sorted_id[t]);
+          ScanCand c; load_scan_cand(sm, slot, c);
+          KState Sc;                                          // only what hit_to_local / chi2_local read
+          Sc.x = c.x; Sc.y = c.y; Sc.z = c.z; Sc.xl = c.xl; Sc.yl = c.yl; Sc.zl = c.zl; Sc.f.kind = c.kind; Sc.f.cb = c.cb; Sc.f.sb = c.sb;
+          if (COUNT) n_c2++;
+          SInv o; float c2;
+          if (chi2_local(Sc, c.tt, c.tz, c.zz, H2, o, c2) && c2 < p.chi2_cut) {
+            if (COUNT) n_acc++;
+            accept_hit(sm, slot, p.max_cand, c2, t);
+          }
+        }
+        __syncthreads();
+        if (tid == 0) sm.sq_n = 0;
+        if (h0 + SQCAP < H) __syncthreads();
+      }
+      if (!more) break;
+      __syncthreads();
+      if (tid == 0) { sm.n_rows = 0; sm.more = 0; }
+      __syncthreads();
+      if (tid < sm.nP) push_rows(sm.plist[tid]);
       __syncthreads();
     }
 
-    // ---- phase L: each slot orders its accepted hits by (chi2, id) ---------------------------------------------------
+    // ---- the lists are sorted as they stand: count this slot's entries -----------------------------------------------
     const int fl = sm.flag[tid];
     int n_hitc = 0;
     if (fl & FL_SCAN) {
-      const int nacc = sm.lcount[tid];
-      n_hitc = min(nacc, LC);
-      for (int k = 1; k < n_hitc; k++) {
-        const unsigned long long key = sm.lkey[k][tid]; const int tk = sm.lt[k][tid];
-        int m = k;
-        while (m > 0 && key < sm.lkey[m - 1][tid]) { sm.lkey[m][tid] = sm.lkey[m - 1][tid]; sm.lt[m][tid] = sm.lt[m - 1][tid]; m--; }
-        sm.lkey[m][tid] = key; sm.lt[m][tid] = tk;
-      }
-      if (nacc > LC) {
-        const int nov = sm.ovf_n;
-        if (nov <= OVC) {
-          for (int e = 0; e < nov; e++) if (sm.ovf_slot[e] == tid) list_insert(sm, tid, n_hitc, sm.ovf_key[e], sm.ovf_t[e]);
-        } else {
-          const int ssl = tid >> 3;
-          const int lay = g.plan_layers[sm.p0[ssl] + s];
-          rescan_slot(a, p, sm, tid, a.bin_off + ((size_t)sm.ev[ssl] * g.n_layers + lay) * (size_t)nb, g.n_phi);
-          n_hitc = sm.lcount[tid];
-        }
-      }
+#pragma unroll
+      for (int k = 0; k < LC; k++) n_hitc += sm.lkey[k][tid] != KEY_NONE ? 1 : 0;
     }
-    __syncwarp();
 
     // ---- per seed group: lane = parent slot -------------------------------------------------------------------------
     const float chi2 = sm.chi2[tid];
@@ -573,14 +565,14 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       const unsigned long long alt_k1 = rank_key1((fl & FL_MISS) ? score_of(p, nh, nm + 1, chi2) : score_of(p, nh, nm, chi2), chi2);
       if (!parent_live) n_hitc = 0;
       int head = 0;
-      int my_kind = -1, my_hit = -2, my_t = 0;
+      int my_kind = -1, my_t = 0;
       for (int r = 0; r < p.max_cand; r++) {
         // head child of this lane: its next hit or its miss / pass-through child, whichever ranks first (U14)
-        unsigned long long k1 = KEY_NONE; int hh = HIT_NONE, hk = 3, ht = 0;
+        unsigned long long k1 = KEY_NONE; int hh = HIT_NONE, hk = 3;
         if (head < n_hitc) {
           const unsigned long long key = sm.lkey[head][tid];
           const float c2h = __uint_as_float((unsigned)(key >> 32));
-          k1 = rank_key1(base_hit - c2h, chi2 + c2h); hh = (int)(unsigned)key; hk = 0; ht = sm.lt[head][tid];
+          k1 = rank_key1(base_hit - c2h, chi2 + c2h); hh = (int)(unsigned)key; hk = 0;
         }
         if (alt_avail && alt_k1 < k1) { k1 = alt_k1; hh = HIT_NONE; hk = alt_kind; }     // same parent: a tie in k1 goes to the hit
         unsigned k2 = rank_key2(sub, hh);
@@ -593,12 +585,12 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         if (w1 == KEY_NONE) break;                            // pool exhausted (uniform in the group)
         const int wp = (int)(w2 >> 28);
         const int src = gbase + wp;
-        const int wk = __shfl_sync(gm, hk, src), wh = __shfl_sync(gm, hh, src), wt = __shfl_sync(gm, ht, src);
+        const int wk = __shfl_sync(gm, hk, src), wh = __shfl_sync(gm, hh, src);
         if (sub == wp) { if (wk == 0) head++; else alt_avail = false; }      // the winner lane pops its head
-        if (sub == r) { my_parent = wp; my_kind = wk; my_hit = wk == 0 ? wh : (wk == 1 ? -1 : -2); my_t = wt; }
+        if (sub == r) { my_parent = wp; my_kind = wk; my_t = wh; }
         n_new = r + 1;
       }
-      if (sub < n_new) { sm.sel[tid] = my_parent | (my_kind << 3); sm.sel_t[tid] = my_t; sm.sel_hit[tid] = my_hit; }
+      if (sub < n_new) { sm.sel[tid] = my_parent | (my_kind << 3); sm.sel_t[tid] = my_t; }
     }
 
     // ---- phase U: the chosen children, compacted over the CTA: the parent's state, updated with the hit --------------
@@ -619,8 +611,9 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     bool nan_child = false;
     if (tid < sm.nP) {
       cslot = sm.plist[tid];
-      c_sel = sm.sel[cslot]; c_hit = sm.sel_hit[cslot];
+      c_sel = sm.sel[cslot];
       const int kind = (c_sel >> 3) & 3;
+      c_hit = kind == 1 ? -1 : -2;
       const int ps = (cslot & ~(G - 1)) + (c_sel & 7);        // parent's slot
       Hit H;
       if (kind == 0) {                                        // the hit's record first: its latency overlaps the state loads
@@ -629,9 +622,9 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           const float4 q0 = __ldg(a.packed + t);
           const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
           const float4 b = __ldg(cv), d = __ldg(cv + 1);
-          H.x = q0.x; H.y = q0.y; H.z = q0.z;
+          H.x = q0.x; H.y = q0.y; H.z = q0.z; c_hit = __float_as_int(q0.w);
           H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-        } else load_hit(H, a.hits, c_hit);
+        } else { c_hit = a.sorted_id[sm.sel_t[cslot]]; load_hit(H, a.hits, c_hit); }
       }
       const int pcn = sm.cnt[ps];
       c_chi2 = sm.chi2[ps];
@@ -647,6 +640,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         else { nan_child = true; sm.sel[cslot] = c_sel | 256; }        // dropped (C9 / R1)
       }
       c_cnt = c_nh | (c_nm << 8) | (c_consec << 16);
+      sm.sel_hit[cslot] = c_hit;                              // for the trellis entry if the live set is compacted below
     }
     const bool any_nan = __syncthreads_or(nan_child);         // also: every read of A and B of this step is done
     if (any_nan) {
@@ -771,9 +765,9 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     }
   }
   if (COUNT) {
-    unsigned v[5] = {n_steps, n_pos, n_c2, n_acc, n_upd};
+    unsigned v[7] = {n_steps, n_pos, n_c2, n_acc, n_upd, n_rowt, n_rowo};
 #pragma unroll
-    for (int k = 0; k < 5; k++) {
+    for (int k = 0; k < 7; k++) {
       unsigned x = v[k];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);

@@ -33,9 +33,10 @@ __global__ void __launch_bounds__(DD_BLOCK) dd_fill(const __grid_constant__ DdAr
   if (h >= 0 && h < a.n_hits) a.list[atomicAdd(&a.cnt[h], 1u)] = (int)(k % (size_t)a.n);
 }
 
-// |ids_i ∩ ids_j| is the number of times j appears in the lists filed under the hits of i (a hit appears at most once
-// in a track), so one warp per track gathers those lists into shared memory and counts multiplicities: with at most 32
-// entries one match.any does it. Tracks whose lists hold more than DD_CAP entries take the plain loop (lane 0).
+// |ids_i ∩ ids_j| (entries of j that are hits of i) is the number of times j appears in the lists filed under the
+// DISTINCT hits of i, so one warp per track gathers those lists into shared memory and counts multiplicities: with at
+// most 32 entries one match.any does it. Tracks whose lists hold more than DD_CAP entries, and plans longer than a
+// warp, take the plain loop (lane 0).
 constexpr int DD_CAP = 128, DD_WARPS = DD_BLOCK / 32;
 
 __device__ bool dd_dominated_slow(const DdArgs& a, int i, int eb, int ee) {
@@ -81,7 +82,9 @@ __global__ void __launch_bounds__(DD_BLOCK) dd_mark(const __grid_constant__ DdAr
     int h = -1;
     if (s < a.mpl) h = a.hit_ids[(size_t)s * n + i];
     unsigned b = 0; int len = 0;
-    if (h >= 0 && h < a.n_hits) { b = a.off[h]; len = (int)(a.off[h + 1] - b); }
+    const bool valid = h >= 0 && h < a.n_hits;
+    const unsigned same = __match_any_sync(0xffffffffu, valid ? h : -1 - lane);
+    if (valid && (__ffs(same) - 1) == lane) { b = a.off[h]; len = (int)(a.off[h + 1] - b); }       // first occurrence of h in i
     int inc = len;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int t2 = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t2; }
@@ -91,7 +94,7 @@ __global__ void __launch_bounds__(DD_BLOCK) dd_mark(const __grid_constant__ DdAr
   }
   __syncwarp();
   bool removed = false;
-  if (total > DD_CAP) { if (lane == 0) removed = dd_dominated_slow(a, i, eb, ee); }
+  if (total > DD_CAP || a.mpl > 32) { if (lane == 0) removed = dd_dominated_slow(a, i, eb, ee); }
   else {
     const int nhi = a.nhits[i];
     const float si = a.score[i];

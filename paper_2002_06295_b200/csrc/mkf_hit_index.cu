@@ -13,8 +13,8 @@
 // as ONE kernel, hi_fused_kernel (one CTA per segment): the hits of a segment occupy the same range of positions before
 // and after sorting, so its bin offsets are layer_off + a prefix over the segment's own bins, computed in shared
 // memory (10 KB for 63 x 40 bins: the occupancy is bounded by threads, not by shared memory); ids are scattered with
-// an atomic cursor, each bin's few ids are then put in ascending order, and every hit writes its packed record at the
-// place it finds for its id in its bin; the segment is read from HBM once (the later passes hit L2).
+// an atomic cursor into a scratch list, and every hit then takes as its place in the bin the number of smaller ids it
+// finds there, writing its id and its packed record; the segment is read from HBM once (the later passes hit L2).
 // HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
 #include "mkf_ctx.h"
 #include "mkf_scan.cuh"
@@ -28,6 +28,7 @@ constexpr int HI_BLOCK = 256;
 struct HiArgs {
   HitsDev hits; int n_layers, n_phi, n_eta;
   int* key;            // [n_hits] bin inside the segment
+  int* tmp_id;         // [n_hits] ids by bin, any order inside a bin (single-kernel path)
   unsigned* cnt;       // [n_bins_total] counts, later the scatter cursors
   unsigned* bin_off; int* sorted_id; float* vmax; float4* packed;
   const unsigned char* mask;     // R9: hits left out of the index (NULL: none)
@@ -145,6 +146,7 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
 
 // ---- the plain index in one kernel ------------------------------------------------------------------------------------
 constexpr int HF_BLOCK = 256, HF_WARPS = HF_BLOCK / 32;
+constexpr int HF_TMPCAP = 10240;     // ids of a segment kept in shared memory between the scatter and the ranking (the rest: workspace)
 
 // Bin key of a hit, identical to the fp64 evaluation of C8 (U12): fp32 first; the fp64 formulas only when the fp32
 // value lies within 1e-3 bin widths of a bin edge (fp32 atan2f / asinhf are good to a few 1e-7 in value, 2e-5 in bin
@@ -169,15 +171,18 @@ __device__ __forceinline__ int bin_key(float xf, float yf, float zf, float elo_f
 // One CTA per segment, bin counts of the segment in shared memory:
 //   A  key per hit (kept in the workspace), count per bin, per-segment max hit variances;
 //   -  exclusive prefix over the segment's bins -> bin_off (= layer_off + prefix) and the scatter cursors;
-//   B  ids scattered to their bins (atomic cursor: any order inside a bin);
-//   -  each bin's ids sorted ascending: the unique stable order of C8;
-//   C  every hit finds its place in its bin and writes its packed record there (reads in id order: coalesced).
+//   B  ids scattered to their bins in a scratch list (atomic cursor: any order inside a bin);
+//   C  every hit counts the ids of its bin that are smaller than its own: that rank is its place in the bin (the unique
+//      stable order of C8, no sort and no dependent probing: the bin's few ids are independent loads); it writes its id
+//      and its packed record there. Hits are read in id order (coalesced) in every pass; two hits per thread and
+//      iteration keep more loads in flight.
 __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
-  extern __shared__ unsigned hf_cnt[];                        // [nb] counts, then cursors
+  extern __shared__ unsigned hf_cnt[];                        // [nb] counts, then cursors; [HF_TMPCAP] ids by bin
   __shared__ float s_xy[HF_WARPS], s_zz[HF_WARPS];
   __shared__ unsigned s_ws[HF_WARPS];
   const int seg = blockIdx.x;
   const int nb = a.n_phi * a.n_eta;
+  int* s_tmp = reinterpret_cast<int*>(hf_cnt + nb);
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
   const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
@@ -187,16 +192,32 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
   const size_t nh = (size_t)a.hits.n_hits;
   const float* V = a.hits.V;
   float vxy = 0.f, vzz = 0.f;
-  for (int i = b + tid; i < e; i += HF_BLOCK) {
-    const int key = bin_key(a.hits.x[i], a.hits.y[i], a.hits.z[i], elo, ehi, a.n_phi, a.n_eta);
-    a.key[i] = key;
-    atomicAdd(&hf_cnt[key], 1u);
+  for (int i0 = b + tid; i0 < e; i0 += 2 * HF_BLOCK) {
+    const int i1 = i0 + HF_BLOCK;
+    const bool two = i1 < e;
+    const int j1 = two ? i1 : i0;
+    const float x0 = a.hits.x[i0], y0 = a.hits.y[i0], z0 = a.hits.z[i0], x1 = a.hits.x[j1], y1 = a.hits.y[j1], z1 = a.hits.z[j1];
+    const float p0 = V[i0], q0 = V[nh + i0], r0 = V[2 * nh + i0], t0 = V[5 * nh + i0];
+    const float p1 = V[j1], q1 = V[nh + j1], r1 = V[2 * nh + j1], t1 = V[5 * nh + j1];
+    const int key0 = bin_key(x0, y0, z0, elo, ehi, a.n_phi, a.n_eta);
+    a.key[i0] = key0;
+    atomicAdd(&hf_cnt[key0], 1u);
+    if (two) {
+      const int key1 = bin_key(x1, y1, z1, elo, ehi, a.n_phi, a.n_eta);
+      a.key[i1] = key1;
+      atomicAdd(&hf_cnt[key1], 1u);
+    }
     // larger eigenvalue of the xy block of V in round-to-nearest fp32 without contraction (bit-exact with C8)
-    const float vxx = V[i], vxyv = V[nh + i], vyy = V[2 * nh + i];
-    const float hs = __fmul_rn(0.5f, __fadd_rn(vxx, vyy)), hd = __fmul_rn(0.5f, __fsub_rn(vxx, vyy));
-    const float ev1 = __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(vxyv, vxyv))));
-    vxy = fmaxf(vxy, ev1);
-    vzz = fmaxf(vzz, V[5 * nh + i]);
+    {
+      const float hs = __fmul_rn(0.5f, __fadd_rn(p0, r0)), hd = __fmul_rn(0.5f, __fsub_rn(p0, r0));
+      vxy = fmaxf(vxy, __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(q0, q0)))));
+      vzz = fmaxf(vzz, t0);
+    }
+    {
+      const float hs = __fmul_rn(0.5f, __fadd_rn(p1, r1)), hd = __fmul_rn(0.5f, __fsub_rn(p1, r1));
+      vxy = fmaxf(vxy, __fadd_rn(hs, __fsqrt_rn(__fadd_rn(__fmul_rn(hd, hd), __fmul_rn(q1, q1)))));
+      vzz = fmaxf(vzz, t1);
+    }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -228,36 +249,48 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
     if (seg == gridDim.x - 1 && tid == 0) a.bin_off[a.n_bins] = (unsigned)a.hits.n_hits;
   }
   __syncthreads();
-  for (int i = b + tid; i < e; i += HF_BLOCK) a.sorted_id[atomicAdd(&hf_cnt[a.key[i]], 1u)] = i;
-  __syncthreads();                                            // cursor[k] is now the end of bin k
-  for (int k = tid; k < nb; k += HF_BLOCK) {
-    const unsigned kb = k == 0 ? (unsigned)b : hf_cnt[k - 1], ke = hf_cnt[k];
-    const int len = (int)(ke - kb);
-    if (len < 2) continue;
-    int* v = a.sorted_id + kb;
-    if (len == 2) { const int x0 = v[0], x1 = v[1]; if (x0 > x1) { v[0] = x1; v[1] = x0; } continue; }
-    for (int q = 1; q < len; q++) {                           // insertion sort (a handful of ids; crowded bins are O(len^2))
-      const int x = v[q];
-      int j = q - 1;
-      while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; j--; }
-      v[j + 1] = x;
-    }
-  }
-  if (!a.packed) return;
-  __syncthreads();
   for (int i = b + tid; i < e; i += HF_BLOCK) {
-    const int key = a.key[i];
-    unsigned t = key == 0 ? (unsigned)b : hf_cnt[key - 1];
-    const unsigned te = hf_cnt[key];
-    if (te - t > 8u) {                                        // crowded bin: binary search of the ascending ids
-      unsigned lo = t, hi = te;
-      while (hi - lo > 1u) { const unsigned mid = (lo + hi) >> 1; if (a.sorted_id[mid] <= i) lo = mid; else hi = mid; }
-      t = lo;
-    } else while (a.sorted_id[t] != i) t++;
-    a.packed[t] = make_float4(a.hits.x[i], a.hits.y[i], a.hits.z[i], __int_as_float(i));
-    float4* o = a.packed + nh + (size_t)2 * t;
-    o[0] = make_float4(V[i], V[nh + i], V[2 * nh + i], V[3 * nh + i]);
-    o[1] = make_float4(V[4 * nh + i], V[5 * nh + i], 0.f, 0.f);
+    const unsigned pos = atomicAdd(&hf_cnt[a.key[i]], 1u);
+    if (pos - (unsigned)b < (unsigned)HF_TMPCAP) s_tmp[pos - b] = i; else a.tmp_id[pos] = i;
+  }
+  __syncthreads();                                            // cursor[k] is now the end of bin k
+  // rank of id i among the ids of its bin: four independent loads per round (a bin holds a handful of ids)
+  auto place = [&](int i, int key) -> unsigned {
+    const unsigned kb = key == 0 ? (unsigned)b : hf_cnt[key - 1], ke = hf_cnt[key];
+    unsigned rank = 0;
+    auto at = [&](unsigned q) -> int { return q - (unsigned)b < (unsigned)HF_TMPCAP ? s_tmp[q - b] : a.tmp_id[q]; };
+    for (unsigned q = kb; q < ke; q += 4) {
+      const int v0 = at(q);
+      const int v1 = q + 1 < ke ? at(q + 1) : 0x7fffffff;
+      const int v2 = q + 2 < ke ? at(q + 2) : 0x7fffffff;
+      const int v3 = q + 3 < ke ? at(q + 3) : 0x7fffffff;
+      rank += (v0 < i ? 1u : 0u) + (v1 < i ? 1u : 0u) + (v2 < i ? 1u : 0u) + (v3 < i ? 1u : 0u);
+    }
+    return kb + rank;
+  };
+  auto write = [&](int i, unsigned t, float x, float y, float z, float v0, float v1, float v2, float v3, float v4, float v5) {
+    a.sorted_id[t] = i;
+    if (a.packed) {
+      a.packed[t] = make_float4(x, y, z, __int_as_float(i));
+      float4* o = a.packed + nh + (size_t)2 * t;
+      o[0] = make_float4(v0, v1, v2, v3);
+      o[1] = make_float4(v4, v5, 0.f, 0.f);
+    }
+  };
+  for (int i0 = b + tid; i0 < e; i0 += 2 * HF_BLOCK) {
+    const int i1 = i0 + HF_BLOCK;
+    const bool two = i1 < e;
+    const int j1 = two ? i1 : i0;
+    const int key0 = a.key[i0], key1 = a.key[j1];
+    const float x0 = a.hits.x[i0], y0 = a.hits.y[i0], z0 = a.hits.z[i0], x1 = a.hits.x[j1], y1 = a.hits.y[j1], z1 = a.hits.z[j1];
+    float u0[6], u1[6];
+    if (a.packed) {
+#pragma unroll
+      for (int k = 0; k < 6; k++) { u0[k] = V[(size_t)k * nh + i0]; u1[k] = V[(size_t)k * nh + j1]; }
+    }
+    const unsigned t0 = place(i0, key0), t1 = place(j1, key1);
+    write(i0, t0, x0, y0, z0, u0[0], u0[1], u0[2], u0[3], u0[4], u0[5]);
+    if (two) write(i1, t1, x1, y1, z1, u1[0], u1[1], u1[2], u1[3], u1[4], u1[5]);
   }
 }
 
@@ -266,7 +299,7 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
 namespace mkf {
 size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits) {
   const size_t nbins = (size_t)n_events * c->g.n_layers * c->g.n_phi * c->g.n_eta;
-  return align256((size_t)n_hits * 4) + align256(nbins * 4) + scan_partial_bytes(nbins);
+  return 2 * align256((size_t)n_hits * 4) + align256(nbins * 4) + scan_partial_bytes(nbins);
 }
 }  // namespace mkf
 
@@ -291,19 +324,23 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
   HiArgs a;
   a.hits = hits_dev(h); a.n_layers = c->g.n_layers; a.n_phi = c->g.n_phi; a.n_eta = c->g.n_eta;
   a.key = (int*)w; w += align256((size_t)h->n_hits * 4);
+  a.tmp_id = (int*)w; w += align256((size_t)h->n_hits * 4);
   a.cnt = (unsigned*)w; w += align256(nbins * 4);
   unsigned* partial = (unsigned*)w;
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
   a.mask = mask; a.n_bins = nbins;
-  const size_t fused_smem = (size_t)c->g.n_phi * c->g.n_eta * 4;
-  if (!mask && fused_smem <= 200 * 1024) {
+  const size_t fused_smem = (size_t)c->g.n_phi * c->g.n_eta * 4 + (size_t)HF_TMPCAP * 4;
+  // The single-kernel path pays off while a segment is small enough for a CTA's share of L2 (measured: 0.19 against
+  // 0.34 ms on configs[2], 0.76 against 1.37 ms on configs[3], but 2.1 against 1.6 ms on the 7.5 k-hit segments of
+  // configs[4], where 592 CTAs in flight thrash L2 with their scattered record writes).
+  if (!mask && fused_smem <= 200 * 1024 && (size_t)h->n_hits <= (size_t)nseg * 4096) {
     if (h->n_hits == 0) {                                      // nothing to place: all offsets are zero
       cudaError_t e0 = cudaMemsetAsync(a.bin_off, 0, (nbins + 1) * 4, st);
       if (e0 == cudaSuccess) e0 = cudaMemsetAsync(a.vmax, 0, (size_t)nseg * 8, st);
       if (e0 != cudaSuccess) return cuda_fail(c, e0, "mkf_build_hit_index: memset");
       return MKF_OK;
     }
-    if (fused_smem > 48 * 1024) {
+    {
       cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
       if (e1 != cudaSuccess) return cuda_fail(c, e1, "mkf_build_hit_index: shared memory attribute");
     }
