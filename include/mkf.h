@@ -61,7 +61,10 @@ typedef struct { int kind;            /* 0 barrel cylinder, 1 disk */
 /* Geometry: all pointers HOST, copied by mkf_create. A "plan" is the ordered list of layers a seed is
  * followed through (U17); plan p = plan_layers[plan_off[p] .. plan_off[p+1]). */
 typedef struct { int n_layers; const mkf_layer* layers; float bz; int n_phi_bins, n_eta_bins;
-                 int n_plans; const int* plan_off; const int* plan_layers; } mkf_geometry;
+                 int n_plans; const int* plan_off; const int* plan_layers;
+                 const float* bz_layer; /* field hook (reading R13; "geometry, material, magnetic field"):
+                                           [n_layers] Bz [T] of the step that ENDS on layer l (a backward step runs in the
+                                           field of the layer it leaves); NULL: bz everywhere */ } mkf_geometry;
 
 typedef struct { float chi2_cut;      /* hit accepted iff chi2 < chi2_cut (30) */
                  int max_cand;        /* live candidates kept per seed per layer, <= MKF_MAX_CAND (6 or 8) */
@@ -69,7 +72,7 @@ typedef struct { float chi2_cut;      /* hit accepted iff chi2 < chi2_cut (30) *
                  int min_hits_keep;   /* stopped candidates with at least this many hits are preserved (4) */
                  float score_hit, score_miss; /* score = score_hit*nhits - score_miss*nmiss - chi2 (U13) */
                  float graze_cos_min; /* U7 (0.25) */
-                 int material_flags;  /* bit0 multiple scattering, bit1 dE/dx (C5) */
+                 int material_flags;  /* bit0 multiple scattering, bit1 dE/dx (C5), bit2 energy-loss straggling (R12; needs bit1) */
                  float dup_frac;      /* duplicate if shared/min(nhits) > dup_frac (0.5) */ } mkf_params;
 
 /* Hits of n_events events, grouped by (event, layer): the hits of (ev, l) are the ids

@@ -149,6 +149,16 @@ double dedx(double p) {                 // -dE/dx [GeV/cm], Bethe-Bloch without 
   return BB_K * SI_ZA * SI_RHO / (beta * beta) *
          (0.5 * std::log(2.0 * M_E_GEV * b2g2 * tmax / (SI_I * SI_I)) - beta * beta);
 }
+// R12: Gaussian energy-loss straggling, variance of the loss in thickness t (radiation lengths
+// along the path): sigma_E^2 = xi Tmax (1 - beta^2/2) with xi = (K/2)(Z/A) rho x / beta^2, x = t X0 (Bohr's variance
+// with the relativistic factor; the same Tmax as Bethe-Bloch).
+double straggling_var(double p, double t) {
+  double m = M_PI_GEV, E = std::sqrt(p * p + m * m), beta2 = p * p / (E * E), gamma = E / m;
+  double b2g2 = beta2 * gamma * gamma;
+  double tmax = 2.0 * M_E_GEV * b2g2 / (1.0 + 2.0 * gamma * M_E_GEV / m + (M_E_GEV / m) * (M_E_GEV / m));
+  double xi = 0.5 * BB_K * SI_ZA * SI_RHO * (t * SI_X0) / beta2;
+  return xi * tmax * (1.0 - 0.5 * beta2);
+}
 double highland(double p, double t) {
   double m = M_PI_GEV, E = std::sqrt(p * p + m * m), beta = p / E;
   return 0.0136 / (beta * p) * std::sqrt(t) * (1.0 + 0.038 * std::log(t));
@@ -179,6 +189,12 @@ int material(int kind, double xx0, int flags, double* u, double* C, double* th0_
     u[IIPT] *= p / p1;
     for (int j = 0; j < 6; j++) { C[IIPT * 6 + j] *= J; }
     for (int j = 0; j < 6; j++) { C[j * 6 + IIPT] *= J; }
+    if (flags & 4) {
+      // R12: the loss fluctuates with variance sigma_E^2 (evaluated with the momentum the state arrives with); a shift
+      // dE of the energy moves ipt by ipt1 (E1 / p1^2) dE at fixed direction
+      double k = u[IIPT] * E1 / (p1 * p1);
+      C[IIPT * 6 + IIPT] += k * k * straggling_var(p, t);
+    }
   }
   if (flags & 1) {
     if (th0_out) *th0_out = th0;
@@ -257,10 +273,14 @@ double cos_alpha(const double* u) {
   return (u[IX] * std::cos(u[IPHI]) + u[IY] * std::sin(u[IPHI])) / std::hypot(u[IX], u[IY]);
 }
 
+// R13 (SURVEY f4 "non-uniform field hook"; PAPER.md:41 lists the magnetic field among the ingredients of the
+// lightweight geometry): the step that ends on layer l runs in the uniform field bz_layer[l].
+inline double bz_of(const mkfo_geometry* g, int layer) { return g->bz_layer ? (double)g->bz_layer[layer] : (double)g->bz; }
+
 // One filter step of C7/C9 up to (not including) the update: propagate -> grazing test -> material.
 // returns 0, or a status bit. `skip` semantics are decided by the caller.
 int step_to_layer(const mkfo_geometry* g, const mkfo_params* p, const mkfo_layer& L, const State& in, State& out) {
-  int rc = propagate(L.kind, (double)L.pos, (double)g->bz, in, out, nullptr, nullptr);
+  int rc = propagate(L.kind, (double)L.pos, bz_of(g, (int)(&L - g->layers)), in, out, nullptr, nullptr);
   if (rc) return rc;
   if (L.kind == 0) { if (cos_alpha(out.u) < (double)p->graze_cos_min) return MKFO_GRAZING; }
   else { if (std::fabs(std::cos(out.u[ITH])) < DISK_GRAZE_COS) return MKFO_GRAZING; }
@@ -388,6 +408,7 @@ int mkfo_material_dir(int kind, double xx0, int flags, int dir, double* u, doubl
 }
 double mkfo_dedx(double p) { return dedx(p); }
 double mkfo_highland(double p, double t) { return highland(p, t); }
+double mkfo_straggling_var(double p, double t) { return straggling_var(p, t); }
 
 int mkfo_chi2(const double* u, const double* C, const double* m, const double* V, double* chi2) {
   double uu[6], CC[36]; std::memcpy(uu, u, sizeof(uu)); std::memcpy(CC, C, sizeof(CC));
@@ -510,7 +531,8 @@ int mkfo_fit_backward(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
         if (rc) { stat |= (unsigned)rc; break; }
       }
       State nx;
-      int rc = propagate(L.kind, (double)L.pos, (double)g->bz, cur, nx, nullptr, nullptr, -1);
+      // R13: going back along the arc that the forward step to the layer being left ran on
+      int rc = propagate(L.kind, (double)L.pos, bz_of(g, prev >= 0 ? prev : pl[s]), cur, nx, nullptr, nullptr, -1);
       if (rc) { stat |= (unsigned)rc; break; }
       if (L.kind == 0) { if (cos_alpha(nx.u) < (double)p->graze_cos_min) { stat |= MKFO_GRAZING; break; } }
       else { if (std::fabs(std::cos(nx.u[ITH])) < DISK_GRAZE_COS) { stat |= MKFO_GRAZING; break; } }
@@ -591,7 +613,7 @@ int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
       for (int c = 0; c < (int)live.size(); c++) {
         Cand& cd = live[c];
         State nx;
-        int rc = propagate(L.kind, (double)L.pos, (double)g->bz, cd.st, nx, nullptr, nullptr);
+        int rc = propagate(L.kind, (double)L.pos, bz_of(g, lay), cd.st, nx, nullptr, nullptr);
         bool skip = rc != 0;
         if (!skip) {                                             // acceptance (C9.1)
           double v = L.kind == 0 ? nx.u[IZ] : std::hypot(nx.u[IX], nx.u[IY]);

@@ -27,9 +27,10 @@ typedef struct { int kind;            /* 0 barrel cylinder, 1 disk */
                  float xx0;           /* thickness in radiation lengths at normal incidence */
                  float eta_lo, eta_hi;/* hit pseudorapidity range spanned by the eta bins */ } mkfo_layer;
 typedef struct { int n_layers; const mkfo_layer* layers; float bz; int n_phi_bins, n_eta_bins;
-                 int n_plans; const int* plan_off; const int* plan_layers; } mkfo_geometry;
+                 int n_plans; const int* plan_off; const int* plan_layers;
+                 const float* bz_layer; /* R13 field hook: Bz of the step that ENDS on layer l (NULL: bz everywhere) */ } mkfo_geometry;
 typedef struct { float chi2_cut; int max_cand; int max_consec_miss; int min_hits_keep;
-                 float score_hit, score_miss; float graze_cos_min; int material_flags; /* 1 MS, 2 dE/dx */
+                 float score_hit, score_miss; float graze_cos_min; int material_flags; /* 1 MS, 2 dE/dx, 4 energy-loss straggling (R12) */
                  float dup_frac; } mkfo_params;
 typedef struct { int n_events; int n_hits; const int* layer_off; /* [n_events*(n_layers+1)] */
                  const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */ } mkfo_hits;
@@ -54,6 +55,9 @@ int mkfo_propagate_dir(int kind, double pos, double bz, int q, int dir, const do
 int mkfo_material_dir(int kind, double xx0, int flags, int dir, double* u, double* C, double* theta0_out, double* dE_out);
 /* Bethe-Bloch -dE/dx [GeV/cm] in silicon for a pion of momentum p [GeV]; Highland theta0 for thickness t. */
 double mkfo_dedx(double p);
+/* R12: variance [GeV^2] of the energy lost in silicon of thickness t (radiation lengths along the path) by a pion of
+ * momentum p: xi Tmax (1 - beta^2 / 2), xi = (K/2)(Z/A) rho t X0 / beta^2 (Gaussian straggling). */
+double mkfo_straggling_var(double p, double t);
 double mkfo_highland(double p, double t);
 /* C6: chi2 of hit m (3) with covariance V (6: xx,xy,yy,xz,yz,zz); returns 0 or S_NOT_PD. */
 int mkfo_chi2(const double* u, const double* C, const double* m, const double* V, double* chi2);

@@ -42,7 +42,7 @@ class Layer(C.Structure):
 class Geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("layers", C.POINTER(Layer)), ("bz", C.c_float),
                 ("n_phi_bins", C.c_int), ("n_eta_bins", C.c_int), ("n_plans", C.c_int),
-                ("plan_off", C.POINTER(C.c_int)), ("plan_layers", C.POINTER(C.c_int))]
+                ("plan_off", C.POINTER(C.c_int)), ("plan_layers", C.POINTER(C.c_int)), ("bz_layer", C.POINTER(C.c_float))]
 
 
 class Params(C.Structure):
@@ -68,6 +68,8 @@ def lib():
         _lib.mkfo_dedx.argtypes = [C.c_double]
         _lib.mkfo_highland.restype = C.c_double
         _lib.mkfo_highland.argtypes = [C.c_double, C.c_double]
+        _lib.mkfo_straggling_var.restype = C.c_double
+        _lib.mkfo_straggling_var.argtypes = [C.c_double, C.c_double]
     return _lib
 
 
@@ -101,8 +103,10 @@ class Oracle:
                                                  float(l["xx0"]), float(l["eta_lo"]), float(l["eta_hi"])) for l in lay])
         self._plan_off = _i32(geom["plan_off"])
         self._plan_layers = _i32(geom["plan_layers"])
+        self._bz_layer = _f32(geom["bz_layer"]) if geom.get("bz_layer") is not None else None      # R13 field hook
         self.g = Geometry(len(lay), self._layers, float(geom["bz"]), int(geom["n_phi_bins"]), int(geom["n_eta_bins"]),
-                          len(self._plan_off) - 1, _p(self._plan_off, C.c_int), _p(self._plan_layers, C.c_int))
+                          len(self._plan_off) - 1, _p(self._plan_off, C.c_int), _p(self._plan_layers, C.c_int),
+                          _p(self._bz_layer, C.c_float) if self._bz_layer is not None else None)
         self.p = Params(float(params["chi2_cut"]), int(params["max_cand"]), int(params["max_consec_miss"]),
                         int(params["min_hits_keep"]), float(params["score_hit"]), float(params["score_miss"]),
                         float(params["graze_cos_min"]), int(params["material_flags"]), float(params["dup_frac"]))
@@ -258,6 +262,10 @@ def dedx(p):
 
 def highland(p, t):
     return lib().mkfo_highland(float(p), float(t))
+
+
+def straggling_var(p, t):
+    return lib().mkfo_straggling_var(float(p), float(t))
 
 
 def chi2(u, Cm, m, V6):

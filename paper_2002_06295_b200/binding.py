@@ -29,7 +29,7 @@ class Layer(C.Structure):
 class Geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("layers", C.POINTER(Layer)), ("bz", C.c_float), ("n_phi_bins", C.c_int),
                 ("n_eta_bins", C.c_int), ("n_plans", C.c_int), ("plan_off", C.POINTER(C.c_int)),
-                ("plan_layers", C.POINTER(C.c_int))]
+                ("plan_layers", C.POINTER(C.c_int)), ("bz_layer", C.POINTER(C.c_float))]
 
 
 class Params(C.Structure):
@@ -142,9 +142,12 @@ class Context:
                                                  float(l["xx0"]), float(l["eta_lo"]), float(l["eta_hi"])) for l in lay])
         self._plan_off = np.ascontiguousarray(geom["plan_off"], np.int32)
         self._plan_layers = np.ascontiguousarray(geom["plan_layers"], np.int32)
+        bzl = geom.get("bz_layer")
+        self._bz_layer = np.ascontiguousarray(bzl, np.float32) if bzl is not None else None
         g = Geometry(len(lay), self._layers, float(geom["bz"]), int(geom["n_phi_bins"]), int(geom["n_eta_bins"]),
                      len(self._plan_off) - 1, self._plan_off.ctypes.data_as(C.POINTER(C.c_int)),
-                     self._plan_layers.ctypes.data_as(C.POINTER(C.c_int)))
+                     self._plan_layers.ctypes.data_as(C.POINTER(C.c_int)),
+                     self._bz_layer.ctypes.data_as(C.POINTER(C.c_float)) if self._bz_layer is not None else None)
         p = Params(float(params["chi2_cut"]), int(params["max_cand"]), int(params["max_consec_miss"]),
                    int(params["min_hits_keep"]), float(params["score_hit"]), float(params["score_miss"]),
                    float(params["graze_cos_min"]), int(params["material_flags"]), float(params["dup_frac"]))

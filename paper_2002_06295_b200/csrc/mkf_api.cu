@@ -17,6 +17,7 @@ extern "C" int mkf_create(mkf_ctx** out, const mkf_geometry* geom, const mkf_par
     const mkf_layer& s = geom->layers[l];
     LayerDev& d = c->g.layers[l];
     d.kind = s.kind; d.pos = s.pos; d.lo = s.lo; d.hi = s.hi; d.xx0 = s.xx0; d.eta_lo = s.eta_lo; d.eta_hi = s.eta_hi;
+    c->g.bz_layer[l] = geom->bz_layer ? geom->bz_layer[l] : geom->bz;
     if ((s.kind != 0 && s.kind != 1) || !(s.eta_hi > s.eta_lo) || (s.kind == 0 && !(s.pos > 0.f))) { delete c; return MKF_INVALID_ARG; }
   }
   int mpl = 0;

@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(128) bs_seed_kernel(const __grid_constant__ Ge
   else {
     p0 = g.plan_off[pl];
     plen = min(g.plan_off[pl + 1] - p0, mpl);
-    const float aq = -(float)a.q[i] * KAPPA * g.bz;
+    const float qk = -(float)a.q[i] * KAPPA;
     const int* loff = a.hits.layer_off + (size_t)ev * (g.n_layers + 1);
     for (int k = 0; k < 3 && ok; k++) {
       const int hid = a.seed_hits[(size_t)k * n + i];
@@ -183,8 +183,8 @@ __global__ void __launch_bounds__(128) bs_seed_kernel(const __grid_constant__ Ge
       int step = -1;
       if (lay >= 0) for (int s = last_step + 1; s < plen; s++) if ((int)g.plan_layers[p0 + s] == lay) { step = s; break; }
       if (step < 0) { stat |= ST_TRUNC; ok = false; break; }
-      const LayerDev L = g.layers[lay];
-      const unsigned rc = step_to_layer(S, !has_ud, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
+      const LayerDev& L = g.layers[lay];
+      const unsigned rc = step_to_layer(S, !has_ud, a.cov, n, (size_t)i, L, qk * g.bz_layer[lay], p.graze_cos_min, p.material_flags, false);
       if (rc) { stat |= rc; ok = false; break; }
       has_ud = true;
       Hit H; load_hit(H, a.hits, hid);
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       int p0 = 0, plen = 0;
       if (seed_ok) { const int pl = a.plan[i]; p0 = g.plan_off[pl]; plen = min(g.plan_off[pl + 1] - p0, mpl); }
       sm.p0[sl] = p0; sm.plen[sl] = plen; sm.ev[sl] = seed_ok ? a.seed_event[i] : 0; sm.last[sl] = seed_last; sm.seed[sl] = i;
-      sm.aq[sl] = -(float)a.q[i] * KAPPA * g.bz;
+      sm.aq[sl] = -(float)a.q[i] * KAPPA;                     // times Bz of the step (R13)
       sm.n_live[sl] = seed_ok ? 1 : 0;
       if (seed_ok) {
 #pragma unroll
@@ -374,10 +374,10 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       const int slot = sm.plist[tid];
       const int ssl = slot >> 3;
       const int lay = g.plan_layers[sm.p0[ssl] + s];
-      const LayerDev L = g.layers[lay];
+      const LayerDev& L = g.layers[lay];
       KState S; ld_state(sm.A, slot, S);
       Prop P;
-      const unsigned rc = propagate_geom(S, L, sm.aq[ssl], p.graze_cos_min, p.material_flags, true, P);
+      const unsigned rc = propagate_geom(S, L, sm.aq[ssl] * g.bz_layer[lay], p.graze_cos_min, p.material_flags, true, P);
       const int cn = sm.cnt[slot];
       const int nh = cn & 0xff, consec = cn >> 16;
       if (rc & (ST_UNREACH | ST_SKIP_ACC)) {

@@ -13,6 +13,7 @@ struct GeomDev {
   int plan_off[MAX_PLANS + 1];
   unsigned char plan_layers[MAX_PLAN_STEPS];
   LayerDev layers[MAX_LAYERS];
+  float bz_layer[MAX_LAYERS];          // R13: field of the step that ends on the layer (all = bz without the hook)
 };
 
 struct ParamsDev {
@@ -111,7 +112,7 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
   const int p0 = g.plan_off[pl];
   int plen = g.plan_off[pl + 1] - p0;
   if (plen > a.max_plan_len) plen = a.max_plan_len;
-  const float aq = -(float)a.q[i] * KAPPA * g.bz;
+  const float qk = -(float)a.q[i] * KAPPA;                       // a = qk Bz of the step (R13)
   unsigned stat = 0;
   int stop_at = plen;
 #ifdef __CUDA_ARCH__
@@ -141,9 +142,10 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
       hid_next = s + 1 < stop_at_loop ? *th : -1;
       if (hid < 0 || stopped) continue;
       if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; continue; }    // not a hit of this call
-      const LayerDev L = g.layers[g.plan_layers[p0 + s]];
+      const int li = g.plan_layers[p0 + s];
+      const LayerDev& L = g.layers[li];
       Hit H; load_hit(H, a.hits, hid);
-      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, aq, p.graze_cos_min, p.material_flags, false);
+      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
       if (rc) { stat |= rc; stopped = true; continue; }
       SInv o; float c2;
       hit_to_local(S, H, o);
@@ -178,7 +180,7 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
   const int p0 = g.plan_off[pl];
   int plen = g.plan_off[pl + 1] - p0;
   if (plen > a.max_plan_len) plen = a.max_plan_len;
-  const float aq = -(float)a.q[i] * KAPPA * g.bz;
+ const float qk = -(float)a.q[i] * KAPPA;
   unsigned stat = 0;
   int stop_at = -1;                                              // steps <= stop_at are not processed
   KState S;
@@ -196,20 +198,20 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
       if (hid >= 0 && !stopped) do {
         if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; break; }
         const int li = g.plan_layers[p0 + s];
-        const LayerDev L = g.layers[li];
+        const LayerDev& L = g.layers[li];
         Hit H; load_hit(H, a.hits, hid);
         Prop P;
-        float J = 1.f, th02 = 0.f, ipt_old = S.ipt;
+        float J = 1.f, th02 = 0.f, q4 = 0.f, ipt_old = S.ipt;
         if (nf > 0) {                                            // give back the material of the layer being left
-          const LayerDev Lp = g.layers[prev];
+          const LayerDev& Lp = g.layers[prev];
           float rp;
-          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
+          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
           S.ipt = ipt_old * rp;                                  // the geometry uses the momentum after the give-back
         }
-        const unsigned rc = propagate_geom<-1>(S, L, aq, p.graze_cos_min, 0, false, P);
+        const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[nf > 0 ? prev : li], p.graze_cos_min, 0, false, P);     // R13: back along the arc of the layer being left
         if (rc) { S.ipt = ipt_old; stat |= rc; stopped = true; break; }
         if (nf == 0) { float c[21]; load_cov(c, a.cov, n, (size_t)i); commit_first(S, c, P, 0); }
-        else commit_step_backward(S, P, J, th02, p.material_flags);
+        else commit_step_backward(S, P, J, th02, q4, p.material_flags);
         SInv o; float c2;
         hit_to_local(S, H, o);
         if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break; }
@@ -225,12 +227,13 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     float l[15], c[21];
     ud_to_cov(S.u, S.d, l);
     if (stat == 0) {                                             // give back the innermost layer's material
-      const LayerDev Lp = g.layers[prev];
-      float rp, J, th02;
-      material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02);
+      const LayerDev& Lp = g.layers[prev];
+      float rp, J, th02, q4;
+      material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
       S.ipt *= rp;
 #pragma unroll
       for (int k = 0; k < 5; k++) l[LI(1, k)] *= (k == 1 ? J * J : J);
+      l[LI(1, 1)] += q4;
       if (p.material_flags & 1) {
         const float g3 = -S.ipt * fast_div(S.cth, S.sth), g2 = fast_rcp(S.sth);
         l[LI(1, 1)] += g3 * g3 * th02; l[LI(2, 1)] += g3 * th02; l[LI(2, 2)] += th02; l[LI(0, 0)] += g2 * g2 * th02;

@@ -100,6 +100,17 @@ def _dedx_si(p):
     return 0.307075e-3 * (14.0 / 28.0855) * 2.329 / b2 * (0.5 * np.log(2 * M_E * bg2 * tmax / (173e-9) ** 2) - b2)
 
 
+def _sigma_e(p, t):
+    """Width [GeV] of the energy-loss fluctuation in thickness t (radiation lengths along the path): Bohr's variance
+    with the relativistic factor, xi Tmax (1 - beta^2/2) (the truth straggles as a Gaussian of this width)."""
+    E = np.sqrt(p * p + M_PION ** 2)
+    b2 = (p / E) ** 2
+    g = E / M_PION
+    tmax = 2 * M_E * (p / M_PION) ** 2 / (1 + 2 * g * M_E / M_PION + (M_E / M_PION) ** 2)
+    xi = 0.5 * 0.307075e-3 * (14.0 / 28.0855) * 2.329 * (t * 9.37) / b2
+    return np.sqrt(xi * tmax * (1 - 0.5 * b2))
+
+
 def _theta0(p, t):
     E = np.sqrt(p * p + M_PION ** 2)
     return 0.0136 / ((p / E) * p) * np.sqrt(t) * (1 + 0.038 * np.log(t))
@@ -140,13 +151,14 @@ def _step(a, st, s):
     return [x + s * sc * np.cos(phi + h), y + s * sc * np.sin(phi + h), z + s / np.tan(th), ipt, phi + w * s, th]
 
 
-def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30):
+def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30, straggle=False, scatter=True):
     """Step every particle through its plan. Returns per plan step, per particle: hit position (3), the layer,
     and a validity mask; also the truth state after the last crossed layer (after its material).
     st0 = [x,y,z,ipt,phi,theta] arrays (float64)."""
     n = len(q)
     layers = geom["layers"]
-    a = -q * KAPPA * geom["bz"]
+    a0 = -q * KAPPA
+    bz_layer = geom.get("bz_layer")                       # field hook: Bz of the step that ends on a layer
     st = [np.array(v, float) for v in st0]
     alive = np.ones(n, bool)
     plan_off, plan_layers = geom["plan_off"], geom["plan_layers"]
@@ -158,11 +170,13 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
         g1, g2 = rng.standard_normal(n), rng.standard_normal(n)
         ue = rng.random(n)
         ga, gb = rng.standard_normal(n), rng.standard_normal(n)
+        gs = rng.standard_normal(n) if straggle else None   # drawn only when asked for: the other workloads keep their draws
         for pl in range(len(plan_off) - 1):
             if step >= plan_off[pl + 1] - plan_off[pl]:
                 continue
             li = int(plan_layers[plan_off[pl] + step])
             lay = layers[li]
+            a = a0 * (geom["bz"] if bz_layer is None else float(bz_layer[li]))
             sel = alive & (plan_of == pl)
             if not sel.any():
                 continue
@@ -210,8 +224,12 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
                 p = 1.0 / (np.abs(nx[3]) * np.abs(sth))
                 th0 = _theta0(p, t)
                 E = np.sqrt(p * p + M_PION ** 2) - _dedx_si(p) * t * 9.37
+                if straggle:
+                    E = E + gs[jj] * _sigma_e(p, t)
                 stopped = E <= M_PION * 1.0001
                 p1 = np.sqrt(np.maximum(E * E - M_PION ** 2, 1e-12))
+                if not scatter:                              # energy loss only (isolates the straggling term in the pins)
+                    th0 = 0.0 * th0
                 th_new = nx[5] + ga[jj] * th0
                 ph_new = nx[4] + gb[jj] * th0 / sth
                 nx[5] = th_new
@@ -277,7 +295,7 @@ def three_point_seed(bz, h1, h2, h3, V1, inflate=100.0):
 # ------------------------------------------------------------------------------------------------------
 def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spectrum="loguniform",
                 pt_range=(0.5, 10.0), n_hard=0, eta_max=1.0, eff=1.0, material=True, shuffle=True,
-                seed_on_pixel=False, inflate=100.0):
+                seed_on_pixel=False, inflate=100.0, straggle=False, scatter=True):
     """Returns dict(hits=..., truth_hits [mpl][n_part], seeds=..., ...). Particles 0..n_primary-1 of each event are
     'primary' (seed candidates), the rest 'secondary' (hits only). Draw order: per particle (pT, eta, phi, q, vx,
     vy, vz) as whole arrays, then `simulate`'s per-step draws, then noise (phi, l) per layer, then the shuffle."""
@@ -301,7 +319,7 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
     theta = 2 * np.arctan(np.exp(-eta))
     plan_of = np.zeros(n, np.int8) if len(geom["plan_off"]) == 2 else np.where(eta >= 0, 0, 1).astype(np.int8)
     hx, hy, hz, hl, final_state = simulate(geom, rng, ev_of, plan_of, q.astype(float), [vx, vy, vz, 1.0 / pt, phi, theta],
-                              eff=eff, material=material)
+                              eff=eff, material=material, straggle=straggle, scatter=scatter)
     mpl = hx.shape[0]
     nl = len(geom["layers"])
     # signal hits
