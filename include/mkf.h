@@ -47,7 +47,8 @@ enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total
 
 /* workspace query ids */
 enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3,
-       MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips, n_seeds = capacity */ };
+       MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips, n_seeds = capacity */,
+       MKF_CALL_FIT_SMOOTH = 5 /* n_seeds = number of tracks; for max_plan_len = mkf_max_plan_len(ctx) */ };
 
 typedef struct mkf_ctx mkf_ctx;       /* opaque: geometry, parameters, last error text */
 
@@ -138,6 +139,19 @@ int mkf_fit(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed cha
  * first failing step and keeps the state after its last good update. */
 int mkf_fit_backward(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed char* plan, const int* track_hits,
             int max_plan_len, mkf_states* out, float* chi2, int* nfit, unsigned* status,
+            void* ws, size_t ws_bytes, void* stream);
+
+/* SURVEY.md f1 / reading R14 of DESIGN.md: two-filter smoother ("Fitting simply applies the KF procedure to
+ * all hits"). Same inputs as mkf_fit. Forward filter keeping, at every fitted hit, the predicted state (propagated,
+ * material applied, hit not yet used); backward filter over the fitted hits from the forward result with covariance
+ * x 1e4; at each hit the weighted mean of the two, in the local frame of the forward point:
+ * M = (P_f + P_b)^-1, a_s = P_f M a, P_s = P_f M P_b. The state at plan step s describes the outer side of that layer.
+ * par_s[max_plan_len][6][n], cov_s[max_plan_len][21][n]: zero where the step has no fitted hit; chi2, nfit, status: the
+ * forward filter's. A track whose forward filter fails at an update, or whose backward filter fails anywhere, is not
+ * smoothed (all zero; status says why). ws: mkf_workspace_bytes(ctx, MKF_CALL_FIT_SMOOTH, 0, 0, n) bytes (24 floats per
+ * track and plan step); max_plan_len must be mkf_max_plan_len(ctx). */
+int mkf_fit_smooth(mkf_ctx*, const mkf_hits*, const mkf_states* seeds, const signed char* plan, const int* track_hits,
+            int max_plan_len, float* par_s, float* cov_s, float* chi2, int* nfit, unsigned* status,
             void* ws, size_t ws_bytes, void* stream);
 
 /* a12 / C9. seeds: n states at their first hit; seed_event[n]; seed_hits[3][n] global hit ids;

@@ -556,6 +556,135 @@ int mkfo_fit_backward(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
   return 0;
 }
 
+// ---- R14: two-filter smoother -----------------------------------------------------------------
+namespace {
+// local frame of a surface at point u: rows (in-surface 1, in-surface 2, ipt, phi, theta); barrel: tangential, z;
+// disk: x, y. Orthonormal rows; the surface normal is left out (the covariance is null along it, U2).
+void local_frame(int kind, const double* u, double* T /* 5x6 */) {
+  std::memset(T, 0, 30 * sizeof(double));
+  if (kind == 0) { double r = std::hypot(u[IX], u[IY]); T[0 * 6 + IX] = -u[IY] / r; T[0 * 6 + IY] = u[IX] / r; T[1 * 6 + IZ] = 1.0; }
+  else { T[0 * 6 + IX] = 1.0; T[1 * 6 + IY] = 1.0; }
+  T[2 * 6 + IIPT] = 1.0; T[3 * 6 + IPHI] = 1.0; T[4 * 6 + ITH] = 1.0;
+}
+// SPD inverse of an n x n matrix by Cholesky (n <= 5); false if not positive definite.
+bool spd_inverse(int n, const double* A, double* Ainv) {
+  double L[25] = {0}, Li[25] = {0};
+  for (int i = 0; i < n; i++) for (int j = 0; j <= i; j++) {
+    double acc = A[i * n + j];
+    for (int k = 0; k < j; k++) acc -= L[i * n + k] * L[j * n + k];
+    if (i == j) { if (!(acc > 0)) return false; L[i * n + i] = std::sqrt(acc); }
+    else L[i * n + j] = acc / L[j * n + j];
+  }
+  for (int i = 0; i < n; i++) { Li[i * n + i] = 1.0 / L[i * n + i];
+    for (int j = 0; j < i; j++) { double acc = 0; for (int k = j; k < i; k++) acc -= L[i * n + k] * Li[k * n + j];
+      Li[i * n + j] = acc / L[i * n + i]; } }
+  for (int i = 0; i < n; i++) for (int j = 0; j < n; j++) {
+    double acc = 0; for (int k = 0; k < n; k++) acc += Li[k * n + i] * Li[k * n + j]; Ainv[i * n + j] = acc; }
+  return true;
+}
+bool smooth_combine(int kind, const double* uf, const double* Cf, const double* ub, const double* Cb, double* us, double* Cs) {
+  double T[30]; local_frame(kind, uf, T);
+  double a[5], Pf[25], Pb[25], M[25], Mi[25], K[25];
+  for (int i = 0; i < 5; i++) {
+    double acc = 0;
+    for (int k = 0; k < 6; k++) { double d = ub[k] - uf[k]; if (k == IPHI) d = std::remainder(d, 2.0 * PI); acc += T[i * 6 + k] * d; }
+    a[i] = acc;
+  }
+  auto project = [&](const double* C, double* P) {
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) {
+      double acc = 0;
+      for (int k = 0; k < 6; k++) for (int l = 0; l < 6; l++) acc += T[i * 6 + k] * C[k * 6 + l] * T[j * 6 + l];
+      P[i * 5 + j] = acc; } };
+  project(Cf, Pf); project(Cb, Pb);
+  for (int i = 0; i < 25; i++) M[i] = Pf[i] + Pb[i];
+  if (!spd_inverse(5, M, Mi)) return false;
+  for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { double acc = 0; for (int k = 0; k < 5; k++) acc += Pf[i * 5 + k] * Mi[k * 5 + j]; K[i * 5 + j] = acc; }
+  double as[5], Ps[25];
+  for (int i = 0; i < 5; i++) { double acc = 0; for (int k = 0; k < 5; k++) acc += K[i * 5 + k] * a[k]; as[i] = acc; }
+  // P_s = P_f M P_b (= P_f - P_f M P_f, without the difference of large numbers when one side knows next to nothing)
+  for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { double acc = 0; for (int k = 0; k < 5; k++) acc += K[i * 5 + k] * Pb[k * 5 + j]; Ps[i * 5 + j] = acc; }
+  for (int i = 0; i < 5; i++) for (int j = 0; j < i; j++) { double m = 0.5 * (Ps[i * 5 + j] + Ps[j * 5 + i]); Ps[i * 5 + j] = Ps[j * 5 + i] = m; }
+  for (int k = 0; k < 6; k++) { double acc = uf[k]; for (int i = 0; i < 5; i++) acc += T[i * 6 + k] * as[i]; us[k] = acc; }
+  for (int k = 0; k < 6; k++) for (int l = 0; l < 6; l++) {
+    double acc = 0; for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) acc += T[i * 6 + k] * Ps[i * 5 + j] * T[j * 6 + l];
+    Cs[k * 6 + l] = acc; }
+  return true;
+}
+}  // namespace
+
+int mkfo_smooth_combine(int kind, const double* u_f, const double* C_f, const double* u_b, const double* C_b, double* u_s, double* C_s) {
+  return smooth_combine(kind, u_f, C_f, u_b, C_b, u_s, C_s) ? 0 : MKFO_S_NOT_PD;
+}
+
+int mkfo_fit_smooth(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, int n, const float* par,
+             const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
+             int max_plan_len, double* par_s, double* cov_s, double* chi2, int* nfit, unsigned* status) {
+  std::memset(par_s, 0, sizeof(double) * (size_t)max_plan_len * 6 * n);
+  std::memset(cov_s, 0, sizeof(double) * (size_t)max_plan_len * 21 * n);
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < n; i++) {
+    State st; load_state(n, i, par, cov, q, st);
+    const int* pl = g->plan_layers + g->plan_off[plan[i]];
+    int plen = std::min(g->plan_off[plan[i] + 1] - g->plan_off[plan[i]], max_plan_len);
+    double c2tot = 0; int nf = 0; unsigned stat = 0; bool smoothable = true;
+    std::vector<State> pred(plen); std::vector<int> steps;
+    // forward filter (C7), keeping the predicted states
+    for (int s = 0; s < plen; s++) {
+      int hid = track_hits[(size_t)s * n + i];
+      if (hid < 0) continue;
+      const mkfo_layer& L = g->layers[pl[s]];
+      State nx;
+      int rc = step_to_layer(g, p, L, st, nx);
+      if (rc) { stat |= (unsigned)rc; break; }
+      State prd = nx;
+      double m[3], V6[6]; load_hit(h, hid, m, V6);
+      double c2;
+      rc = chi2_update(nx.u, nx.C, m, V6, &c2, true);
+      if (rc) { stat |= (unsigned)rc; smoothable = false; break; }
+      if (has_nan(nx)) { stat |= MKFO_NAN; smoothable = false; break; }
+      pred[s] = prd; steps.push_back(s);
+      st = nx; c2tot += c2; nf++;
+    }
+    chi2[i] = c2tot; nfit[i] = nf; 
+    if (smoothable && nf > 0) {
+      // backward filter (R7) over the fitted hits, from the forward result with a weak prior
+      State cur = st;
+      for (int k = 0; k < 36; k++) cur.C[k] *= 1e4;
+      std::vector<State> sm(plen); bool ok = true; int prev = -1;
+      for (int k = nf - 1; k >= 0 && ok; k--) {
+        int s = steps[k];
+        const mkfo_layer& L = g->layers[pl[s]];
+        State c2s = cur;
+        if (prev >= 0) {
+          const mkfo_layer& Lp = g->layers[prev];
+          int rc = material(Lp.kind, (double)Lp.xx0, p->material_flags, c2s.u, c2s.C, nullptr, nullptr, -1);
+          if (rc) { stat |= (unsigned)rc; ok = false; break; }
+        }
+        State nx;
+        int rc = propagate(L.kind, (double)L.pos, bz_of(g, prev >= 0 ? prev : pl[s]), c2s, nx, nullptr, nullptr, -1);
+        if (rc) { stat |= (unsigned)rc; ok = false; break; }
+        if (L.kind == 0) { if (cos_alpha(nx.u) < (double)p->graze_cos_min) { stat |= MKFO_GRAZING; ok = false; break; } }
+        else { if (std::fabs(std::cos(nx.u[ITH])) < DISK_GRAZE_COS) { stat |= MKFO_GRAZING; ok = false; break; } }
+        double m[3], V6[6], c2; load_hit(h, track_hits[(size_t)s * n + i], m, V6);
+        rc = chi2_update(nx.u, nx.C, m, V6, &c2, true);
+        if (rc) { stat |= (unsigned)rc; ok = false; break; }
+        if (has_nan(nx)) { stat |= MKFO_NAN; ok = false; break; }
+        State out; out.q = nx.q;
+        if (!smooth_combine(L.kind, pred[s].u, pred[s].C, nx.u, nx.C, out.u, out.C)) { stat |= MKFO_S_NOT_PD; ok = false; break; }
+        sm[s] = out;
+        cur = nx; prev = pl[s];
+      }
+      if (ok) for (int k = 0; k < nf; k++) {
+        int s = steps[k];
+        for (int a = 0; a < 6; a++) par_s[((size_t)s * 6 + a) * n + i] = sm[s].u[a];
+        for (int a = 0; a < 6; a++) for (int b = 0; b <= a; b++) cov_s[((size_t)s * 21 + a * (a + 1) / 2 + b) * n + i] = sm[s].C[a * 6 + b];
+      }
+    }
+    status[i] = stat;
+  }
+  return 0;
+}
+
 // ---- C9 ---------------------------------------------------------------------------------------------
 int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, const unsigned* bin_off,
              const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,

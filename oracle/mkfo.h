@@ -82,6 +82,22 @@ int mkfo_mask_hits(int n, int n_hits, const int* hit_ids, int max_plan_len, cons
 int mkfo_fit(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,
              const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
              int max_plan_len, double* par_out, double* cov_out, double* chi2, int* nfit, unsigned* status);
+/* R14 (SURVEY f1 "backward fit + smoother"; "Fitting simply applies the KF procedure to all hits").
+ * Two-filter smoother. Forward filter as mkfo_fit, keeping at every fitted hit k the PREDICTED state (propagated, the
+ * layer's material applied, hit k not yet used: hits 0..k-1). Backward filter (R7) over the fitted hits, seeded with the
+ * forward result at the last fitted hit, covariance x 1e4 (a prior worth 1e-4 of the data); at hit k its FILTERED state
+ * (hits k..last) describes the same place: the outer side of layer k. Smoothed state at hit k = their weighted mean,
+ * taken in the local frame of the forward point (in-surface 1, in-surface 2, ipt, phi, theta): a = T (u_b - u_f),
+ * M = (P_f + P_b)^-1, a_s = P_f M a, P_s = P_f M P_b (symmetrised); u_s = u_f + T^T a_s, C_s = T^T P_s T.
+ * par_s[max_plan_len][6][n], cov_s[max_plan_len][21][n]: smoothed state per plan step (zero where the step has no
+ * fitted hit); chi2 / nfit / status: those of the forward filter. A track whose forward filter fails at an update
+ * (S not PD, NaN) or whose backward filter fails anywhere is not smoothed (all zero, status says why). */
+int mkfo_fit_smooth(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,
+             const float* cov, const signed char* q, const signed char* plan, const int* track_hits,
+             int max_plan_len, double* par_s, double* cov_s, double* chi2, int* nfit, unsigned* status);
+/* The combination step alone (for the pins): forward (u_f, C_f) and backward (u_b, C_b) on a surface of `kind`. */
+int mkfo_smooth_combine(int kind, const double* u_f, const double* C_f, const double* u_b, const double* C_b,
+             double* u_s, double* C_s);
 /* R7. Backward fit: seeds are states on the layer of each track's LAST hit; hits are processed from the last to the
  * first; output = state at the innermost hit before that layer's material. Same arguments as mkfo_fit. */
 int mkfo_fit_backward(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, int n, const float* par,

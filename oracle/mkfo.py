@@ -163,6 +163,20 @@ class Oracle:
         assert rc == 0
         return out
 
+    def fit_smooth(self, h, par, cov, q, plan, track_hits):
+        """R14: par_s (mpl, 6, n), cov_s (mpl, 21, n) smoothed states per plan step (zero where no fitted hit)."""
+        hs = self.hits(h)
+        par, cov, q, plan, th = _f32(par), _f32(cov), _i8(q), _i8(plan), _i32(track_hits)
+        n = par.shape[1]
+        mpl = th.shape[0]
+        out = dict(par_s=np.zeros((mpl, 6, n)), cov_s=np.zeros((mpl, 21, n)), chi2=np.zeros(n), nfit=np.zeros(n, np.int32),
+                   status=np.zeros(n, np.uint32))
+        rc = self.L.mkfo_fit_smooth(C.byref(self.g), C.byref(self.p), C.byref(hs), n, _p(par, C.c_float), _p(cov, C.c_float),
+                                    _p(q, C.c_byte), _p(plan, C.c_byte), _p(th, C.c_int), mpl, _dp(out["par_s"]),
+                                    _dp(out["cov_s"]), _dp(out["chi2"]), _p(out["nfit"], C.c_int), _p(out["status"], C.c_uint))
+        assert rc == 0
+        return out
+
     def build_tracks(self, h, idx, par, cov, q, seed_event, seed_hits, plan, brute_force=False, max_plan_len=None):
         hs = self.hits(h)
         par, cov, q, plan = _f32(par), _f32(cov), _i8(q), _i8(plan)
@@ -254,6 +268,14 @@ def material(kind, xx0, flags, u, Cm):
     th0, dE = C.c_double(0), C.c_double(0)
     rc = lib().mkfo_material(int(kind), C.c_double(xx0), int(flags), _dp(u), _dp(Cm), C.byref(th0), C.byref(dE))
     return rc, u, Cm, th0.value, dE.value
+
+
+def smooth_combine(kind, u_f, C_f, u_b, C_b):
+    """R14: weighted mean of a forward and a backward estimate on a surface. Returns (rc, u_s, C_s)."""
+    u_s, C_s = np.zeros(6), np.zeros((6, 6))
+    a = [np.ascontiguousarray(x, np.float64) for x in (u_f, C_f, u_b, C_b)]
+    rc = lib().mkfo_smooth_combine(int(kind), _dp(a[0]), _dp(a[1]), _dp(a[2]), _dp(a[3]), _dp(u_s), _dp(C_s))
+    return rc, u_s, C_s
 
 
 def dedx(p):

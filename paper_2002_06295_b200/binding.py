@@ -15,10 +15,11 @@ from . import build as _build
 OK, INVALID_ARG, CUDA_ERROR, WORKSPACE_TOO_SMALL, UNSUPPORTED = 0, -1, -2, -3, -4
 PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8, 16, 32
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
+CALL_FIT_SMOOTH = 5
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
            "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_fit_backward_host", "mkf_build_host",
-           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters"]
+           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters", "mkf_fit_smooth"]
 
 
 class Layer(C.Structure):
@@ -94,6 +95,7 @@ def lib():
         L.mkf_mask_hits.argtypes = [vp, i, i, vp, i, vp, vp, vp, i, C.c_float, vp, vp]
         L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
         L.mkf_fit_backward.argtypes = L.mkf_fit.argtypes
+        L.mkf_fit_smooth.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, vp, vp, vp, vp, vp, vp, sz, vp]
         L.mkf_pack_hits.argtypes = [vp, C.POINTER(Hits), vp, vp]
         L.mkf_set_build_counters.argtypes = [vp, vp]
         L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
@@ -241,6 +243,17 @@ class Context:
         """mkf_set_build_counters: int64 CUDA tensor [8] (zeroed by the caller) or None."""
         self._counters = counters                               # keep the tensor alive while the library holds its address
         self._check(self.L.mkf_set_build_counters(self.h, _dev(counters, torch.int64) if counters is not None else None), "mkf_set_build_counters")
+
+    def fit_smooth(self, hits, seeds, plan, track_hits, par_s, cov_s, chi2, nfit, status, ws):
+        """mkf_fit_smooth (reading R14): par_s float32 [mpl, 6, n], cov_s float32 [mpl, 21, n]."""
+        hs = self.hits_struct(hits, _dev)
+        n = int(seeds["par"].shape[1])
+        s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
+        rc = self.L.mkf_fit_smooth(self.h, C.byref(hs), C.byref(s), _dev(plan, torch.int8), _dev(track_hits, torch.int32),
+                                   int(track_hits.shape[0]), _dev(par_s, torch.float32), _dev(cov_s, torch.float32),
+                                   _dev(chi2, torch.float32), _dev(nfit, torch.int32), _dev(status, torch.int32),
+                                   ws.data_ptr(), ws.numel(), _stream())
+        self._check(rc, "mkf_fit_smooth")
 
     def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status, ws=None):
         hs = self.hits_struct(hits, _dev)

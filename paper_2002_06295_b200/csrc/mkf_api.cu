@@ -145,3 +145,41 @@ static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_st
   a.par_out = out->par; a.cov_out = out->cov; a.chi2 = chi2; a.nfit = nfit; a.status = status;
   return fit_launch(c, backward, a, (cudaStream_t)stream);
 }
+
+// ---- two-filter smoother (reading R14) ----------------------------------------------------------------
+__global__ void __launch_bounds__(FIT_BLOCK) mkf_fit_smooth_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ ParamsDev p,
+                                                                   const __grid_constant__ SmoothArgs a) {
+  const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
+  if (i < a.f.n) fit_smooth_one(g, p, a, i);
+}
+
+namespace mkf { size_t smooth_ws_bytes(int n, int mpl) { return align256((size_t)SM_NF * mpl * n * sizeof(float)); } }
+
+extern "C" int mkf_fit_smooth(mkf_ctx* c, const mkf_hits* h, const mkf_states* seeds, const signed char* plan, const int* track_hits,
+                              int max_plan_len, float* par_s, float* cov_s, float* chi2, int* nfit, unsigned* status,
+                              void* ws, size_t ws_bytes, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || !seeds) return fail(c, MKF_INVALID_ARG, "mkf_fit_smooth: null argument");
+  if (seeds->n < 0 || max_plan_len < 1) return fail(c, MKF_INVALID_ARG, "mkf_fit_smooth: bad sizes");
+  if (seeds->n == 0) return MKF_OK;
+  if (!plan || !track_hits || !par_s || !cov_s || !chi2 || !nfit || !status || !h->x || !h->y || !h->z || !h->V ||
+      !seeds->par || !seeds->cov || !seeds->q)
+    return fail(c, MKF_INVALID_ARG, "mkf_fit_smooth: null array");
+  if ((size_t)h->rec & 15) return fail(c, MKF_INVALID_ARG, "mkf_fit_smooth: hit records not 16-byte aligned");
+  const size_t need = smooth_ws_bytes(seeds->n, max_plan_len);
+  if (ws_bytes < need || !ws) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_fit_smooth: workspace too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t n = (size_t)seeds->n;
+  cudaError_t e = cudaMemsetAsync(par_s, 0, n * max_plan_len * 6 * sizeof(float), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(cov_s, 0, n * max_plan_len * 21 * sizeof(float), st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "mkf_fit_smooth: memset");
+  SmoothArgs a;
+  a.f.hits = hits_dev(h);
+  a.f.n = seeds->n; a.f.ld = seeds->n; a.f.par = seeds->par; a.f.cov = seeds->cov; a.f.q = seeds->q; a.f.plan = plan;
+  a.f.track_hits = track_hits; a.f.max_plan_len = max_plan_len;
+  a.f.par_out = nullptr; a.f.cov_out = nullptr; a.f.chi2 = chi2; a.f.nfit = nfit; a.f.status = status;
+  a.par_s = par_s; a.cov_s = cov_s; a.ws = (float*)ws;
+  mkf_fit_smooth_kernel<<<(a.f.n + FIT_BLOCK - 1) / FIT_BLOCK, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
+  MKF_LAUNCHED(c, "mkf_fit_smooth_kernel");
+  return MKF_OK;
+}

@@ -249,3 +249,212 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
 }
 
 }  // namespace mkf
+
+// ---- two-filter smoother of one track (reading R14) ---------------------------------------------------
+// Forward filter as fit_one, keeping the PREDICTED state of every fitted hit (propagated, material applied, hit not yet
+// used) in the workspace; backward filter (R7) over the fitted hits, seeded with the forward result and D x 1e4; at each
+// hit the weighted mean of the stored prediction and the backward filtered state, taken in the local frame of the
+// forward point. The combination runs in double (a 5x5 Cholesky per hit; the filters stay in fp32).
+namespace mkf {
+
+struct SmoothArgs {
+  FitArgs f;                   // par_out / cov_out unused
+  float* par_s;                // [mpl][6][ld]
+  float* cov_s;                // [mpl][21][ld]
+  float* ws;                   // [24][mpl][ld] predicted states
+};
+
+constexpr int SM_NF = 24;      // x, y, z, xl, yl, zl, ipt, phi, th, u[10], d[5]
+
+MKF_HD void ud_to_cov_d(const float* u, const float* d, double* p) {
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j <= i; j++) {
+      double acc = (i == j ? (double)d[i] : (double)u[UI(j, i)] * (double)d[i]);
+#pragma unroll
+      for (int k = i + 1; k < 5; k++) acc += (double)u[UI(i, k)] * (double)d[k] * (double)u[UI(j, k)];
+      p[LI(i, j)] = acc;
+    }
+}
+
+// Smoothed state from the stored forward prediction fw[SM_NF] (on a surface of `kind`) and the backward filtered state
+// Sb. Local order (phi, ipt, theta, w2, w1). Returns false if P_f + P_b is not positive definite.
+MKF_HD bool smooth_combine_dev(const float* fw, int kind, const KState& Sb, float* par6, float* c21) {
+  const double xf = (double)fw[0] + (double)fw[3], yf = (double)fw[1] + (double)fw[4], zf = (double)fw[2] + (double)fw[5];
+  double cbf = 1.0, sbf = 0.0;
+  if (kind == 0) { const double ir = 1.0 / sqrt(xf * xf + yf * yf); cbf = xf * ir; sbf = yf * ir; }
+  double Pf[15], Pb[15];
+  ud_to_cov_d(fw + 9, fw + 19, Pf);
+  ud_to_cov_d(Sb.u, Sb.d, Pb);
+  if (kind == 0) {                                               // the backward frame seen from the forward one
+    const double cosd = cbf * (double)Sb.f.cb + sbf * (double)Sb.f.sb;
+#pragma unroll
+    for (int k = 0; k < 4; k++) Pb[LI(4, k)] *= cosd;
+    Pb[LI(4, 4)] *= cosd * cosd;
+  }
+  const double dx = ((double)Sb.x - (double)fw[0]) + ((double)Sb.xl - (double)fw[3]);
+  const double dy = ((double)Sb.y - (double)fw[1]) + ((double)Sb.yl - (double)fw[4]);
+  const double dz = ((double)Sb.z - (double)fw[2]) + ((double)Sb.zl - (double)fw[5]);
+  double a[5];
+  const double TWO_PI = 6.283185307179586;
+  double dphi = (double)Sb.phi - (double)fw[7];
+  dphi -= TWO_PI * rint(dphi / TWO_PI);
+  a[0] = dphi; a[1] = (double)Sb.ipt - (double)fw[6]; a[2] = (double)Sb.th - (double)fw[8];
+  if (kind == 0) { a[3] = dz; a[4] = cbf * dy - sbf * dx; } else { a[3] = dy; a[4] = dx; }
+  // M = (Pf + Pb)^-1 by Cholesky
+  double L[15], Li[15];
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j <= i; j++) {
+      double acc = Pf[LI(i, j)] + Pb[LI(i, j)];
+#pragma unroll
+      for (int k = 0; k < j; k++) acc -= L[LI(i, k)] * L[LI(j, k)];
+      if (i == j) { if (!(acc > 0.0)) return false; L[LI(i, i)] = sqrt(acc); }
+      else L[LI(i, j)] = acc / L[LI(j, j)];
+    }
+#pragma unroll
+  for (int i = 0; i < 5; i++) {
+    Li[LI(i, i)] = 1.0 / L[LI(i, i)];
+#pragma unroll
+    for (int j = 0; j < i; j++) {
+      double acc = 0.0;
+#pragma unroll
+      for (int k = j; k < i; k++) acc -= L[LI(i, k)] * Li[LI(k, j)];
+      Li[LI(i, j)] = acc * Li[LI(i, i)];
+    }
+  }
+  double M[15];
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j <= i; j++) {
+      double acc = 0.0;
+#pragma unroll
+      for (int k = i; k < 5; k++) acc += Li[LI(k, i)] * Li[LI(k, j)];
+      M[LI(i, j)] = acc;
+    }
+  double K[5][5];
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j < 5; j++) {
+      double acc = 0.0;
+#pragma unroll
+      for (int k = 0; k < 5; k++) acc += Pf[LI(i, k)] * M[LI(k, j)];
+      K[i][j] = acc;
+    }
+  double as[5];
+#pragma unroll
+  for (int i = 0; i < 5; i++) {
+    double acc = 0.0;
+#pragma unroll
+    for (int k = 0; k < 5; k++) acc += K[i][k] * a[k];
+    as[i] = acc;
+  }
+  float l[15];
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j <= i; j++) {
+      double s1 = 0.0, s2 = 0.0;                                 // P_s = P_f M P_b, symmetrised
+#pragma unroll
+      for (int k = 0; k < 5; k++) { s1 += K[i][k] * Pb[LI(k, j)]; s2 += K[j][k] * Pb[LI(k, i)]; }
+      l[LI(i, j)] = (float)(0.5 * (s1 + s2));
+    }
+  Frame ff; ff.kind = kind; ff.cb = (float)cbf; ff.sb = (float)sbf;
+  cov_from_local(l, ff, c21);
+  double xs = xf, ys = yf, zs = zf;
+  if (kind == 0) { xs -= sbf * as[4]; ys += cbf * as[4]; zs += as[3]; } else { xs += as[4]; ys += as[3]; }
+  par6[0] = (float)xs; par6[1] = (float)ys; par6[2] = (float)zs;
+  par6[3] = (float)((double)fw[6] + as[1]); par6[4] = wrap_phi((float)((double)fw[7] + as[0])); par6[5] = (float)((double)fw[8] + as[2]);
+  return true;
+}
+
+MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArgs& sa, int i) {
+  const FitArgs& a = sa.f;
+  const size_t n = (size_t)a.ld;
+  const int mpl = a.max_plan_len;
+  const int pl = a.plan[i];
+  if ((unsigned)pl >= (unsigned)g.n_plans) { a.chi2[i] = 0.f; a.nfit[i] = 0; a.status[i] = ST_TRUNC; return; }
+  const int p0 = g.plan_off[pl];
+  const int plen = min(g.plan_off[pl + 1] - p0, mpl);
+  const float qk = -(float)a.q[i] * KAPPA;
+  unsigned stat = 0;
+  KState S;
+  load_params(S, a.par, n, (size_t)i);
+  float c2tot = 0.f; int nf = 0, last_s = -1; bool smoothable = true;
+  for (int s = 0; s < plen; s++) {
+    const int hid = a.track_hits[(size_t)s * n + i];
+    if (hid < 0) continue;
+    if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; break; }
+    const int li = g.plan_layers[p0 + s];
+    const LayerDev& L = g.layers[li];
+    const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
+    if (rc) { stat |= rc; break; }
+    float* w = sa.ws + (size_t)s * n + i;
+    const size_t st = (size_t)mpl * n;
+    w[0] = S.x; w[st] = S.y; w[2 * st] = S.z; w[3 * st] = S.xl; w[4 * st] = S.yl; w[5 * st] = S.zl;
+    w[6 * st] = S.ipt; w[7 * st] = S.phi; w[8 * st] = S.th;
+#pragma unroll
+    for (int k = 0; k < 10; k++) w[(9 + k) * st] = S.u[k];
+#pragma unroll
+    for (int k = 0; k < 5; k++) w[(19 + k) * st] = S.d[k];
+    Hit H; load_hit(H, a.hits, hid);
+    SInv o; float c2;
+    hit_to_local(S, H, o);
+    if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; smoothable = false; break; }
+    if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; smoothable = false; break; }
+    c2tot += c2; nf++; last_s = s;
+  }
+  a.chi2[i] = c2tot; a.nfit[i] = nf;
+  bool ok = smoothable && nf > 0;
+  if (ok) {
+#pragma unroll
+    for (int k = 0; k < 5; k++) S.d[k] *= 1e4f;                  // the backward filter starts from a weak prior
+    int prev = -1;
+    for (int s = last_s; s >= 0 && ok; s--) {
+      const int hid = a.track_hits[(size_t)s * n + i];
+      if (hid < 0) continue;
+      const int li = g.plan_layers[p0 + s];
+      const LayerDev& L = g.layers[li];
+      float J = 1.f, th02 = 0.f, q4 = 0.f;
+      if (prev >= 0) {
+        const LayerDev& Lp = g.layers[prev];
+        float rp;
+        material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
+        S.ipt *= rp;
+      }
+      Prop P;
+      const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[prev >= 0 ? prev : li], p.graze_cos_min, 0, false, P);
+      if (rc) { stat |= rc; ok = false; break; }
+      commit_step_backward(S, P, J, th02, q4, p.material_flags);
+      Hit H; load_hit(H, a.hits, hid);
+      SInv o; float c2;
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
+      if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; ok = false; break; }
+      float fw[SM_NF];
+      const size_t st = (size_t)mpl * n;
+      const float* w = sa.ws + (size_t)s * n + i;
+#pragma unroll
+      for (int k = 0; k < SM_NF; k++) fw[k] = w[k * st];
+      float par6[6], c21[21];
+      if (!smooth_combine_dev(fw, L.kind, S, par6, c21)) { stat |= ST_S_NOT_PD; ok = false; break; }
+#pragma unroll
+      for (int k = 0; k < 6; k++) sa.par_s[((size_t)s * 6 + k) * n + i] = par6[k];
+#pragma unroll
+      for (int k = 0; k < 21; k++) sa.cov_s[((size_t)s * 21 + k) * n + i] = c21[k];
+      prev = li;
+    }
+    if (!ok)                                                     // not smoothed: every state of the track is zero
+      for (int s = 0; s < mpl; s++) {
+        for (int k = 0; k < 6; k++) sa.par_s[((size_t)s * 6 + k) * n + i] = 0.f;
+        for (int k = 0; k < 21; k++) sa.cov_s[((size_t)s * 21 + k) * n + i] = 0.f;
+      }
+  }
+  a.status[i] = stat;
+}
+
+}  // namespace mkf

@@ -14,6 +14,7 @@ size_t hit_index_ws_bytes(const mkf_ctx* c, int n_events, int n_hits);
 size_t dedup_ws_bytes(int n_hits, int n, int mpl);
 size_t strips_ws_bytes(int n_strips, int capacity);
 size_t build_ws_bytes(const mkf_ctx* c, int n_events, int n_seeds);
+size_t smooth_ws_bytes(int n, int mpl);
 int fit_launch(mkf_ctx* c, bool backward, const FitArgs& a, cudaStream_t st);
 }
 using namespace mkf;
@@ -25,6 +26,7 @@ extern "C" size_t mkf_workspace_bytes(const mkf_ctx* c, int call_id, int n_event
     case MKF_CALL_REMOVE_DUPLICATES: return dedup_ws_bytes(n_hits, n_seeds, c->max_plan_len);
     case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits, n_seeds);
     case MKF_CALL_BUILD_TRACKS: return build_ws_bytes(c, n_events, n_seeds);
+    case MKF_CALL_FIT_SMOOTH: return smooth_ws_bytes(n_seeds, c->max_plan_len);
     default: return 0;      // the fit keeps everything in registers
   }
 }

@@ -151,7 +151,7 @@ def _step(a, st, s):
     return [x + s * sc * np.cos(phi + h), y + s * sc * np.sin(phi + h), z + s / np.tan(th), ipt, phi + w * s, th]
 
 
-def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30, straggle=False, scatter=True):
+def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30, straggle=False, scatter=True, keep_truth=False):
     """Step every particle through its plan. Returns per plan step, per particle: hit position (3), the layer,
     and a validity mask; also the truth state after the last crossed layer (after its material).
     st0 = [x,y,z,ipt,phi,theta] arrays (float64)."""
@@ -165,6 +165,7 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
     mpl = int(np.max(np.diff(plan_off)))
     hx = np.zeros((mpl, n)); hy = np.zeros((mpl, n)); hz = np.zeros((mpl, n))
     hl = np.full((mpl, n), -1, np.int32)
+    tstates = np.full((mpl, 6, n), np.nan) if keep_truth else None    # truth after each crossed layer (after its material)
     for step in range(mpl):
         # fixed draw order per step: smear1, smear2, efficiency, scatter alpha, scatter beta
         g1, g2 = rng.standard_normal(n), rng.standard_normal(n)
@@ -238,6 +239,10 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
                 alive[jj[stopped]] = False
             for k in range(6):
                 st[k][jj] = nx[k]
+                if keep_truth:
+                    tstates[step, k, jj] = nx[k]
+    if keep_truth:
+        return hx, hy, hz, hl, np.stack(st), tstates
     return hx, hy, hz, hl, np.stack(st)
 
 
@@ -295,7 +300,7 @@ def three_point_seed(bz, h1, h2, h3, V1, inflate=100.0):
 # ------------------------------------------------------------------------------------------------------
 def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spectrum="loguniform",
                 pt_range=(0.5, 10.0), n_hard=0, eta_max=1.0, eff=1.0, material=True, shuffle=True,
-                seed_on_pixel=False, inflate=100.0, straggle=False, scatter=True):
+                seed_on_pixel=False, inflate=100.0, straggle=False, scatter=True, keep_truth=False):
     """Returns dict(hits=..., truth_hits [mpl][n_part], seeds=..., ...). Particles 0..n_primary-1 of each event are
     'primary' (seed candidates), the rest 'secondary' (hits only). Draw order: per particle (pT, eta, phi, q, vx,
     vy, vz) as whole arrays, then `simulate`'s per-step draws, then noise (phi, l) per layer, then the shuffle."""
@@ -318,8 +323,9 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
     q = np.where(u_q < 0.5, -1, 1).astype(np.int8)
     theta = 2 * np.arctan(np.exp(-eta))
     plan_of = np.zeros(n, np.int8) if len(geom["plan_off"]) == 2 else np.where(eta >= 0, 0, 1).astype(np.int8)
-    hx, hy, hz, hl, final_state = simulate(geom, rng, ev_of, plan_of, q.astype(float), [vx, vy, vz, 1.0 / pt, phi, theta],
-                              eff=eff, material=material, straggle=straggle, scatter=scatter)
+    sim = simulate(geom, rng, ev_of, plan_of, q.astype(float), [vx, vy, vz, 1.0 / pt, phi, theta],
+                   eff=eff, material=material, straggle=straggle, scatter=scatter, keep_truth=keep_truth)
+    hx, hy, hz, hl, final_state = sim[:5]
     mpl = hx.shape[0]
     nl = len(geom["layers"])
     # signal hits
@@ -384,6 +390,8 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
                  track_hits=np.ascontiguousarray(truth_hits[:, sid]))
     truth = dict(pt=pt, eta=eta, phi=phi, q=q, vx=vx, vy=vy, vz=vz, theta=theta, event=ev_of, primary=primary,
                  final_state=final_state)
+    if keep_truth:
+        truth["states"] = sim[5]                          # (mpl, 6, n_particles): truth after each crossed layer
     return dict(geom=geom, hits=hits, truth_hits=truth_hits, hit_particle=PART.astype(np.int32), hit_layer=LAY.astype(np.int32),
                 seeds=seeds, truth=truth, max_plan_len=mpl)
 
