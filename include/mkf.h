@@ -48,7 +48,8 @@ enum { MKF_MAX_LAYERS = 64, MKF_MAX_PLANS = 8, MKF_MAX_PLAN_STEPS = 192 /* total
 /* workspace query ids */
 enum { MKF_CALL_BUILD_HIT_INDEX = 0, MKF_CALL_FIT = 1, MKF_CALL_BUILD_TRACKS = 2, MKF_CALL_REMOVE_DUPLICATES = 3,
        MKF_CALL_CLUSTER_STRIPS = 4 /* n_hits = number of strips, n_seeds = capacity */,
-       MKF_CALL_FIT_SMOOTH = 5 /* n_seeds = number of tracks; for max_plan_len = mkf_max_plan_len(ctx) */ };
+       MKF_CALL_FIT_SMOOTH = 5 /* n_seeds = number of tracks; for max_plan_len = mkf_max_plan_len(ctx) */,
+       MKF_CALL_BUILD_TRACKS_OVERLAP = 6 };
 
 typedef struct mkf_ctx mkf_ctx;       /* opaque: geometry, parameters, last error text */
 
@@ -85,7 +86,10 @@ typedef struct { float chi2_cut;      /* hit accepted iff chi2 < chi2_cut (30) *
  * every kernel that gathers by id reads `rec` when it is given. x, y, z, V must be valid in either case. */
 typedef struct { int n_events; int n_hits; const int* layer_off;
                  const float *x, *y, *z; const float* V; /* V[6][n_hits]: xx,xy,yy,xz,yz,zz */
-                 const float* rec; } mkf_hits;
+                 const float* rec;
+                 const int* module; /* [n_hits] detector module of each hit, or NULL. Only overlap-hit recovery reads it
+                                       (mkf_build_tracks_overlap); mkf_build_hit_index copies it into the packed records. */
+               } mkf_hits;
 
 /* The phi/eta-binned hit index (C8), written by mkf_build_hit_index, read by mkf_build_tracks.
  * bin_off  [n_events*n_layers*n_phi*n_eta + 1]  exclusive prefix of hits per bin (bin = ie*n_phi + ip inside
@@ -93,7 +97,7 @@ typedef struct { int n_events; int n_hits; const int* layer_off;
  * sorted_id[n_hits]  hit ids ordered by (segment, bin, id);
  * vmax     [n_events*n_layers*2]  per segment: max over hits of the larger eigenvalue of the xy block of V, max V_zz;
  * packed   [n_hits*12]  the hits in sorted order, as a block of n_hits 16-byte positions {x,y,z,id(bits)} followed by
- *          a block of n_hits 32-byte covariances {Vxx,Vxy,Vyy,Vxz | Vyz,Vzz,0,0} (a derived copy so that a bin scan
+ *          a block of n_hits 32-byte covariances {Vxx,Vxy,Vyy,Vxz | Vyz,Vzz,module(bits),0} (a derived copy so that a bin scan
  *          reads contiguous memory; may be NULL in mkf_build_hit_index, in which case mkf_build_tracks gathers from
  *          the SoA arrays instead). */
 typedef struct { unsigned* bin_off; int* sorted_id; float* vmax; float* packed; } mkf_hit_index;
@@ -168,6 +172,20 @@ int mkf_build_tracks(mkf_ctx*, const mkf_hits*, const mkf_hit_index*, const mkf_
             const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
             mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status,
             void* ws, size_t ws_bytes, void* stream);
+
+/* SURVEY.md f2 / reading R15 of DESIGN.md: mkf_build_tracks with overlap-hit recovery ("the recovery of hits
+ * in overlapping detector modules, so that more than one hit per layer can be assigned to tracks"). hits->module must
+ * be given (also to mkf_build_hit_index, if its packed records are used). A candidate that took hit h1 on a layer may
+ * take ONE more hit of that layer: the best one (chi2 against the state already updated with h1, below chi2_cut) among
+ * its parent's max_cand best hits of the layer (by chi2 against the propagated state) that rank after h1 in that list
+ * (a pair is then made once, by the child of its better hit), with module[h2] != module[h1]. The state is updated again; chi2, nhits and score include it (an update that does not stay finite is not
+ * taken). The ranking of the layer is done on the first hits alone. hit_ids2[max_plan_len][n]: the second hit of each
+ * plan step, or -2. ws: mkf_workspace_bytes(ctx, MKF_CALL_BUILD_TRACKS_OVERLAP, n_events, n_hits, n_seeds).
+ * mkf_remove_duplicates and mkf_fit keep working on hit_ids (one hit per layer). */
+int mkf_build_tracks_overlap(mkf_ctx*, const mkf_hits*, const mkf_hit_index*, const mkf_states* seeds,
+            const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
+            mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, int* hit_ids2,
+            unsigned* status, void* ws, size_t ws_bytes, void* stream);
 
 /* Work counters of mkf_build_tracks (SURVEY.md §8d asks for candidate-layer-steps/s and chi2 evaluations/s): while
  * `counters` (device, 8 x unsigned long long, zeroed by the caller) is set, every mkf_build_tracks call on this context

@@ -349,6 +349,7 @@ void window(const mkfo_geometry* g, const mkfo_params* p, int layer, const doubl
 struct Cand {
   State st; double chi2; int nhits, nmiss, consec; unsigned status;
   std::vector<int> hits;                                         // per plan step: id | -1 | -2
+  std::vector<int> hits2;                                        // R15: a second hit of the step (overlapping module) | -2
 };
 struct Child { double score, chi2; int parent; int hit; int kind; /* 0 hit, 1 miss, 2 pass-through */ };
 const int HIT_INF = std::numeric_limits<int>::max();
@@ -686,12 +687,22 @@ int mkfo_fit_smooth(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hit
 }
 
 // ---- C9 ---------------------------------------------------------------------------------------------
-int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, const unsigned* bin_off,
+}  // extern "C"
+namespace {
+// R15 ("the recovery of hits in overlapping detector modules, so that more than one hit per layer
+// can be assigned to tracks"): with `module` given (module id per hit; overlapping modules of a layer sit on the same
+// surface of the lightweight geometry), a child that took hit h1 on a layer may take ONE more hit of that layer: h2 is
+// looked for among its parent's N_c best hits of the layer (by chi2 against the propagated state, the list the
+// selection works on) that rank after h1 in that list, with module[h2] != module[h1]; its chi2 against the state already updated with h1 (C6:
+// no propagation, no material) must be below the cut; the smallest such chi2 wins (first in list order on a tie). The
+// state is updated again, chi2 += chi2_2, nhits += 1 (so the score gains score_hit - chi2_2); an update that does not
+// stay finite is not taken. The ranking of the layer itself (C9.6) is done on the first hits alone.
+int build_tracks_impl(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, const unsigned* bin_off,
              const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,
              const float* cov, const signed char* q, const int* seed_event, const int* seed_hits,
              const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
              double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
-             long long* n_chi2_evals) {
+             long long* n_chi2_evals, const int* module, int* hit_ids2) {
   int nl = g->n_layers, nphi = g->n_phi_bins, neta = g->n_eta_bins, nb = nphi * neta;
   long long evals_total = 0;
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : evals_total)
@@ -706,7 +717,7 @@ int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
     // seed candidate: fit the seed state through its own three hits (reading U18b)
     Cand seed; load_state(n, i, par, cov, q, seed.st);
     seed.chi2 = 0; seed.nhits = 0; seed.nmiss = 0; seed.consec = 0; seed.status = 0;
-    seed.hits.assign(max_plan_len, -2);
+    seed.hits.assign(max_plan_len, -2); seed.hits2.assign(max_plan_len, -2);
     int last_step = -1; bool seed_ok = true;
     for (int k = 0; k < 3 && seed_ok; k++) {
       int hid = seed_hits[(size_t)k * n + i];
@@ -791,6 +802,7 @@ int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
         } else ranked.push_back(ch);
       }
       std::sort(ranked.begin(), ranked.end(), child_before);
+      const std::vector<Child>& ranked_all = ranked;              // within one parent: ascending chi2, then hit id
       int nc = p->max_cand;
       if ((int)ranked.size() > nc) note((ranked[nc - 1].score - ranked[nc].score) / p->score_hit);
       std::vector<Cand> next;
@@ -805,6 +817,29 @@ int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
           chi2_update(c.st.u, c.st.C, m, V6, &c2, true);
           c.chi2 += c2; c.nhits++; c.consec = 0; c.hits[s] = ch.hit;
           if (has_nan(c.st)) { c.status |= MKFO_NAN; offer_short(live[ch.parent]); continue; }
+          if (module) {                                          // R15: one more hit from an overlapping module
+            std::vector<Child> plist;                            // the parent's hits of this layer, best first
+            for (const Child& o2 : ranked_all) if (o2.kind == 0 && o2.parent == ch.parent) plist.push_back(o2);
+            int best = -1; double best_c2 = 0; bool after = false;
+            for (int k2 = 0; k2 < (int)plist.size() && k2 < nc; k2++) {
+              int h2 = plist[k2].hit;
+              if (h2 == ch.hit) { after = true; continue; }
+              // only hits that rank AFTER the first one in the parent's list: the pair (h1, h2) is then made once, by the
+              // child of its better hit (the other order would give the same state and a twin candidate)
+              if (!after || module[h2] == module[ch.hit]) continue;
+              double m2[3], V62[6], c2b; load_hit(h, h2, m2, V62);
+              if (chi2_update(c.st.u, c.st.C, m2, V62, &c2b, false)) continue;
+              if (!(c2b < (double)p->chi2_cut)) continue;
+              note((c2b - p->chi2_cut) / p->chi2_cut);
+              if (best < 0 || c2b < best_c2) { best = h2; best_c2 = c2b; }
+            }
+            if (best >= 0) {
+              State s2 = c.st;
+              double m2[3], V62[6], c2b; load_hit(h, best, m2, V62);
+              chi2_update(s2.u, s2.C, m2, V62, &c2b, true);
+              if (!has_nan(s2)) { c.st = s2; c.chi2 += c2b; c.nhits++; c.hits2[s] = best; }
+            }
+          }
         }
         next.push_back(c);
       }
@@ -825,9 +860,30 @@ int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_h
     chi2[i] = out.chi2; score[i] = score_of(p, out.nhits, out.nmiss, out.chi2);
     nhits[i] = out.nhits; nmiss[i] = out.nmiss; status[i] = out.status; margin[i] = mrg;
     for (int s = 0; s < max_plan_len; s++) hit_ids[(size_t)s * n + i] = out.hits[s];
+    if (hit_ids2) for (int s = 0; s < max_plan_len; s++) hit_ids2[(size_t)s * n + i] = out.hits2[s];
   }
   if (n_chi2_evals) *n_chi2_evals = evals_total;
   return 0;
+}
+}  // namespace
+extern "C" {
+int mkfo_build_tracks(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, const unsigned* bin_off,
+             const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,
+             const float* cov, const signed char* q, const int* seed_event, const int* seed_hits,
+             const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
+             double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
+             long long* n_chi2_evals) {
+  return build_tracks_impl(g, p, h, bin_off, sorted_id, vmax, brute_force, n, par, cov, q, seed_event, seed_hits, plan, max_plan_len,
+                           par_out, cov_out, chi2, score, nhits, nmiss, hit_ids, status, margin, n_chi2_evals, nullptr, nullptr);
+}
+int mkfo_build_tracks_overlap(const mkfo_geometry* g, const mkfo_params* p, const mkfo_hits* h, const unsigned* bin_off,
+             const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,
+             const float* cov, const signed char* q, const int* seed_event, const int* seed_hits,
+             const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
+             double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
+             long long* n_chi2_evals, const int* module, int* hit_ids2) {
+  return build_tracks_impl(g, p, h, bin_off, sorted_id, vmax, brute_force, n, par, cov, q, seed_event, seed_hits, plan, max_plan_len,
+                           par_out, cov_out, chi2, score, nhits, nmiss, hit_ids, status, margin, n_chi2_evals, module, hit_ids2);
 }
 
 // ---- C10 --------------------------------------------------------------------------------------------

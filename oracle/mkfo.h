@@ -112,6 +112,16 @@ int mkfo_build_tracks(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*
              const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
              double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
              long long* n_chi2_evals);
+/* R15: mkfo_build_tracks with overlap-hit recovery. module[n_hits]: module id per hit;
+ * hit_ids2[max_plan_len][n]: the second hit taken on a plan step, or -2. A child that took hit h1 may take one more
+ * hit of the same layer from another module: the best (chi2 against the state updated with h1, below the cut) among its
+ * parent's N_c best hits of the layer that rank after h1 there (so a pair is made once, by the child of its better hit). nhits, chi2 and score include it. module == NULL: mkfo_build_tracks. */
+int mkfo_build_tracks_overlap(const mkfo_geometry*, const mkfo_params*, const mkfo_hits*, const unsigned* bin_off,
+             const int* sorted_id, const float* vmax, int brute_force, int n, const float* par,
+             const float* cov, const signed char* q, const int* seed_event, const int* seed_hits,
+             const signed char* plan, int max_plan_len, double* par_out, double* cov_out, double* chi2,
+             double* score, int* nhits, int* nmiss, int* hit_ids, unsigned* status, double* margin,
+             long long* n_chi2_evals, const int* module, int* hit_ids2);
 /* C10. track_off[n_events+1]; hit_ids[max_plan_len][n]; keep[n], n_kept[n_events]. */
 int mkfo_remove_duplicates(const mkfo_params*, int n_events, const int* track_off, const int* hit_ids,
              int max_plan_len, const int* nhits, const float* score, unsigned char* keep, int* n_kept);

@@ -177,7 +177,8 @@ class Oracle:
         assert rc == 0
         return out
 
-    def build_tracks(self, h, idx, par, cov, q, seed_event, seed_hits, plan, brute_force=False, max_plan_len=None):
+    def build_tracks(self, h, idx, par, cov, q, seed_event, seed_hits, plan, brute_force=False, max_plan_len=None, module=None):
+        """module (int32[n_hits], reading R15): overlap-hit recovery; the result then also holds hit_ids2."""
         hs = self.hits(h)
         par, cov, q, plan = _f32(par), _f32(cov), _i8(q), _i8(plan)
         se, sh = _i32(seed_event), _i32(seed_hits)
@@ -190,13 +191,19 @@ class Oracle:
         bo = np.ascontiguousarray(idx["bin_off"], np.uint32)
         si = _i32(idx["sorted_id"])
         vm = _f32(idx["vmax"])
-        rc = self.L.mkfo_build_tracks(C.byref(self.g), C.byref(self.p), C.byref(hs), _p(bo, C.c_uint), _p(si, C.c_int),
-                                      _p(vm, C.c_float), int(bool(brute_force)), n, _p(par, C.c_float),
-                                      _p(cov, C.c_float), _p(q, C.c_byte), _p(se, C.c_int), _p(sh, C.c_int),
-                                      _p(plan, C.c_byte), mpl, _dp(out["par"]), _dp(out["cov"]), _dp(out["chi2"]),
-                                      _dp(out["score"]), _p(out["nhits"], C.c_int), _p(out["nmiss"], C.c_int),
-                                      _p(out["hit_ids"], C.c_int), _p(out["status"], C.c_uint), _dp(out["margin"]),
-                                      C.byref(nev))
+        args = [C.byref(self.g), C.byref(self.p), C.byref(hs), _p(bo, C.c_uint), _p(si, C.c_int),
+                _p(vm, C.c_float), int(bool(brute_force)), n, _p(par, C.c_float),
+                _p(cov, C.c_float), _p(q, C.c_byte), _p(se, C.c_int), _p(sh, C.c_int),
+                _p(plan, C.c_byte), mpl, _dp(out["par"]), _dp(out["cov"]), _dp(out["chi2"]),
+                _dp(out["score"]), _p(out["nhits"], C.c_int), _p(out["nmiss"], C.c_int),
+                _p(out["hit_ids"], C.c_int), _p(out["status"], C.c_uint), _dp(out["margin"]), C.byref(nev)]
+        if module is not None:
+            mod = _i32(module)
+            assert mod.shape[0] == hs.n_hits
+            out["hit_ids2"] = np.zeros((mpl, n), np.int32)
+            rc = self.L.mkfo_build_tracks_overlap(*args, _p(mod, C.c_int), _p(out["hit_ids2"], C.c_int))
+        else:
+            rc = self.L.mkfo_build_tracks(*args)
         assert rc == 0
         out["n_chi2_evals"] = nev.value
         return out

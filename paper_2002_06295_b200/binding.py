@@ -15,11 +15,11 @@ from . import build as _build
 OK, INVALID_ARG, CUDA_ERROR, WORKSPACE_TOO_SMALL, UNSUPPORTED = 0, -1, -2, -3, -4
 PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8, 16, 32
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
-CALL_FIT_SMOOTH = 5
+CALL_FIT_SMOOTH, CALL_BUILD_TRACKS_OVERLAP = 5, 6
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
            "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_fit_backward_host", "mkf_build_host",
-           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters", "mkf_fit_smooth"]
+           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters", "mkf_fit_smooth", "mkf_build_tracks_overlap"]
 
 
 class Layer(C.Structure):
@@ -41,7 +41,7 @@ class Params(C.Structure):
 
 class Hits(C.Structure):
     _fields_ = [("n_events", C.c_int), ("n_hits", C.c_int), ("layer_off", C.c_void_p), ("x", C.c_void_p),
-                ("y", C.c_void_p), ("z", C.c_void_p), ("V", C.c_void_p), ("rec", C.c_void_p)]
+                ("y", C.c_void_p), ("z", C.c_void_p), ("V", C.c_void_p), ("rec", C.c_void_p), ("module", C.c_void_p)]
 
 
 class HitIndex(C.Structure):
@@ -100,6 +100,8 @@ def lib():
         L.mkf_set_build_counters.argtypes = [vp, vp]
         L.mkf_build_tracks.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
                                        C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.mkf_build_tracks_overlap.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), C.POINTER(States), vp, vp, vp, i,
+                                               C.POINTER(States), vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.mkf_remove_duplicates.argtypes = [vp, i, i, i, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
         ll = C.POINTER(C.c_longlong)
         L.mkf_cluster_strips.argtypes = [vp, C.POINTER(Strips), C.POINTER(StripParams), C.POINTER(Clusters), vp, sz, vp]
@@ -186,9 +188,10 @@ class Context:
     # ---- marshalling helpers ------------------------------------------------------------------------------
     @staticmethod
     def hits_struct(h, ptr, i32=torch.int32, f32=torch.float32):
-        rec = h.get("rec")
+        rec, mod = h.get("rec"), h.get("module") if ptr is _dev else None
         return Hits(int(h["n_events"]), int(h["x"].shape[0]), ptr(h["layer_off"], i32), ptr(h["x"], f32), ptr(h["y"], f32),
-                    ptr(h["z"], f32), ptr(h["V"], f32), ptr(rec, f32) if rec is not None else None)
+                    ptr(h["z"], f32), ptr(h["V"], f32), ptr(rec, f32) if rec is not None else None,
+                    ptr(mod, i32) if mod is not None else None)
 
     def pack_hits(self, hits, rec):
         """mkf_pack_hits: rec float32 CUDA tensor [n_hits * 12] receives the 48-byte hit records (mkf_hits.rec)."""
@@ -255,24 +258,33 @@ class Context:
                                    ws.data_ptr(), ws.numel(), _stream())
         self._check(rc, "mkf_fit_smooth")
 
-    def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status, ws=None):
+    def build_tracks(self, hits, idx, seeds, seed_event, seed_hits, plan, out, chi2, score, nhits, nmiss, hit_ids, status, ws=None, hit_ids2=None):
+        """hit_ids2 (int32 [mpl, n]) given: mkf_build_tracks_overlap (reading R15; hits must hold `module`)."""
         hs = self.hits_struct(hits, _dev)
         packed = idx.get("packed")
         ix = HitIndex(_dev(idx["bin_off"], torch.int32), _dev(idx["sorted_id"], torch.int32), _dev(idx["vmax"], torch.float32),
                       _dev(packed, torch.float32) if packed is not None else None)
         n = int(seeds["par"].shape[1])
         if ws is None:                                          # scratch for the call (kept for the next one of the same size)
-            need = max(self.workspace_bytes(CALL_BUILD_TRACKS, int(hits["n_events"]), int(hits["x"].shape[0]), n), 256)
+            need = max(self.workspace_bytes(CALL_BUILD_TRACKS_OVERLAP if hit_ids2 is not None else CALL_BUILD_TRACKS,
+                                            int(hits["n_events"]), int(hits["x"].shape[0]), n), 256)
             if getattr(self, "_build_ws", None) is None or self._build_ws.numel() < need:
                 self._build_ws = torch.empty(need, dtype=torch.uint8, device=seeds["par"].device)
             ws = self._build_ws
         s = States(n, _dev(seeds["par"], torch.float32), _dev(seeds["cov"], torch.float32), _dev(seeds["q"], torch.int8))
         o = States(n, _dev(out["par"], torch.float32), _dev(out["cov"], torch.float32), _dev(seeds["q"], torch.int8))
-        rc = self.L.mkf_build_tracks(self.h, C.byref(hs), C.byref(ix), C.byref(s), _dev(seed_event, torch.int32),
-                                     _dev(seed_hits, torch.int32), _dev(plan, torch.int8), int(hit_ids.shape[0]), C.byref(o),
-                                     _dev(chi2, torch.float32), _dev(score, torch.float32), _dev(nhits, torch.int32),
-                                     _dev(nmiss, torch.int32), _dev(hit_ids, torch.int32), _dev(status, torch.int32),
-                                     ws.data_ptr() if ws is not None else None, ws.numel() if ws is not None else 0, _stream())
+        if hit_ids2 is not None:
+            rc = self.L.mkf_build_tracks_overlap(self.h, C.byref(hs), C.byref(ix), C.byref(s), _dev(seed_event, torch.int32),
+                                                 _dev(seed_hits, torch.int32), _dev(plan, torch.int8), int(hit_ids.shape[0]), C.byref(o),
+                                                 _dev(chi2, torch.float32), _dev(score, torch.float32), _dev(nhits, torch.int32),
+                                                 _dev(nmiss, torch.int32), _dev(hit_ids, torch.int32), _dev(hit_ids2, torch.int32),
+                                                 _dev(status, torch.int32), ws.data_ptr(), ws.numel(), _stream())
+        else:
+            rc = self.L.mkf_build_tracks(self.h, C.byref(hs), C.byref(ix), C.byref(s), _dev(seed_event, torch.int32),
+                                         _dev(seed_hits, torch.int32), _dev(plan, torch.int8), int(hit_ids.shape[0]), C.byref(o),
+                                         _dev(chi2, torch.float32), _dev(score, torch.float32), _dev(nhits, torch.int32),
+                                         _dev(nmiss, torch.int32), _dev(hit_ids, torch.int32), _dev(status, torch.int32),
+                                         ws.data_ptr() if ws is not None else None, ws.numel() if ws is not None else 0, _stream())
         self._check(rc, "mkf_build_tracks")
 
     def remove_duplicates(self, n_hits, track_off, hit_ids, nhits, score, keep, n_kept, ws):
@@ -380,8 +392,8 @@ def to_device(d, keys, device="cuda"):
     return {k: torch.from_numpy(np.ascontiguousarray(d[k])).to(device) for k in keys}
 
 
-def hits_to_device(hits, device="cuda"):
-    h = to_device(hits, ["layer_off", "x", "y", "z", "V"], device)
+def hits_to_device(hits, device="cuda", with_module=False):
+    h = to_device(hits, ["layer_off", "x", "y", "z", "V"] + (["module"] if with_module else []), device)
     h["n_events"] = int(hits["n_events"])
     return h
 

@@ -57,6 +57,8 @@ struct BuildArgs {
   float* par_out; float* cov_out; float* chi2; float* score; int* nhits; int* nmiss; int* hit_ids; unsigned* status;
   float* wseed;             // [NW][n]   seed kernel -> build kernel
   unsigned* trellis;        // [n][mpl][G]
+  int* trellis2;            // [n][mpl][G] R15: second hit of a step (-2: none); null without overlap recovery
+  int* hit_ids2;            // [mpl][n] or null
   const int* order;         // [n] seed processed at position k
   unsigned* key; unsigned* bucket; int n_buckets;      // counting sort of the seeds
   unsigned long long* counters;
@@ -74,7 +76,7 @@ struct Smem {
   int wrow[SL], wphi[SL];                                     // window: next row | end row << 8 ; w0 | wn << 8
   unsigned long long lkey[LC][SL];                 // the LC best hits of the candidate on this layer, ascending:
                                                    // chi2 bits << 32 | position t of the hit in the sorted index
-  int sel[SL], sel_t[SL], sel_hit[SL];             // the children picked for the new live set: parent | kind << 3 | dead << 8
+  int sel[SL], sel_t[SL], sel_hit[SL], sel_hit2[SL];  // the children picked for the new live set: parent | kind << 3 | dead << 8
   int plist[SL]; int nP;
   int wsum[BT / 32];
   int n_live[NS], p0[NS], plen[NS], ev[NS], last[NS], seed[NS];
@@ -192,6 +194,7 @@ __global__ void __launch_bounds__(128) bs_seed_kernel(const __grid_constant__ Ge
       hit_to_local(S, H, o);
       if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
       for (int s = last_step + 1; s < step; s++) tr[s * G] = 0u;            // hit code 0 == -2 (not crossed), parent 0
+      if (a.trellis2) for (int s = last_step + 1; s <= step; s++) a.trellis2[((size_t)i * mpl + s) * G] = -2;
       chi2 += c2; nh++; last_step = step;
       tr[step * G] = (unsigned)(hid + 2);
     }
@@ -259,6 +262,45 @@ __device__ __forceinline__ unsigned long long rank_key1(float score, float chi2)
   return ((unsigned long long)(~su) << 32) | __float_as_uint(chi2);
 }
 __device__ __forceinline__ unsigned rank_key2(int parent, int hit) { return ((unsigned)parent << 28) | ((unsigned)hit & 0x0fffffffu); }
+// R15: one more hit of the layer from an overlapping module. S: the child's state, already
+// updated with its first hit (position t1 in the sorted index, module mod1). Candidates: the parent's list of this layer
+// (its max_cand best hits by chi2 against the propagated state) behind the first hit. The best chi2 against S below the cut wins; the update
+// is taken only if it stays finite. Returns the hit id taken (or -2) and adds its chi2. Kept out of line: it is off the
+// path of the plain build.
+__device__ __noinline__ int overlap_hit(const BuildArgs& a, const ParamsDev& p, const Smem& sm, int ps, unsigned t1, int mod1,
+                                        KState& S, float& chi2_add) {
+  float tt, tz, zz;
+  cov_aa(S, tt, tz, zz);
+  float best = p.chi2_cut; int best_id = -2; Hit Hb;
+  bool after = false;                                              // only hits that rank after the first one in the list
+  for (int k = 0; k < p.max_cand; k++) {
+    const unsigned long long key = sm.lkey[k][ps];
+    if (key == KEY_NONE) break;
+    const unsigned t2 = (unsigned)key;
+    if (t2 == t1) { after = true; continue; }
+    if (!after) continue;
+    Hit H2; int id2, mod2;
+    if (a.packed) {
+      const float4 q0 = __ldg(a.packed + t2);
+      const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t2;
+      const float4 b = __ldg(cv), d = __ldg(cv + 1);
+      H2.x = q0.x; H2.y = q0.y; H2.z = q0.z; id2 = __float_as_int(q0.w); mod2 = __float_as_int(d.z);
+      H2.v[0] = b.x; H2.v[1] = b.y; H2.v[2] = b.z; H2.v[3] = b.w; H2.v[4] = d.x; H2.v[5] = d.y;
+    } else { id2 = a.sorted_id[t2]; mod2 = a.hits.module[id2]; load_hit(H2, a.hits, id2); }
+    if (mod2 == mod1) continue;
+    SInv o2; float c2b;
+    if (!chi2_local(S, tt, tz, zz, H2, o2, c2b)) continue;
+    if (c2b < best) { best = c2b; best_id = id2; Hb = H2; }
+  }
+  if (best_id < 0) return -2;
+  KState S2 = S;
+  SInv o; float c2u;
+  hit_to_local(S2, Hb, o);
+  if (!(kalman_update(S2, o, c2u) && state_finite(S2) && fabsf(c2u) <= 3.0e38f)) return -2;
+  S = S2; chi2_add = c2u;
+  return best_id;
+}
+
 #ifndef MKF_BUILD_MIN_BLOCKS
 #define MKF_BUILD_MIN_BLOCKS (64 / MKF_BUILD_NS)
 #endif
@@ -607,7 +649,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       __syncthreads();
     }
     KState S;
-    float c_chi2 = 0.f; int c_cnt = 0, cslot = -1, c_sel = 0, c_hit = 0;
+    float c_chi2 = 0.f; int c_cnt = 0, cslot = -1, c_sel = 0, c_hit = 0, c_hit2 = -2;
     bool nan_child = false;
     if (tid < sm.nP) {
       cslot = sm.plist[tid];
@@ -615,16 +657,16 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       const int kind = (c_sel >> 3) & 3;
       c_hit = kind == 1 ? -1 : -2;
       const int ps = (cslot & ~(G - 1)) + (c_sel & 7);        // parent's slot
-      Hit H;
+      Hit H; int mod1 = 0;
       if (kind == 0) {                                        // the hit's record first: its latency overlaps the state loads
         if (a.packed) {
           const int t = sm.sel_t[cslot];
           const float4 q0 = __ldg(a.packed + t);
           const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
           const float4 b = __ldg(cv), d = __ldg(cv + 1);
-          H.x = q0.x; H.y = q0.y; H.z = q0.z; c_hit = __float_as_int(q0.w);
+          H.x = q0.x; H.y = q0.y; H.z = q0.z; c_hit = __float_as_int(q0.w); mod1 = __float_as_int(d.z);
           H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;
-        } else { c_hit = a.sorted_id[sm.sel_t[cslot]]; load_hit(H, a.hits, c_hit); }
+        } else { c_hit = a.sorted_id[sm.sel_t[cslot]]; load_hit(H, a.hits, c_hit); if (a.hit_ids2) mod1 = a.hits.module[c_hit]; }
       }
       const int pcn = sm.cnt[ps];
       c_chi2 = sm.chi2[ps];
@@ -636,11 +678,17 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         SInv o; float c2;
         hit_to_local(S, H, o);
         if (COUNT) n_upd++;
-        if (kalman_update(S, o, c2) && state_finite(S) && fabsf(c2) <= 3.0e38f) { c_chi2 += c2; c_nh++; c_consec = 0; }
-        else { nan_child = true; sm.sel[cslot] = c_sel | 256; }        // dropped (C9 / R1)
+        if (kalman_update(S, o, c2) && state_finite(S) && fabsf(c2) <= 3.0e38f) {
+          c_chi2 += c2; c_nh++; c_consec = 0;
+          if (a.hit_ids2) {                                   // R15: one more hit from an overlapping module
+            float c2b = 0.f;
+            c_hit2 = overlap_hit(a, p, sm, ps, (unsigned)sm.sel_t[cslot], mod1, S, c2b);
+            if (c_hit2 >= 0) { c_chi2 += c2b; c_nh++; }
+          }
+        } else { nan_child = true; sm.sel[cslot] = c_sel | 256; }      // dropped (C9 / R1)
       }
       c_cnt = c_nh | (c_nm << 8) | (c_consec << 16);
-      sm.sel_hit[cslot] = c_hit;                              // for the trellis entry if the live set is compacted below
+      sm.sel_hit[cslot] = c_hit; sm.sel_hit2[cslot] = c_hit2;  // for the trellis entries if the live set is compacted below
     }
     const bool any_nan = __syncthreads_or(nan_child);         // also: every read of A and B of this step is done
     if (any_nan) {
@@ -676,9 +724,10 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       sm.chi2[cslot] = c_chi2; sm.cnt[cslot] = c_cnt;
       const int si = sm.seed[cslot >> 3];
       a.trellis[((size_t)si * mpl + s) * G + (cslot & (G - 1))] = (unsigned)(c_hit + 2) | ((unsigned)(c_sel & 7) << 28);
+      if (a.trellis2) a.trellis2[((size_t)si * mpl + s) * G + (cslot & (G - 1))] = c_hit2;
     }
     if (seed_act) {
-      if (noop) { if (parent_live) trellis[(size_t)s * G + sub] = (unsigned)sub << 28; }        // hit code 0 == -2 (not crossed)
+      if (noop) { if (parent_live) { trellis[(size_t)s * G + sub] = (unsigned)sub << 28; if (a.trellis2) a.trellis2[((size_t)i * mpl + s) * G + sub] = -2; } }   // hit code 0 == -2 (not crossed)
       else if (sub == 0) sm.n_live[sl] = n_new;
       t_last = s;
     }
@@ -694,10 +743,12 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           KState Sm; ld_state(sm.A, from, Sm);
           const float mchi2 = sm.chi2[from]; const int mcnt = sm.cnt[from];
           const unsigned ent = (unsigned)(sm.sel_hit[from] + 2) | ((unsigned)(sm.sel[from] & 7) << 28);
+          const int ent2 = sm.sel_hit2[from];
           __syncwarp(gm);
           if (sub < cntl) {
             st_state(sm.A, tid, Sm); sm.chi2[tid] = mchi2; sm.cnt[tid] = mcnt;
             trellis[(size_t)s * G + sub] = ent;
+            if (a.trellis2) a.trellis2[((size_t)i * mpl + s) * G + sub] = ent2;
           }
           if (sub == 0) sm.n_live[sl] = cntl;
         }
@@ -753,15 +804,22 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       if (sub == 0) {
         for (int s = min(s0 + G, mpl) - 1; s >= s0; s--) {
           int v = -2;
+          int v2 = -2;
           if (s == tail_step) v = tail_val;
-          else if (s <= bt_step) { const unsigned e = staged ? tsm[s * G + slot] : trellis[(size_t)s * G + slot]; v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28); }
+          else if (s <= bt_step) {
+            const unsigned e = staged ? tsm[s * G + slot] : trellis[(size_t)s * G + slot];
+            if (a.trellis2) v2 = a.trellis2[((size_t)i * mpl + s) * G + slot];
+            v = (int)(e & 0x0fffffffu) - 2; slot = (int)(e >> 28);
+          }
           sm.sel_t[(tid & ~(G - 1)) + (s - s0)] = v;
+          sm.sel_hit2[(tid & ~(G - 1)) + (s - s0)] = v2;
         }
       }
       __syncwarp(gm);
-      if (s0 + sub < mpl) mine = sm.sel_t[(tid & ~(G - 1)) + sub];
+      int mine2 = -2;
+      if (s0 + sub < mpl) { mine = sm.sel_t[(tid & ~(G - 1)) + sub]; mine2 = sm.sel_hit2[(tid & ~(G - 1)) + sub]; }
       __syncwarp(gm);
-      if (s0 + sub < mpl) a.hit_ids[(size_t)(s0 + sub) * n + i] = mine;
+      if (s0 + sub < mpl) { a.hit_ids[(size_t)(s0 + sub) * n + i] = mine; if (a.hit_ids2) a.hit_ids2[(size_t)(s0 + sub) * n + i] = mine2; }
     }
   }
   if (COUNT) {
@@ -787,9 +845,32 @@ size_t build_ws_bytes(const mkf_ctx* c, int n_events, int n_seeds) {
 }
 }  // namespace mkf
 
+static int build_tracks_common(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
+                                const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
+                                mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, int* hit_ids2,
+                                unsigned* status, void* ws, size_t ws_bytes, void* stream);
+
 extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
                                 const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
                                 mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids,
+                                unsigned* status, void* ws, size_t ws_bytes, void* stream) {
+  return build_tracks_common(c, h, idx, seeds, seed_event, seed_hits, plan, max_plan_len, out, chi2, score, nhits, nmiss, hit_ids, nullptr,
+                             status, ws, ws_bytes, stream);
+}
+
+extern "C" int mkf_build_tracks_overlap(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
+                                const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
+                                mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, int* hit_ids2,
+                                unsigned* status, void* ws, size_t ws_bytes, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || !h->module || !hit_ids2) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks_overlap: hits->module and hit_ids2 are needed");
+  return build_tracks_common(c, h, idx, seeds, seed_event, seed_hits, plan, max_plan_len, out, chi2, score, nhits, nmiss, hit_ids, hit_ids2,
+                             status, ws, ws_bytes, stream);
+}
+
+static int build_tracks_common(mkf_ctx* c, const mkf_hits* h, const mkf_hit_index* idx, const mkf_states* seeds,
+                                const int* seed_event, const int* seed_hits, const signed char* plan, int max_plan_len,
+                                mkf_states* out, float* chi2, float* score, int* nhits, int* nmiss, int* hit_ids, int* hit_ids2,
                                 unsigned* status, void* ws, size_t ws_bytes, void* stream) {
   if (!c) return MKF_INVALID_ARG;
   if (!h || !idx || !seeds || !out) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null argument");
@@ -804,7 +885,8 @@ extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_ind
     return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: null array");
   if (h->n_events < 1) return fail(c, MKF_INVALID_ARG, "mkf_build_tracks: no events");
   if (c->g.n_phi > 255 || c->g.n_eta > 255) return fail(c, MKF_UNSUPPORTED, "mkf_build_tracks: more than 255 phi or eta bins");
-  const size_t need = build_ws_bytes(c, h->n_events, seeds->n);
+  const size_t tr2_bytes = hit_ids2 ? align256((size_t)seeds->n * max_plan_len * G * 4) : 0;
+  const size_t need = build_ws_bytes(c, h->n_events, seeds->n) + tr2_bytes;
   if (ws_bytes < need || !ws) return fail(c, MKF_WORKSPACE_TOO_SMALL, "mkf_build_tracks: workspace too small");
   cudaStream_t st = (cudaStream_t)stream;
   const size_t n = (size_t)seeds->n, nbk = n_buckets_of(c, h->n_events);
@@ -823,7 +905,9 @@ extern "C" int mkf_build_tracks(mkf_ctx* c, const mkf_hits* h, const mkf_hit_ind
   a.key = (unsigned*)w; w += align256(n * 4);
   a.bucket = (unsigned*)w; w += align256((nbk + 1) * 4);
   unsigned* bucket_off = (unsigned*)w; w += align256((nbk + 1) * 4);
-  unsigned* partial = (unsigned*)w;
+  unsigned* partial = (unsigned*)w; w += scan_partial_bytes(nbk);
+  a.trellis2 = hit_ids2 ? (int*)w : nullptr;
+  a.hit_ids2 = hit_ids2;
   a.n_buckets = (int)nbk;
   a.counters = c->build_counters;
   cudaError_t e = cudaMemsetAsync(a.bucket, 0, nbk * 4, st);

@@ -45,6 +45,6 @@ inline int cuda_fail(mkf_ctx* c, cudaError_t e, const char* where) {
 inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 inline HitsDev hits_dev(const mkf_hits* h) {
   HitsDev d; d.n_events = h->n_events; d.n_hits = h->n_hits; d.layer_off = h->layer_off;
-  d.x = h->x; d.y = h->y; d.z = h->z; d.V = h->V; d.rec = (const float4*)h->rec; return d;
+  d.x = h->x; d.y = h->y; d.z = h->z; d.V = h->V; d.rec = (const float4*)h->rec; d.module = h->module; return d;
 }
 }  // namespace mkf

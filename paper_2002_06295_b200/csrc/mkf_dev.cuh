@@ -21,7 +21,7 @@ struct ParamsDev {
   float score_hit, score_miss, graze_cos_min; int material_flags; float dup_frac;
 };
 
-struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; const float4* rec; };
+struct HitsDev { int n_events, n_hits; const int* layer_off; const float *x, *y, *z, *V; const float4* rec; const int* module; };
 
 // Parameters of a caller's state; the covariance is read separately by the first propagation (commit_first).
 MKF_HD void load_params(KState& S, const float* par, size_t n, size_t i) {

@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
   a.packed[t] = make_float4(a.hits.x[id], a.hits.y[id], a.hits.z[id], __int_as_float(id));
   float4* o = a.packed + nh + (size_t)2 * t;
   o[0] = make_float4(V[id], V[nh + id], V[2 * nh + id], V[3 * nh + id]);
-  o[1] = make_float4(V[4 * nh + id], V[5 * nh + id], 0.f, 0.f);
+  o[1] = make_float4(V[4 * nh + id], V[5 * nh + id], a.hits.module ? __int_as_float(a.hits.module[id]) : 0.f, 0.f);
 }
 
 
@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
       a.packed[t] = make_float4(x, y, z, __int_as_float(i));
       float4* o = a.packed + nh + (size_t)2 * t;
       o[0] = make_float4(v0, v1, v2, v3);
-      o[1] = make_float4(v4, v5, 0.f, 0.f);
+      o[1] = make_float4(v4, v5, a.hits.module ? __int_as_float(a.hits.module[i]) : 0.f, 0.f);
     }
   };
   for (int i0 = b + tid; i0 < e; i0 += 2 * HF_BLOCK) {

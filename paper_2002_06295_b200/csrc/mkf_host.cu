@@ -27,6 +27,7 @@ extern "C" size_t mkf_workspace_bytes(const mkf_ctx* c, int call_id, int n_event
     case MKF_CALL_CLUSTER_STRIPS: return strips_ws_bytes(n_hits, n_seeds);
     case MKF_CALL_BUILD_TRACKS: return build_ws_bytes(c, n_events, n_seeds);
     case MKF_CALL_FIT_SMOOTH: return smooth_ws_bytes(n_seeds, c->max_plan_len);
+    case MKF_CALL_BUILD_TRACKS_OVERLAP: return build_ws_bytes(c, n_events, n_seeds) + align256((size_t)n_seeds * c->max_plan_len * 8 * 4);
     default: return 0;      // the fit keeps everything in registers
   }
 }
@@ -119,7 +120,7 @@ mkf_hits upload_hits(Arena& A, const mkf_ctx* c, const mkf_hits* h, cudaStream_t
   const size_t nh = (size_t)h->n_hits;
   d.layer_off = A.up(h->layer_off, (size_t)h->n_events * (c->g.n_layers + 1), st);
   d.x = A.up(h->x, nh, st); d.y = A.up(h->y, nh, st); d.z = A.up(h->z, nh, st); d.V = A.up(h->V, 6 * nh, st);
-  d.rec = nullptr;
+  d.rec = nullptr; d.module = nullptr;
   return d;
 }
 

@@ -151,7 +151,7 @@ def _step(a, st, s):
     return [x + s * sc * np.cos(phi + h), y + s * sc * np.sin(phi + h), z + s / np.tan(th), ipt, phi + w * s, th]
 
 
-def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30, straggle=False, scatter=True, keep_truth=False):
+def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_graze=0.30, straggle=False, scatter=True, keep_truth=False, keep_cross=False):
     """Step every particle through its plan. Returns per plan step, per particle: hit position (3), the layer,
     and a validity mask; also the truth state after the last crossed layer (after its material).
     st0 = [x,y,z,ipt,phi,theta] arrays (float64)."""
@@ -166,6 +166,7 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
     hx = np.zeros((mpl, n)); hy = np.zeros((mpl, n)); hz = np.zeros((mpl, n))
     hl = np.full((mpl, n), -1, np.int32)
     tstates = np.full((mpl, 6, n), np.nan) if keep_truth else None    # truth after each crossed layer (after its material)
+    xing = np.zeros((3, mpl, n)) if keep_cross else None              # true crossing points (for a second, overlapping-module hit)
     for step in range(mpl):
         # fixed draw order per step: smear1, smear2, efficiency, scatter alpha, scatter beta
         g1, g2 = rng.standard_normal(n), rng.standard_normal(n)
@@ -217,6 +218,8 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
                 rr = rr + g2[jj] * lay["sig_l"]
                 px, py, pz = rr * np.cos(ph), rr * np.sin(ph), np.full(jj.size, lay["pos"])
             hx[step, jj] = px; hy[step, jj] = py; hz[step, jj] = pz
+            if keep_cross:
+                xing[0, step, jj] = nx[0]; xing[1, step, jj] = nx[1]; xing[2, step, jj] = nx[2]
             hl[step, jj] = np.where(made, li, -1)
             # material on the truth
             if material and lay["xx0"] > 0:
@@ -241,8 +244,8 @@ def simulate(geom, rng, ev_of, plan_of, q, st0, eff=1.0, material=True, truth_gr
                 st[k][jj] = nx[k]
                 if keep_truth:
                     tstates[step, k, jj] = nx[k]
-    if keep_truth:
-        return hx, hy, hz, hl, np.stack(st), tstates
+    if keep_truth or keep_cross:
+        return hx, hy, hz, hl, np.stack(st), tstates, xing
     return hx, hy, hz, hl, np.stack(st)
 
 
@@ -300,7 +303,8 @@ def three_point_seed(bz, h1, h2, h3, V1, inflate=100.0):
 # ------------------------------------------------------------------------------------------------------
 def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spectrum="loguniform",
                 pt_range=(0.5, 10.0), n_hard=0, eta_max=1.0, eff=1.0, material=True, shuffle=True,
-                seed_on_pixel=False, inflate=100.0, straggle=False, scatter=True, keep_truth=False):
+                seed_on_pixel=False, inflate=100.0, straggle=False, scatter=True, keep_truth=False, overlap_frac=0.0,
+                n_modules_phi=64):
     """Returns dict(hits=..., truth_hits [mpl][n_part], seeds=..., ...). Particles 0..n_primary-1 of each event are
     'primary' (seed candidates), the rest 'secondary' (hits only). Draw order: per particle (pT, eta, phi, q, vx,
     vy, vz) as whole arrays, then `simulate`'s per-step draws, then noise (phi, l) per layer, then the shuffle."""
@@ -324,7 +328,8 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
     theta = 2 * np.arctan(np.exp(-eta))
     plan_of = np.zeros(n, np.int8) if len(geom["plan_off"]) == 2 else np.where(eta >= 0, 0, 1).astype(np.int8)
     sim = simulate(geom, rng, ev_of, plan_of, q.astype(float), [vx, vy, vz, 1.0 / pt, phi, theta],
-                   eff=eff, material=material, straggle=straggle, scatter=scatter, keep_truth=keep_truth)
+                   eff=eff, material=material, straggle=straggle, scatter=scatter, keep_truth=keep_truth,
+                   keep_cross=overlap_frac > 0)
     hx, hy, hz, hl, final_state = sim[:5]
     mpl = hx.shape[0]
     nl = len(geom["layers"])
@@ -332,6 +337,31 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
     st_idx, p_idx = np.nonzero(hl >= 0)
     X = [hx[st_idx, p_idx]]; Y = [hy[st_idx, p_idx]]; Z = [hz[st_idx, p_idx]]
     LAY = [hl[st_idx, p_idx]]; EV = [ev_of[p_idx]]; PART = [p_idx.astype(np.int64)]; STEP = [st_idx.astype(np.int32)]
+    # overlap hits: a fraction of the crossings is seen by a second, overlapping module of the same layer: an
+    # independent measurement of the same true crossing point (drawn last but for the noise and the shuffle)
+    SECOND = []
+    if overlap_frac > 0:
+        cross = sim[6]
+        pick = rng.random(len(st_idx)) < overlap_frac
+        g1, g2 = rng.standard_normal(len(st_idx)), rng.standard_normal(len(st_idx))
+        for li, lay in enumerate(geom["layers"]):
+            m = pick & (LAY[0] == li)
+            if not m.any():
+                continue
+            cx_, cy_, cz_ = cross[0, st_idx[m], p_idx[m]], cross[1, st_idx[m], p_idx[m]], cross[2, st_idx[m], p_idx[m]]
+            if lay["kind"] == 0:
+                R = lay["pos"]
+                ph = np.arctan2(cy_, cx_) + g1[m] * lay["sig_t"] / R
+                X.append(R * np.cos(ph)); Y.append(R * np.sin(ph)); Z.append(cz_ + g2[m] * lay["sig_l"])
+            else:
+                rr = np.hypot(cx_, cy_)
+                ph = np.arctan2(cy_, cx_) + g1[m] * lay["sig_t"] / rr
+                rr = rr + g2[m] * lay["sig_l"]
+                X.append(rr * np.cos(ph)); Y.append(rr * np.sin(ph)); Z.append(np.full(m.sum(), lay["pos"]))
+            LAY.append(np.full(m.sum(), li, np.int32)); EV.append(ev_of[p_idx[m]]); PART.append(p_idx[m].astype(np.int64))
+            STEP.append(np.full(m.sum(), -1, np.int32))                      # not a first hit: never a seed or truth_hits entry
+            SECOND.append((st_idx[m], p_idx[m]))
+    n_first = len(st_idx)
     # noise hits: n_noise per event spread evenly over layers
     if n_noise > 0:
         per_layer = n_noise // nl
@@ -348,12 +378,21 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
     X, Y, Z = np.concatenate(X), np.concatenate(Y), np.concatenate(Z)
     LAY, EV, PART, STEP = np.concatenate(LAY), np.concatenate(EV), np.concatenate(PART), np.concatenate(STEP)
     nh = len(X)
+    # module ids: n_modules_phi modules around every layer; the second hit of a crossing sits in the neighbouring module
+    MOD = (np.floor((np.arctan2(Y, X) + np.pi) * n_modules_phi / (2 * np.pi)).astype(np.int64) % n_modules_phi)
+    if SECOND:
+        n_second = sum(len(a_) for a_, _ in SECOND)
+        first_of = np.full((mpl, n), -1, np.int64)
+        first_of[st_idx, p_idx] = np.arange(n_first)
+        src = np.concatenate([first_of[a_, b_] for a_, b_ in SECOND])
+        MOD[n_first:n_first + n_second] = (MOD[src] + 1) % n_modules_phi
+    MOD = (LAY.astype(np.int64) * n_modules_phi + MOD).astype(np.int32)
     key = EV.astype(np.int64) * nl + LAY
     if shuffle:
         order = np.lexsort((rng.random(nh), key))
     else:
         order = np.argsort(key, kind="stable")
-    X, Y, Z, LAY, EV, PART, STEP, key = X[order], Y[order], Z[order], LAY[order], EV[order], PART[order], STEP[order], key[order]
+    X, Y, Z, LAY, EV, PART, STEP, key, MOD = X[order], Y[order], Z[order], LAY[order], EV[order], PART[order], STEP[order], key[order], MOD[order]
     counts = np.bincount(key, minlength=n_events * nl).reshape(n_events, nl)
     layer_off = np.zeros((n_events, nl + 1), np.int64)
     ev_start = np.concatenate([[0], np.cumsum(counts.sum(1))])
@@ -365,10 +404,10 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
         if m.any():
             V[:, m] = hit_cov(lay, X[m], Y[m])
     truth_hits = np.full((mpl, n), -1, np.int32)
-    sig = PART >= 0
+    sig = (PART >= 0) & (STEP >= 0)
     truth_hits[STEP[sig], PART[sig]] = np.nonzero(sig)[0].astype(np.int32)
     hits = dict(n_events=n_events, layer_off=layer_off.astype(np.int32).reshape(-1), x=X.astype(np.float32),
-                y=Y.astype(np.float32), z=Z.astype(np.float32), V=V.astype(np.float32))
+                y=Y.astype(np.float32), z=Z.astype(np.float32), V=V.astype(np.float32), module=MOD)
     # seeds: first three hits in plan order (optionally restricted to pixel layers)
     if seed_on_pixel:
         is_pix = np.zeros(nl, bool); is_pix[geom["pixel_layers"]] = True
