@@ -101,7 +101,10 @@ struct FitArgs {
 // The track keeps its last good state when a step fails. Failures found before the covariance is touched
 // (unreachable, grazing, energy exhausted) leave the state as it was; the two that can only be seen after the
 // update (S not positive definite, non-finite result) re-run the track from its seed up to the failing step.
+// STRAG: the context asks for energy-loss straggling (material flag 4, R12); without it that code is not compiled in.
+template <bool STRAG>
 MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
+  const int mflags = STRAG ? p.material_flags : (p.material_flags & 3);
   const size_t n = (size_t)a.ld;
   const int pl = a.plan[i];
   if ((unsigned)pl >= (unsigned)g.n_plans) {                     // not a plan of this geometry: the seed goes out, flagged
@@ -143,9 +146,9 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
       if (hid < 0 || stopped) continue;
       if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; continue; }    // not a hit of this call
       const int li = g.plan_layers[p0 + s];
-      const LayerDev& L = g.layers[li];
+      const LayerDev L = g.layers[li];
       Hit H; load_hit(H, a.hits, hid);
-      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
+      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, mflags, false);
       if (rc) { stat |= rc; stopped = true; continue; }
       SInv o; float c2;
       hit_to_local(S, H, o);
@@ -169,7 +172,9 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
 // material of the layer being left, propagate backward (s <= 0), transport, update. After the innermost hit that
 // layer's material is given back too (done on the covariance at the output boundary), so the result is the state
 // before it. A failing step stops the track, which keeps the state after its last good update.
+template <bool STRAG>
 MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
+  const int mflags = STRAG ? p.material_flags : (p.material_flags & 3);
   const size_t n = (size_t)a.ld;
   const int pl = a.plan[i];
   if ((unsigned)pl >= (unsigned)g.n_plans) {
@@ -205,13 +210,13 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
         if (nf > 0) {                                            // give back the material of the layer being left
           const LayerDev& Lp = g.layers[prev];
           float rp;
-          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
+          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, mflags, rp, J, th02, q4);
           S.ipt = ipt_old * rp;                                  // the geometry uses the momentum after the give-back
         }
         const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[nf > 0 ? prev : li], p.graze_cos_min, 0, false, P);     // R13: back along the arc of the layer being left
         if (rc) { S.ipt = ipt_old; stat |= rc; stopped = true; break; }
         if (nf == 0) { float c[21]; load_cov(c, a.cov, n, (size_t)i); commit_first(S, c, P, 0); }
-        else commit_step_backward(S, P, J, th02, q4, p.material_flags);
+        else commit_step_backward(S, P, J, th02, q4, mflags);
         SInv o; float c2;
         hit_to_local(S, H, o);
         if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break; }
@@ -229,12 +234,12 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     if (stat == 0) {                                             // give back the innermost layer's material
       const LayerDev& Lp = g.layers[prev];
       float rp, J, th02, q4;
-      material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
+      material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, mflags, rp, J, th02, q4);
       S.ipt *= rp;
 #pragma unroll
       for (int k = 0; k < 5; k++) l[LI(1, k)] *= (k == 1 ? J * J : J);
       l[LI(1, 1)] += q4;
-      if (p.material_flags & 1) {
+      if (mflags & 1) {
         const float g3 = -S.ipt * fast_div(S.cth, S.sth), g2 = fast_rcp(S.sth);
         l[LI(1, 1)] += g3 * g3 * th02; l[LI(2, 1)] += g3 * th02; l[LI(2, 2)] += th02; l[LI(0, 0)] += g2 * g2 * th02;
       }
