@@ -37,6 +37,7 @@ constexpr int LC = 8;                // accepted hits kept per candidate and lay
 constexpr int ROWCAP = 24 * NS;        // row parts (contiguous runs of hits) in the CTA's table per scan round
 constexpr int SQCAP = 48 * NS;        // survivors of the position test queued per scan pass (= hits looked at per pass)
 constexpr int RUN_MAX = (1 << 22) - 1; // longest run of hits in one table entry (queue entries hold run << 22 | offset)
+constexpr int NWARP = BT / 32, WQ = SQCAP / NWARP;   // survivor queue of one warp
 constexpr int HIT_NONE = 0x7fffffff; // "hit id" of miss / pass-through children in the order U14
 static_assert(G == MAX_CAND, "one slot per candidate");
 static_assert(BT % 32 == 0 && BT <= 1024, "CTA size");
@@ -72,7 +73,7 @@ struct Smem {
   int flag[SL]; unsigned ostat[SL];
   uint2 rows[ROWCAP]; int n_rows, more;                       // runs of hits to scan: (slot | n << 8, first position); more: a window has rows left
   int runpre[ROWCAP + 1];                                     // exclusive prefix of the runs' lengths: the hits of a round as one list
-  unsigned sq[SQCAP]; int sq_n;                               // survivors of the position test: run << 22 | offset in the run
+  unsigned sq[SQCAP + BT]; int next;                            // survivors of the position test: run << 22 | offset in the run
   int wrow[SL], wphi[SL];                                     // window: next row | end row << 8 ; w0 | wn << 8
   unsigned long long lkey[LC][SL];                 // the LC best hits of the candidate on this layer, ascending:
                                                    // chi2 bits << 32 | position t of the hit in the sorted index
@@ -474,82 +475,123 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         int run = base + inc - sum;
 #pragma unroll
         for (int k = 0; k < PER; k++) { const int j = tid * PER + k; if (j <= NR) sm.runpre[j] = run; run += loc[k]; }
-        if (tid == 0) { sm.runpre[NR] = tot; sm.sq_n = 0; }
+        if (tid == 0) { sm.runpre[NR] = tot; sm.next = NWARP * WQ; }
         __syncthreads();
       }
       const int H = sm.runpre[NR];
-      for (int h0 = 0; h0 < H; h0 += SQCAP) {
-        // ---- pass A: hits [h0, h1), a contiguous share per thread (its next position is fetched ahead) ------------------
-        const int h1 = min(h0 + SQCAP, H);
-        const int share = (h1 - h0 + BT - 1) / BT;
-        int q = h0 + tid * share;
-        const int qe = min(q + share, h1);
+      // the warps take parts of WQ hits from the list as they get free and work through them on their own: no CTA barrier
+      // and no shared counter between the two passes
+      unsigned* wq = sm.sq + warp * (WQ + 32);
+      int nq = 0;                                             // queued survivors (uniform in the warp); a rest < 32 waits for the next part
+      const unsigned lt = (1u << lane) - 1u;
+      // a list of up to NWARP x WQ hits is dealt out in equal parts; of a longer one every warp gets a first part of WQ hits
+      // and takes further ones from a counter as it gets free
+      const int part = min(WQ, (H + NWARP - 1) / NWARP);
+      const bool steal = H > NWARP * WQ;                      // sm.next starts at NWARP x WQ
+      bool first = true;
+      for (bool last = false; !last;) {
+        int c0 = warp * part;
+        if (!first) {
+          if (steal) { if (lane == 0) c0 = atomicAdd(&sm.next, WQ); c0 = __shfl_sync(0xffffffffu, c0, 0); }
+          else c0 = H;
+        }
+        first = false;
+        last = c0 >= H;
+        // ---- pass A: hits [c0, c1), a contiguous share per lane (its next position is fetched ahead); the loop is uniform
+        // in the warp, survivors are queued by ballot -----------------------------------------------------------------
+        const int c1 = min(c0 + part, H);
+        const int share = last ? 0 : (c1 - c0 + 31) >> 5;
+        int q = c0 + lane * share;
+        const int qe = min(q + share, c1);
+        int j = 0, rb = 0, re = 0, slot = 0, kind = 0;
+        float cx = 0.f, cy = 0.f, cz = 0.f, cxl = 0.f, cyl = 0.f, czl = 0.f, cb = 0.f, sb = 0.f, l1 = 0.f, l2 = 0.f;
+        const unsigned* worst = nullptr; const float4* pp = nullptr; float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
         if (q < qe) {
           int lo = 0, hi = NR;                                // run of hit q: last j with runpre[j] <= q
           while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sm.runpre[mid] <= q) lo = mid; else hi = mid; }
-          int j = lo;
-          while (q < qe) {
-            const uint2 r = sm.rows[j];
-            const int slot = (int)(r.x & 0xffu);
-            const int rb = sm.runpre[j], re = rb + (int)(r.x >> 8);
-            const int qs = min(qe, re);
-            if (a.packed) {
-              const float cx = sm.B[F_X][slot], cy = sm.B[F_Y][slot], cz = sm.B[F_Z][slot];
-              const float cxl = sm.B[F_XL][slot], cyl = sm.B[F_YL][slot], czl = sm.B[F_ZL][slot];
-              const int kind = __float_as_int(sm.B[F_FK][slot]); const float cb = sm.B[F_FCB][slot], sb = sm.B[F_FSB][slot];
-              const float l1 = sm.lim1[slot], l2 = sm.lim2[slot];
-              const unsigned* worst = reinterpret_cast<const unsigned*>(&sm.lkey[p.max_cand - 1][slot]) + 1;    // chi2 bits of the list's last hit
-              const float4* pp = a.packed + r.y + (q - rb);
-              float4 qn = __ldg(pp);
-              for (; q < qs; q++) {
-                // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11); once
-                // the candidate's list is full only a hit better than its last one can matter, so the cut follows it
-                const float4 q0 = qn;
-                pp++;
-                if (q + 1 < qs) qn = __ldg(pp);
-                if (COUNT) n_pos++;
-                const float cut = fminf(p.chi2_cut, __uint_as_float(min(*(volatile const unsigned*)worst, 0x7f800000u)));
-                const float rx = (q0.x - cx) - cxl, ry = (q0.y - cy) - cyl, rz = (q0.z - cz) - czl;
-                const float r1 = kind == 0 ? cb * ry - sb * rx : rx, r2 = kind == 0 ? rz : ry;
-                if (!(r1 * r1 > cut * l1 || r2 * r2 > cut * l2)) sm.sq[atomicAdd(&sm.sq_n, 1)] = ((unsigned)j << 22) | (unsigned)(q - rb);
-              }
-            } else {
-              if (COUNT) n_pos += qs - q;
-              for (; q < qs; q++) sm.sq[atomicAdd(&sm.sq_n, 1)] = ((unsigned)j << 22) | (unsigned)(q - rb);
-            }
-            j++;
-          }
+          j = lo - 1; re = q;                                 // the first iteration opens run lo
         }
-        __syncthreads();
-        // ---- pass B: one thread per survivor ---------------------------------------------------------------------------
-        const int nq = sm.sq_n;
-        for (int k = tid; k < nq; k += BT) {
-          const unsigned e = sm.sq[k];
+        for (int it = 0; it < share; it++) {
+          bool surv = false; unsigned ent = 0;
+          if (q < qe) {
+            if (q >= re) {                                    // next run (runs of length 0 are skipped)
+              do { j++; rb = sm.runpre[j]; re = sm.runpre[j + 1]; } while (q >= re);
+              const uint2 r = sm.rows[j];
+              slot = (int)(r.x & 0xffu);
+              if (a.packed) {
+                cx = sm.B[F_X][slot]; cy = sm.B[F_Y][slot]; cz = sm.B[F_Z][slot];
+                cxl = sm.B[F_XL][slot]; cyl = sm.B[F_YL][slot]; czl = sm.B[F_ZL][slot];
+                kind = __float_as_int(sm.B[F_FK][slot]); cb = sm.B[F_FCB][slot]; sb = sm.B[F_FSB][slot];
+                l1 = sm.lim1[slot]; l2 = sm.lim2[slot];
+                worst = reinterpret_cast<const unsigned*>(&sm.lkey[p.max_cand - 1][slot]) + 1;    // chi2 bits of the list's last hit
+                pp = a.packed + r.y + (q - rb);
+                qn = __ldg(pp);
+              }
+            }
+            ent = ((unsigned)j << 22) | (unsigned)(q - rb);
+            if (COUNT) n_pos++;
+            if (a.packed) {
+              // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11); once
+              // the candidate's list is full only a hit better than its last one can matter, so the cut follows it
+              const float4 q0 = qn;
+              pp++;
+              if (q + 1 < min(qe, re)) qn = __ldg(pp);
+              const float cut = fminf(p.chi2_cut, __uint_as_float(min(*(volatile const unsigned*)worst, 0x7f800000u)));
+              const float rx = (q0.x - cx) - cxl, ry = (q0.y - cy) - cyl, rz = (q0.z - cz) - czl;
+              const float r1 = kind == 0 ? cb * ry - sb * rx : rx, r2 = kind == 0 ? rz : ry;
+              surv = !(r1 * r1 > cut * l1 || r2 * r2 > cut * l2);
+            } else surv = true;
+            q++;
+          }
+          const unsigned bal = __ballot_sync(0xffffffffu, surv);
+          if (surv) wq[nq + __popc(bal & lt)] = ent;
+          nq += __popc(bal);
+        }
+        __syncwarp();
+        // ---- pass B: one lane per survivor, full warps only while more hits follow ----------------------------------------
+        const int nproc = last ? nq : (nq & ~31);
+        float4 nq0 = make_float4(0.f, 0.f, 0.f, 0.f), nb4 = nq0, nd4 = nq0; int nslot = 0; unsigned nt = 0;
+        auto fetch = [&](int k) {                             // the survivor's hit, one queue entry ahead of its use
+          const unsigned e = wq[k];
           const uint2 r = sm.rows[e >> 22];
-          const int slot = (int)(r.x & 0xffu);
-          const unsigned t = r.y + (e & 0x3fffffu);
+          nslot = (int)(r.x & 0xffu);
+          nt = r.y + (e & 0x3fffffu);
+          if (a.packed) {
+            nq0 = __ldg(a.packed + nt);
+            const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * nt;
+            nb4 = __ldg(cv); nd4 = __ldg(cv + 1);
+          }
+        };
+        if (lane < nproc) fetch(lane);
+        for (int k = lane; k < nproc; k += 32) {
+          const int slot2 = nslot; const unsigned t = nt;
           Hit H2;
           if (a.packed) {
-            const float4 q0 = __ldg(a.packed + t);
-            const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
-            const float4 b4 = __ldg(cv), d4 = __ldg(cv + 1);
-            H2.x = q0.x; H2.y = q0.y; H2.z = q0.z;
-            H2.v[0] = b4.x; H2.v[1] = b4.y; H2.v[2] = b4.z; H2.v[3] = b4.w; H2.v[4] = d4.x; H2.v[5] = d4.y;
+            H2.x = nq0.x; H2.y = nq0.y; H2.z = nq0.z;
+            H2.v[0] = nb4.x; H2.v[1] = nb4.y; H2.v[2] = nb4.z; H2.v[3] = nb4.w; H2.v[4] = nd4.x; H2.v[5] = nd4.y;
           } else load_hit(H2, a.hits, a.sorted_id[t]);
-          ScanCand c; load_scan_cand(sm, slot, c);
+          if (k + 32 < nproc) fetch(k + 32);
+          ScanCand c; load_scan_cand(sm, slot2, c);
           KState Sc;                                          // only what hit_to_local / chi2_local read
           Sc.x = c.x; Sc.y = c.y; Sc.z = c.z; Sc.xl = c.xl; Sc.yl = c.yl; Sc.zl = c.zl; Sc.f.kind = c.kind; Sc.f.cb = c.cb; Sc.f.sb = c.sb;
           if (COUNT) n_c2++;
           SInv o; float c2;
           if (chi2_local(Sc, c.tt, c.tz, c.zz, H2, o, c2) && c2 < p.chi2_cut) {
             if (COUNT) n_acc++;
-            accept_hit(sm, slot, p.max_cand, c2, t);
+            accept_hit(sm, slot2, p.max_cand, c2, t);
           }
         }
-        __syncthreads();
-        if (tid == 0) sm.sq_n = 0;
-        if (h0 + SQCAP < H) __syncthreads();
+        __syncwarp();
+        if (!last) {
+          const int rem = nq - nproc;
+          const unsigned e = lane < rem ? wq[nproc + lane] : 0u;
+          __syncwarp();
+          if (lane < rem) wq[lane] = e;
+          nq = rem;
+          __syncwarp();
+        }
       }
+      __syncthreads();
       if (!more) break;
       __syncthreads();
       if (tid == 0) { sm.n_rows = 0; sm.more = 0; }
