@@ -52,12 +52,13 @@ def peaks():
     return p
 
 
-def ncu_traffic(kernel):
-    """dram__bytes_read + dram__bytes_write of one launch of `kernel` on its full-size workload, from the last
-    `ncu --set full` capture: profiles/traffic.json records the value and the commit it was captured at."""
+def ncu_traffic(kernel, units):
+    """dram__bytes_read + dram__bytes_write of one launch of `kernel` from the last `ncu --set full` capture, scaled
+    from the units (layer-steps, events) of the captured launch to those of this run's launch (the kernels stream:
+    traffic is linear in the units). profiles/traffic.json holds the captured bytes, units, commit and workload."""
     try:
         t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[kernel]
-        return float(t["bytes"]), t.get("commit"), t.get("workload")
+        return float(t["bytes"]) * float(units) / float(t["units"]), t.get("commit"), t.get("workload")
     except Exception:
         return None, None, None
 
@@ -370,9 +371,9 @@ def run_fit(R, w, seed, workload=None):
     kernel = "mkf_fit_backward_kernel" if backward else "mkf_fit_kernel"
     bps = ALGO_BYTES_PER_LAYER_STEP_REC if shuffled else ALGO_BYTES_PER_LAYER_STEP
     ach = ALGO_FLOP_PER_LAYER_STEP * u / t_launch / 1e12
-    traffic, tcommit, twl = ncu_traffic(kernel + ("/records" if shuffled else ""))
+    traffic, tcommit, twl = ncu_traffic(kernel + ("/records" if shuffled else ""), u)
     rec["roofline"] = dict(bound="alu", kernel=kernel, achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
-                           traffic=traffic if a.scale == 1.0 else None, traffic_commit=tcommit, algorithmic_bytes=bps * u,
+                           traffic=traffic, traffic_commit=tcommit, algorithmic_bytes=bps * u,
                            peak_source=pk["fp32_source"], algorithmic_flop_per_layer_step=ALGO_FLOP_PER_LAYER_STEP,
                            note="algorithmic 1.0 kflop per layer-step (SURVEY §8d); the U-D kernels execute fewer: see profiles/ for the executed FP32 rate",
                            hbm=dict(achieved=bps * u / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s", frac=bps * u / t_launch / 1e9 / pk["hbm_gbs"],
@@ -475,9 +476,9 @@ def run_build(R, w, seed):
     in_bytes = n * (27 * 4 + 1 + 1 + 4 + 12)
     algo_bytes = BUILD_BYTES_POS * pos_tests + BUILD_BYTES_COV * chi2_evals + BUILD_BYTES_UPD * updates + out_bytes + in_bytes
     algo_flop = BUILD_FLOP_STEP * cand_steps + BUILD_FLOP_CHI2 * chi2_evals + BUILD_FLOP_UPDATE * updates
-    traffic, tcommit, twl = ncu_traffic("mkf_build_kernel/" + w)
+    traffic, tcommit, twl = ncu_traffic("mkf_build_kernel/" + w, nev)
     rec["roofline"] = dict(bound="hbm", kernel="mkf_build_kernel", achieved=algo_bytes / t_b / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
-                           frac=algo_bytes / t_b / 1e9 / pk["hbm_gbs"], traffic=traffic if a.scale == 1.0 else None, traffic_commit=tcommit,
+                           frac=algo_bytes / t_b / 1e9 / pk["hbm_gbs"], traffic=traffic, traffic_commit=tcommit,
                            algorithmic_bytes=algo_bytes, peak_source=pk["source"],
                            alu=dict(achieved=algo_flop / t_b / 1e12, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=algo_flop / t_b / 1e12 / pk["fp32_tflops"],
                                     algorithmic_flop=algo_flop, peak_source=pk["fp32_source"]),
@@ -561,9 +562,9 @@ def run_strips(R, w, seed):
     nclu = int(out["n_clusters"].item())
     algo = STRIP_BYTES_IN * float(n) + STRIP_BYTES_PER_CLUSTER * nclu
     t_launch = ms_step * 1e-3
-    traffic, tcommit, _ = ncu_traffic("sc_cluster_kernel")
+    traffic, tcommit, _ = ncu_traffic("sc_cluster_kernel", n)
     rec["roofline"] = dict(bound="hbm", kernel="sc_cluster_kernel", achieved=algo / t_launch / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
-                           frac=algo / t_launch / 1e9 / pk["hbm_gbs"], traffic=traffic if a.scale == 1.0 else None, traffic_commit=tcommit,
+                           frac=algo / t_launch / 1e9 / pk["hbm_gbs"], traffic=traffic, traffic_commit=tcommit,
                            algorithmic_bytes=algo, clusters=nclu, peak_source=pk["source"],
                            note="7 B per strip in (adc u16, noise f32, bad u8) + 20 B per cluster out; the timed step also holds one memset of the tile states")
     if not a.no_cpu_baseline:
