@@ -364,6 +364,25 @@ def run_fit(R, w, seed, workload=None):
             return float(r["nfit"].sum()), r["h2d_bytes"], r["d2h_bytes"]
         rec["e2e"] = R.e2e(e2e_step, METRIC["fit"][1])
         del hits_p, seeds_p, out_p
+    # ---- f1: the two-filter smoother (mkf_fit_smooth, reading R14) on the first quarter of the tracks ----------------
+    if w == "fit" and not a.no_chain:
+        ns = max(1, n // 4)
+        mpl = ds["track_hits"].shape[0]
+        sds = {k: (v[..., :ns].contiguous() if k != "plan" and k != "q" else v[:ns].contiguous()) for k, v in ds.items()}
+        par_s = torch.empty((mpl, 6, ns), dtype=torch.float32, device="cuda")
+        cov_s = torch.empty((mpl, 21, ns), dtype=torch.float32, device="cuda")
+        so = B.alloc_fit_out(ns)
+        wss = torch.empty(max(ctx.workspace_bytes(B.CALL_FIT_SMOOTH, 0, 0, ns), 256), dtype=torch.uint8, device="cuda")
+
+        def smooth_step():
+            ctx.fit_smooth(dh, sds, sds["plan"], sds["track_hits"], par_s, cov_s, so["chi2"], so["nfit"], so["status"], wss)
+        ms_s, _, clk_s = R.timed(ctx, smooth_step, steps=min(a.steps, 10))
+        us = float(so["nfit"].sum().item())
+        ts = ms_s / min(a.steps, 10) * 1e-3
+        rec["smoother"] = dict(workload="mkf_fit_smooth on the first %d helices of configs[1]: forward pass, backward pass and the combined state at every fitted hit" % ns,
+                               value=us / ts, unit="smoothed layer-steps/s", ms_per_step=ts * 1e3, units_per_step=us, clocks=clk_s,
+                               out_bytes_per_layer_step=27 * 4, workspace_bytes=int(wss.numel()))
+        del par_s, cov_s, wss, sds
     if R.rank != 0:
         return rec
     # ---- roofline of the kernel (the step is one launch) ---------------------------------------------------------
@@ -524,8 +543,43 @@ def run_build(R, w, seed):
                                   value=uf / tf, unit="layer-steps/s", ms_per_step=ms_f / a.steps, units_per_step=uf, clocks=clk,
                                   roofline=dict(bound="alu", kernel="mkf_fit_kernel", achieved=ALGO_FLOP_PER_LAYER_STEP * uf / tf / 1e12, peak=pk["fp32_tflops"],
                                                 unit="TFLOP/s", frac=ALGO_FLOP_PER_LAYER_STEP * uf / tf / 1e12 / pk["fp32_tflops"]))
+    # ---- f2: overlap-hit recovery on the configs[3] recipe with a quarter of the crossings seen by a second module ----
+    if which == 3 and not a.no_chain:
+        rec["overlap_recovery"] = run_overlap(R, seed)
     ctx.close()
     return rec
+
+
+def run_overlap(R, seed):
+    """mkf_build_hit_index + mkf_build_tracks_overlap (reading R15) on 50 events x scale of the configs[3]
+    recipe generated with overlap_frac = 0.25 (module ids from the generator)."""
+    import torch
+    from paper_2002_06295_b200 import binding as B
+    a = R.a
+    ev, prm = make_build_workload(3, seed, 0.25 * a.scale, overlap_frac=0.25)
+    geom, hits, s = ev["geom"], ev["hits"], ev["seeds"]
+    ctx = B.Context(geom, prm)
+    dh = B.hits_to_device(hits, with_module=True)
+    nh, nev, n = hits["x"].shape[0], hits["n_events"], s["par"].shape[1]
+    idx, ws = B.alloc_hit_index(ctx, nev, nh)
+    ds = B.to_device(dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"]), ["par", "cov", "q", "plan", "event", "hits"])
+    out = B.alloc_build_out(n, ctx.max_plan_len)
+    h2 = torch.empty((ctx.max_plan_len, n), dtype=torch.int32, device="cuda")
+    wso = torch.empty(max(ctx.workspace_bytes(B.CALL_BUILD_TRACKS_OVERLAP, nev, nh, n), 256), dtype=torch.uint8, device="cuda")
+
+    def step(h2=h2):
+        ctx.build_hit_index(dh, idx, ws)
+        ctx.build_tracks(dh, idx, ds, ds["event"], ds["hits"], ds["plan"], out, out["chi2"], out["score"], out["nhits"],
+                         out["nmiss"], out["hit_ids"], out["status"], ws=wso, hit_ids2=h2)
+
+    ms_o, launches, clk = R.timed(ctx, step)
+    ms_p, _, _ = R.timed(ctx, lambda: step(None), warm=1)
+    n2 = int((h2 >= 0).sum().item())
+    ctx.close()
+    return dict(workload="configs[3] recipe, %d events, overlap_frac 0.25: mkf_build_hit_index + mkf_build_tracks_overlap" % nev,
+                value=nev / (ms_o / a.steps * 1e-3), unit="events/s", ms_per_step=ms_o / a.steps, units_per_step=float(nev), clocks=clk,
+                gpu_launches=int(launches), n_hits=int(nh), n_seeds=int(n), second_hits_attached=n2,
+                ms_per_step_without_recovery=ms_p / a.steps)
 
 
 def run_strips(R, w, seed):
@@ -647,7 +701,7 @@ def main():
                 ms_per_step=head["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None, dtype=head["dtype"], data="synthetic",
                 config=cfg, clocks=head["clocks"], e2e=head.get("e2e"), gpu_launches=head["gpu_launches"], roofline=head.get("roofline"),
                 cpu_baseline=head.get("cpu_baseline"), impl="mkf", units_per_step=head["units_per_step"])
-    for k in ("parts", "chained_fit", "pack_hits_ms", "pack_hits_gbs", "n_hits", "n_seeds"):
+    for k in ("parts", "chained_fit", "overlap_recovery", "smoother", "pack_hits_ms", "pack_hits_gbs", "n_hits", "n_seeds"):
         if k in head:
             line[k] = head[k]
     if others:

@@ -74,35 +74,38 @@ def shuffle_hit_order(hits, seeds, seed):
 
 
 def _build_chunk(job):
-    which, n_ev, seed = job
-    ev, prm = datagen.config(which, scale=n_ev / BUILD_EVENTS[which], seed=seed)
+    which, n_ev, seed, ovl = job
+    ev, prm = datagen.config(which, scale=n_ev / BUILD_EVENTS[which], seed=seed, **(dict(overlap_frac=ovl) if ovl else {}))
     s = ev["seeds"]
     keep = dict(par=s["par"], cov=s["cov"], q=s["q"], plan=s["plan"], event=s["event"], hits=s["hits"], track_hits=s["track_hits"])
     return ev["geom"], prm, ev["hits"], keep
 
 
-def make_build_workload(which, seed, scale):
+def make_build_workload(which, seed, scale, overlap_frac=0.0):
     """configs[2..4] as chunks of BUILD_CHUNK events (seeds 64 seed + k), concatenated: hit ids, event ids offset.
-    At scale <= one chunk this is exactly datagen.config(which, scale, 64 seed)."""
+    At scale <= one chunk this is exactly datagen.config(which, scale, 64 seed). overlap_frac > 0 (configs[3] only):
+    that fraction of the crossings is also seen by a neighbouring module; hits then carry `module`."""
     total = max(1, int(round(BUILD_EVENTS[which] * scale)))
     per = BUILD_CHUNK[which]
     jobs, done, k = [], 0, 0
     while done < total:
         m = min(per, total - done)
-        jobs.append((which, m, seed * 64 + k)); done += m; k += 1
+        jobs.append((which, m, seed * 64 + k, overlap_frac)); done += m; k += 1
     res = _pool_map(_build_chunk, jobs)
     geom, prm = res[0][0], res[0][1]
     nl = len(geom["layers"])
-    X, Y, Z, V, LO, S = [], [], [], [], [], []
+    X, Y, Z, V, LO, S, MOD = [], [], [], [], [], [], []
     nh0 = ev0 = 0
     for _, _, h, s in res:
-        X.append(h["x"]); Y.append(h["y"]); Z.append(h["z"]); V.append(h["V"])
+        X.append(h["x"]); Y.append(h["y"]); Z.append(h["z"]); V.append(h["V"]); MOD.append(h["module"])
         LO.append(h["layer_off"].astype(np.int64) + nh0)
         s = dict(s, event=s["event"] + ev0, hits=s["hits"] + nh0, track_hits=np.where(s["track_hits"] >= 0, s["track_hits"] + nh0, s["track_hits"]))
         S.append(s)
         nh0 += h["x"].shape[0]; ev0 += h["n_events"]
     hits = dict(n_events=ev0, layer_off=np.concatenate(LO).astype(np.int32), x=np.concatenate(X), y=np.concatenate(Y), z=np.concatenate(Z),
                 V=np.ascontiguousarray(np.concatenate(V, axis=1)))
+    if overlap_frac:
+        hits["module"] = np.concatenate(MOD).astype(np.int32)
     assert hits["layer_off"].shape[0] == ev0 * (nl + 1)
     seeds = {k2: np.ascontiguousarray(np.concatenate([s[k2] for s in S], axis=-1)) for k2 in S[0]}
     return dict(geom=geom, hits=hits, seeds=seeds), prm

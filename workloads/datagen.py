@@ -438,7 +438,7 @@ def make_events(geom, seed, n_events, n_primary, n_secondary=0, n_noise=0, spect
 # ------------------------------------------------------------------------------------------------------
 # the five BASELINE.json configs (scale < 1 shrinks counts for tests; geometry and distributions unchanged)
 # ------------------------------------------------------------------------------------------------------
-def config(i, scale=1.0, seed=0):
+def config(i, scale=1.0, seed=0, overlap_frac=0.0):
     s = lambda v, lo=1: max(lo, int(round(v * scale)))
     if i == 0:
         g = geometry_barrel(10, 4.0, 40.0, 100.0, 0.02)
@@ -452,7 +452,7 @@ def config(i, scale=1.0, seed=0):
     if i == 3:
         g = geometry_barrel_endcap()
         return (make_events(g, seed, s(200), 1500, n_secondary=3900, n_noise=16000, spectrum="soft",
-                            pt_range=(0.3, 50.0), n_hard=50, eta_max=2.5, eff=0.95, seed_on_pixel=True),
+                            pt_range=(0.3, 50.0), n_hard=50, eta_max=2.5, eff=0.95, seed_on_pixel=True, overlap_frac=overlap_frac),
                 default_params(max_cand=6, min_hits_keep=4))
     if i == 4:
         g = geometry_barrel_endcap()
