@@ -152,7 +152,10 @@ static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_st
 }
 
 // ---- two-filter smoother (reading R14) ----------------------------------------------------------------
-__global__ void __launch_bounds__(FIT_BLOCK) mkf_fit_smooth_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ ParamsDev p,
+#ifndef MKF_SMOOTH_MIN_BLOCKS
+#define MKF_SMOOTH_MIN_BLOCKS 3
+#endif
+__global__ void __launch_bounds__(FIT_BLOCK, MKF_SMOOTH_MIN_BLOCKS) mkf_fit_smooth_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ ParamsDev p,
                                                                    const __grid_constant__ SmoothArgs a) {
   const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
   if (i < a.f.n) fit_smooth_one(g, p, a, i);

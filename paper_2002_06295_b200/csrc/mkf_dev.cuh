@@ -390,10 +390,13 @@ MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArg
   KState S;
   load_params(S, a.par, n, (size_t)i);
   float c2tot = 0.f; int nf = 0, last_s = -1; bool smoothable = true;
-  for (int s = 0; s < plen; s++) {
-    const int hid = a.track_hits[(size_t)s * n + i];
+  int hid_next = plen > 0 ? a.track_hits[i] : -1;                // ids one step ahead, the hit before the propagation:
+  for (int s = 0; s < plen; s++) {                               // their latency overlaps the arithmetic
+    const int hid = hid_next;
+    hid_next = s + 1 < plen ? a.track_hits[(size_t)(s + 1) * n + i] : -1;
     if (hid < 0) continue;
     if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; break; }
+    Hit H; load_hit(H, a.hits, hid);
     const int li = g.plan_layers[p0 + s];
     const LayerDev& L = g.layers[li];
     const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
@@ -406,7 +409,6 @@ MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArg
     for (int k = 0; k < 10; k++) w[(9 + k) * st] = S.u[k];
 #pragma unroll
     for (int k = 0; k < 5; k++) w[(19 + k) * st] = S.d[k];
-    Hit H; load_hit(H, a.hits, hid);
     SInv o; float c2;
     hit_to_local(S, H, o);
     if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; smoothable = false; break; }
@@ -419,9 +421,12 @@ MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArg
 #pragma unroll
     for (int k = 0; k < 5; k++) S.d[k] *= 1e4f;                  // the backward filter starts from a weak prior
     int prev = -1;
+    hid_next = a.track_hits[(size_t)last_s * n + i];
     for (int s = last_s; s >= 0 && ok; s--) {
-      const int hid = a.track_hits[(size_t)s * n + i];
+      const int hid = hid_next;
+      hid_next = s > 0 ? a.track_hits[(size_t)(s - 1) * n + i] : -1;
       if (hid < 0) continue;
+      Hit H; load_hit(H, a.hits, hid);
       const int li = g.plan_layers[p0 + s];
       const LayerDev& L = g.layers[li];
       float J = 1.f, th02 = 0.f, q4 = 0.f;
@@ -435,7 +440,6 @@ MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArg
       const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[prev >= 0 ? prev : li], p.graze_cos_min, 0, false, P);
       if (rc) { stat |= rc; ok = false; break; }
       commit_step_backward(S, P, J, th02, q4, p.material_flags);
-      Hit H; load_hit(H, a.hits, hid);
       SInv o; float c2;
       hit_to_local(S, H, o);
       if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
