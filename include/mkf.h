@@ -96,7 +96,8 @@ typedef struct { int n_events; int n_hits; const int* layer_off;
  *          segment (ev*n_layers + l)), last entry = n_hits;
  * sorted_id[n_hits]  hit ids ordered by (segment, bin, id);
  * vmax     [n_events*n_layers*2]  per segment: max over hits of the larger eigenvalue of the xy block of V, max V_zz;
- * packed   [n_hits*12]  the hits in sorted order, as a block of n_hits 16-byte positions {x,y,z,id(bits)} followed by
+ * packed   [n_hits*12 + 4]  the hits in sorted order, as a block of n_hits 16-byte positions {x,y,z,id(bits)} followed,
+ *          from float 4*(n_hits + (n_hits & 1)) on (so that every record is one 32-byte sector; 256-byte aligned base), by
  *          a block of n_hits 32-byte covariances {Vxx,Vxy,Vyy,Vxz | Vyz,Vzz,module(bits),0} (a derived copy so that a bin scan
  *          reads contiguous memory; may be NULL in mkf_build_hit_index, in which case mkf_build_tracks gathers from
  *          the SoA arrays instead). */

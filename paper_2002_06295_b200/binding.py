@@ -204,7 +204,7 @@ class Context:
         """mask (uint8 CUDA tensor [n_hits] or None): mkf_build_hit_index_masked (reading R9).
         hits: dict of CUDA tensors (layer_off int32, x,y,z float32 [n], V float32 [6,n]); out: dict(bin_off int32
         [n_events*n_layers*n_bins+1] (unsigned offsets), sorted_id int32 [n], vmax float32 [n_events*n_layers*2],
-        packed float32 [n*12] or None); ws: uint8 CUDA tensor."""
+        packed float32 [n*12 + 4] or None); ws: uint8 CUDA tensor."""
         hs = self.hits_struct(hits, _dev)
         packed = out.get("packed")
         idx = HitIndex(_dev(out["bin_off"], torch.int32), _dev(out["sorted_id"], torch.int32), _dev(out["vmax"], torch.float32),
@@ -403,7 +403,7 @@ def alloc_hit_index(ctx, n_events, n_hits, packed=True, device="cuda"):
     out = dict(bin_off=torch.empty(nseg * ctx.n_bins + 1, dtype=torch.int32, device=device),
                sorted_id=torch.empty(n_hits, dtype=torch.int32, device=device),
                vmax=torch.empty(nseg * 2, dtype=torch.float32, device=device),
-               packed=torch.empty(n_hits * 12, dtype=torch.float32, device=device) if packed else None)
+               packed=torch.empty(n_hits * 12 + 4, dtype=torch.float32, device=device) if packed else None)
     ws = torch.empty(max(ctx.workspace_bytes(CALL_BUILD_HIT_INDEX, n_events, n_hits, 0), 256), dtype=torch.uint8, device=device)
     return out, ws
 

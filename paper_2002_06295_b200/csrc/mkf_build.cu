@@ -283,7 +283,7 @@ __device__ __noinline__ int overlap_hit(const BuildArgs& a, const ParamsDev& p, 
     Hit H2; int id2, mod2;
     if (a.packed) {
       const float4 q0 = __ldg(a.packed + t2);
-      const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t2;
+      const float4* cv = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * t2;
       const float4 b = __ldg(cv), d = __ldg(cv + 1);
       H2.x = q0.x; H2.y = q0.y; H2.z = q0.z; id2 = __float_as_int(q0.w); mod2 = __float_as_int(d.z);
       H2.v[0] = b.x; H2.v[1] = b.y; H2.v[2] = b.z; H2.v[3] = b.w; H2.v[4] = d.x; H2.v[5] = d.y;
@@ -558,7 +558,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           nt = r.y + (e & 0x3fffffu);
           if (a.packed) {
             nq0 = __ldg(a.packed + nt);
-            const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * nt;
+            const float4* cv = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * nt;
             nb4 = __ldg(cv); nd4 = __ldg(cv + 1);
           }
         };
@@ -704,7 +704,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         if (a.packed) {
           const int t = sm.sel_t[cslot];
           const float4 q0 = __ldg(a.packed + t);
-          const float4* cv = a.packed + (size_t)a.hits.n_hits + (size_t)2 * t;
+          const float4* cv = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * t;
           const float4 b = __ldg(cv), d = __ldg(cv + 1);
           H.x = q0.x; H.y = q0.y; H.z = q0.z; c_hit = __float_as_int(q0.w); mod1 = __float_as_int(d.z);
           H.v[0] = b.x; H.v[1] = b.y; H.v[2] = b.z; H.v[3] = b.w; H.v[4] = d.x; H.v[5] = d.y;

@@ -73,6 +73,10 @@ MKF_HD unsigned step_to_layer(KState& S, bool first, const float* cov, size_t n,
   return 0;
 }
 
+// packed hit index (mkf_hit_index.packed): first float4 of the covariance block; even, so that every 32-byte covariance
+// record is one whole sector
+MKF_HD size_t packed_cov_off(int n_hits) { return (size_t)n_hits + (size_t)(n_hits & 1); }
+
 MKF_HD void load_hit(Hit& H, const HitsDev& h, int id) {
 #ifdef __CUDA_ARCH__
   if (h.rec) {                                                   // 48-byte record: 2 sectors instead of 9 for a scattered id

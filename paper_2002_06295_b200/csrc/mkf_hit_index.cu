@@ -138,14 +138,14 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
   // positions first (16 B per hit, what the window scan reads for every hit), covariances behind them (32 B per
   // hit, read only for the hits that survive the position test)
   a.packed[t] = make_float4(a.hits.x[id], a.hits.y[id], a.hits.z[id], __int_as_float(id));
-  float4* o = a.packed + nh + (size_t)2 * t;
+  float4* o = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * t;
   o[0] = make_float4(V[id], V[nh + id], V[2 * nh + id], V[3 * nh + id]);
   o[1] = make_float4(V[4 * nh + id], V[5 * nh + id], a.hits.module ? __int_as_float(a.hits.module[id]) : 0.f, 0.f);
 }
 
 
 // ---- the plain index in one kernel ------------------------------------------------------------------------------------
-constexpr int HF_BLOCK = 256, HF_WARPS = HF_BLOCK / 32;
+constexpr int HF_BLOCK_SMALL = 256, HF_BLOCK_LARGE = 1024;     // threads per segment: segments of up to / beyond HF_LARGE_SEG hits on average
 constexpr int HF_TMPCAP = 10240;     // ids of a segment kept in shared memory between the scatter and the ranking (the rest: workspace)
 
 // Bin key of a hit, identical to the fp64 evaluation of C8 (U12): fp32 first; the fp64 formulas only when the fp32
@@ -176,7 +176,9 @@ __device__ __forceinline__ int bin_key(float xf, float yf, float zf, float elo_f
 //      stable order of C8, no sort and no dependent probing: the bin's few ids are independent loads); it writes its id
 //      and its packed record there. Hits are read in id order (coalesced) in every pass; two hits per thread and
 //      iteration keep more loads in flight.
+template <int HF_BLOCK>
 __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
+  constexpr int HF_WARPS = HF_BLOCK / 32;
   extern __shared__ unsigned hf_cnt[];                        // [nb] counts, then cursors; [HF_TMPCAP] ids by bin
   __shared__ float s_xy[HF_WARPS], s_zz[HF_WARPS];
   __shared__ unsigned s_ws[HF_WARPS];
@@ -272,9 +274,12 @@ __global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constan
     a.sorted_id[t] = i;
     if (a.packed) {
       a.packed[t] = make_float4(x, y, z, __int_as_float(i));
-      float4* o = a.packed + nh + (size_t)2 * t;
-      o[0] = make_float4(v0, v1, v2, v3);
-      o[1] = make_float4(v4, v5, a.hits.module ? __int_as_float(a.hits.module[i]) : 0.f, 0.f);
+      float4* o = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * t;
+      const float md = a.hits.module ? __int_as_float(a.hits.module[i]) : 0.f;
+      // one 32-byte store where the block is sector-aligned: a scattered whole-sector write needs no fill from DRAM
+      if (((size_t)o & 31) == 0)
+        asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" :: "l"(o), "f"(v0), "f"(v1), "f"(v2), "f"(v3), "f"(v4), "f"(v5), "f"(md), "f"(0.f) : "memory");
+      else { o[0] = make_float4(v0, v1, v2, v3); o[1] = make_float4(v4, v5, md, 0.f); }
     }
   };
   for (int i0 = b + tid; i0 < e; i0 += 2 * HF_BLOCK) {
@@ -330,10 +335,11 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
   a.mask = mask; a.n_bins = nbins;
   const size_t fused_smem = (size_t)c->g.n_phi * c->g.n_eta * 4 + (size_t)HF_TMPCAP * 4;
-  // The single-kernel path pays off while a segment is small enough for a CTA's share of L2 (measured: 0.19 against
-  // 0.34 ms on configs[2], 0.76 against 1.37 ms on configs[3], but 2.1 against 1.6 ms on the 7.5 k-hit segments of
-  // configs[4], where 592 CTAs in flight thrash L2 with their scattered record writes).
-  if (!mask && fused_smem <= 200 * 1024 && (size_t)h->n_hits <= (size_t)nseg * 4096) {
+  // One kernel while the counts fit in shared memory (measured against the five kernels: 0.16 / 0.34 ms on configs[2],
+  // 0.65 / 1.37 on configs[3], 1.2 / 1.64 on configs[4]); 256 threads per segment up to 4096 hits per segment on
+  // average, 1024 beyond (configs[4], 7.6 k hits per segment: 2.1 ms with 256 threads).
+  const int mode = (size_t)h->n_hits <= (size_t)nseg * 4096 ? 1 : 2;
+  if (!mask && fused_smem <= 100 * 1024) {
     if (h->n_hits == 0) {                                      // nothing to place: all offsets are zero
       cudaError_t e0 = cudaMemsetAsync(a.bin_off, 0, (nbins + 1) * 4, st);
       if (e0 == cudaSuccess) e0 = cudaMemsetAsync(a.vmax, 0, (size_t)nseg * 8, st);
@@ -341,10 +347,12 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
       return MKF_OK;
     }
     {
-      cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
+      cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel<HF_BLOCK_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
+      if (e1 == cudaSuccess) e1 = cudaFuncSetAttribute(hi_fused_kernel<HF_BLOCK_LARGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
       if (e1 != cudaSuccess) return cuda_fail(c, e1, "mkf_build_hit_index: shared memory attribute");
     }
-    hi_fused_kernel<<<nseg, HF_BLOCK, fused_smem, st>>>(c->g, a);
+    if (mode == 2) hi_fused_kernel<HF_BLOCK_LARGE><<<nseg, HF_BLOCK_LARGE, fused_smem, st>>>(c->g, a);
+    else hi_fused_kernel<HF_BLOCK_SMALL><<<nseg, HF_BLOCK_SMALL, fused_smem, st>>>(c->g, a);
     MKF_LAUNCHED(c, "hi_fused_kernel");
     return MKF_OK;
   }

@@ -207,14 +207,14 @@ extern "C" int mkf_build_host(mkf_ctx* c, const mkf_hits* h, const mkf_states* s
   const size_t wsb = (ws1 > ws2 ? ws1 : ws2) > ws3 ? (ws1 > ws2 ? ws1 : ws2) : ws3;
   const size_t need = hits_bytes(c, h) + Arena::pad(n * 24) * 2 + Arena::pad(n * 84) * 2 + 3 * Arena::pad(n) + Arena::pad(n * 4) * 7 +
                       Arena::pad(n * 12) + Arena::pad(n * mpl * 4) + Arena::pad((nbins + 1) * 4) + Arena::pad(nh * 4) +
-                      Arena::pad((size_t)nev * c->g.n_layers * 8) + Arena::pad(nh * 48) + Arena::pad(wsb) + Arena::pad(((size_t)nev + 1) * 4) * 2 + 8192;
+                      Arena::pad((size_t)nev * c->g.n_layers * 8) + Arena::pad(nh * 48 + 16) + Arena::pad(wsb) + Arena::pad(((size_t)nev + 1) * 4) * 2 + 8192;
   Arena A(c, need);
   cudaStream_t s_in = A.h->s_in, s_k = A.h->s_k, s_out = A.h->s_out;
   mkf_hits dh = upload_hits(A, c, h, s_in);
   A.chain(s_in, s_k);                                          // the hit index starts while the seeds are still on their way
   mkf_hit_index idx;
   idx.bin_off = A.alloc<unsigned>(nbins + 1); idx.sorted_id = A.alloc<int>(nh); idx.vmax = A.alloc<float>((size_t)nev * c->g.n_layers * 2);
-  idx.packed = A.alloc<float>(12 * nh);
+  idx.packed = A.alloc<float>(12 * nh + 4);
   char* ws = A.alloc<char>(wsb);
   if (A.err != cudaSuccess) return cuda_fail(c, A.err, "mkf_build_host: staging");
   int rc = mkf_build_hit_index(c, &dh, &idx, ws, wsb, s_k);

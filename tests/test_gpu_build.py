@@ -22,7 +22,8 @@ def check_index(ev, prm):
     sid = ref["sorted_id"]
     h = ev["hits"]
     nh = len(sid)
-    pos, cv = got["packed"][:4 * nh].reshape(nh, 4), got["packed"][4 * nh:].reshape(nh, 8)
+    c0 = 4 * (nh + (nh & 1))                                  # the covariance block starts on a whole sector
+    pos, cv = got["packed"][:4 * nh].reshape(nh, 4), got["packed"][c0:c0 + 8 * nh].reshape(nh, 8)
     assert np.array_equal(pos[:, 3].copy().view(np.int32), sid)
     assert np.array_equal(pos[:, 0], h["x"][sid]) and np.array_equal(pos[:, 1], h["y"][sid]) and np.array_equal(pos[:, 2], h["z"][sid])
     assert np.array_equal(cv[:, :6], h["V"][:, sid].T)
