@@ -145,8 +145,16 @@ __global__ void __launch_bounds__(HI_BLOCK) hi_pack(const __grid_constant__ HiAr
 
 
 // ---- the plain index in one kernel ------------------------------------------------------------------------------------
-constexpr int HF_BLOCK_SMALL = 256, HF_BLOCK_LARGE = 1024;     // threads per segment: segments of up to / beyond HF_LARGE_SEG hits on average
-constexpr int HF_TMPCAP = 10240;     // ids of a segment kept in shared memory between the scatter and the ranking (the rest: workspace)
+// threads per segment, CTAs per SM, ids of a segment kept in shared memory between the scatter and the ranking (the rest:
+// workspace): for segments of up to / beyond 4096 hits on average
+// (measured on configs[2] / [3] / [4]: 256 x 4 CTAs and 1024 x 1: 0.16 / 0.66 / 0.76 ms; 256 x 6 with 6144 ids and 512 x 3:
+// 0.18 / 0.76 / 1.13; 256 x 5 with 8192 ids and 512 x 2: 0.17 / 0.70 / 0.94: more segments in flight than L2 holds cost more than
+// the occupancy gives)
+#define MKF_HF_S 256, 4, 10240
+#define MKF_HF_L 1024, 1, 10240
+template <int B, int M, int T> struct HfCfg { static constexpr int block = B, minb = M, tmpcap = T; };
+using HfSmall = HfCfg<MKF_HF_S>;
+using HfLarge = HfCfg<MKF_HF_L>;
 
 // Bin key of a hit, identical to the fp64 evaluation of C8 (U12): fp32 first; the fp64 formulas only when the fp32
 // value lies within 1e-3 bin widths of a bin edge (fp32 atan2f / asinhf are good to a few 1e-7 in value, 2e-5 in bin
@@ -176,9 +184,9 @@ __device__ __forceinline__ int bin_key(float xf, float yf, float zf, float elo_f
 //      stable order of C8, no sort and no dependent probing: the bin's few ids are independent loads); it writes its id
 //      and its packed record there. Hits are read in id order (coalesced) in every pass; two hits per thread and
 //      iteration keep more loads in flight.
-template <int HF_BLOCK>
-__global__ void __launch_bounds__(HF_BLOCK) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
-  constexpr int HF_WARPS = HF_BLOCK / 32;
+template <class CFG>
+__global__ void __launch_bounds__(CFG::block, CFG::minb) hi_fused_kernel(const __grid_constant__ GeomDev g, const __grid_constant__ HiArgs a) {
+  constexpr int HF_BLOCK = CFG::block, HF_WARPS = HF_BLOCK / 32, HF_TMPCAP = CFG::tmpcap;
   extern __shared__ unsigned hf_cnt[];                        // [nb] counts, then cursors; [HF_TMPCAP] ids by bin
   __shared__ float s_xy[HF_WARPS], s_zz[HF_WARPS];
   __shared__ unsigned s_ws[HF_WARPS];
@@ -334,25 +342,26 @@ extern "C" int mkf_build_hit_index_masked(mkf_ctx* c, const mkf_hits* h, const u
   unsigned* partial = (unsigned*)w;
   a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
   a.mask = mask; a.n_bins = nbins;
-  const size_t fused_smem = (size_t)c->g.n_phi * c->g.n_eta * 4 + (size_t)HF_TMPCAP * 4;
+  const size_t cnt_smem = (size_t)c->g.n_phi * c->g.n_eta * 4;
   // One kernel while the counts fit in shared memory (measured against the five kernels: 0.16 / 0.34 ms on configs[2],
-  // 0.65 / 1.37 on configs[3], 1.2 / 1.64 on configs[4]); 256 threads per segment up to 4096 hits per segment on
+  // 0.65 / 1.37 on configs[3], 0.77 / 1.64 on configs[4]); 256 threads per segment up to 4096 hits per segment on
   // average, 1024 beyond (configs[4], 7.6 k hits per segment: 2.1 ms with 256 threads).
   const int mode = (size_t)h->n_hits <= (size_t)nseg * 4096 ? 1 : 2;
-  if (!mask && fused_smem <= 100 * 1024) {
+  if (!mask && cnt_smem <= 64 * 1024) {
     if (h->n_hits == 0) {                                      // nothing to place: all offsets are zero
       cudaError_t e0 = cudaMemsetAsync(a.bin_off, 0, (nbins + 1) * 4, st);
       if (e0 == cudaSuccess) e0 = cudaMemsetAsync(a.vmax, 0, (size_t)nseg * 8, st);
       if (e0 != cudaSuccess) return cuda_fail(c, e0, "mkf_build_hit_index: memset");
       return MKF_OK;
     }
+    const size_t smem_s = cnt_smem + (size_t)HfSmall::tmpcap * 4, smem_l = cnt_smem + (size_t)HfLarge::tmpcap * 4;
     {
-      cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel<HF_BLOCK_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
-      if (e1 == cudaSuccess) e1 = cudaFuncSetAttribute(hi_fused_kernel<HF_BLOCK_LARGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem);
+      cudaError_t e1 = cudaFuncSetAttribute(hi_fused_kernel<HfSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s);
+      if (e1 == cudaSuccess) e1 = cudaFuncSetAttribute(hi_fused_kernel<HfLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l);
       if (e1 != cudaSuccess) return cuda_fail(c, e1, "mkf_build_hit_index: shared memory attribute");
     }
-    if (mode == 2) hi_fused_kernel<HF_BLOCK_LARGE><<<nseg, HF_BLOCK_LARGE, fused_smem, st>>>(c->g, a);
-    else hi_fused_kernel<HF_BLOCK_SMALL><<<nseg, HF_BLOCK_SMALL, fused_smem, st>>>(c->g, a);
+    if (mode == 2) hi_fused_kernel<HfLarge><<<nseg, HfLarge::block, smem_l, st>>>(c->g, a);
+    else hi_fused_kernel<HfSmall><<<nseg, HfSmall::block, smem_s, st>>>(c->g, a);
     MKF_LAUNCHED(c, "hi_fused_kernel");
     return MKF_OK;
   }
