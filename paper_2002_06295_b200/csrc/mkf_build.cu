@@ -305,7 +305,7 @@ __device__ __noinline__ int overlap_hit(const BuildArgs& a, const ParamsDev& p, 
 #ifndef MKF_BUILD_MIN_BLOCKS
 #define MKF_BUILD_MIN_BLOCKS (64 / MKF_BUILD_NS)
 #endif
-template <bool COUNT>
+template <bool COUNT, bool PACKED>
 __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(const __grid_constant__ GeomDev g,
                                                                 const __grid_constant__ ParamsDev p,
                                                                 const __grid_constant__ BuildArgs a) {
@@ -511,6 +511,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sm.runpre[mid] <= q) lo = mid; else hi = mid; }
           j = lo - 1; re = q;                                 // the first iteration opens run lo
         }
+#pragma unroll 1
         for (int it = 0; it < share; it++) {
           bool surv = false; unsigned ent = 0;
           if (q < qe) {
@@ -518,7 +519,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
               do { j++; rb = sm.runpre[j]; re = sm.runpre[j + 1]; } while (q >= re);
               const uint2 r = sm.rows[j];
               slot = (int)(r.x & 0xffu);
-              if (a.packed) {
+              if (PACKED) {
                 cx = sm.B[F_X][slot]; cy = sm.B[F_Y][slot]; cz = sm.B[F_Z][slot];
                 cxl = sm.B[F_XL][slot]; cyl = sm.B[F_YL][slot]; czl = sm.B[F_ZL][slot];
                 kind = __float_as_int(sm.B[F_FK][slot]); cb = sm.B[F_FCB][slot]; sb = sm.B[F_FSB][slot];
@@ -530,7 +531,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
             }
             ent = ((unsigned)j << 22) | (unsigned)(q - rb);
             if (COUNT) n_pos++;
-            if (a.packed) {
+            if (PACKED) {
               // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11); once
               // the candidate's list is full only a hit better than its last one can matter, so the cut follows it
               const float4 q0 = qn;
@@ -556,7 +557,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           const uint2 r = sm.rows[e >> 22];
           nslot = (int)(r.x & 0xffu);
           nt = r.y + (e & 0x3fffffu);
-          if (a.packed) {
+          if (PACKED) {
             nq0 = __ldg(a.packed + nt);
             const float4* cv = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * nt;
             nb4 = __ldg(cv); nd4 = __ldg(cv + 1);
@@ -566,7 +567,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         for (int k = lane; k < nproc; k += 32) {
           const int slot2 = nslot; const unsigned t = nt;
           Hit H2;
-          if (a.packed) {
+          if (PACKED) {
             H2.x = nq0.x; H2.y = nq0.y; H2.z = nq0.z;
             H2.v[0] = nb4.x; H2.v[1] = nb4.y; H2.v[2] = nb4.z; H2.v[3] = nb4.w; H2.v[4] = nd4.x; H2.v[5] = nd4.y;
           } else load_hit(H2, a.hits, a.sorted_id[t]);
@@ -701,7 +702,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       const int ps = (cslot & ~(G - 1)) + (c_sel & 7);        // parent's slot
       Hit H; int mod1 = 0;
       if (kind == 0) {                                        // the hit's record first: its latency overlaps the state loads
-        if (a.packed) {
+        if (PACKED) {
           const int t = sm.sel_t[cslot];
           const float4 q0 = __ldg(a.packed + t);
           const float4* cv = a.packed + packed_cov_off(a.hits.n_hits) + (size_t)2 * t;
@@ -961,15 +962,13 @@ static int build_tracks_common(mkf_ctx* c, const mkf_hits* h, const mkf_hit_inde
   MKF_LAUNCHED(c, "bs_order_kernel");
   const size_t smem = sizeof(Smem);
   const int grid = (a.n + NS - 1) / NS;
-  if (a.counters) {
-    e = cudaFuncSetAttribute(mkf_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
-    mkf_build_kernel<true><<<grid, BT, smem, st>>>(c->g, c->p, a);
-  } else {
-    e = cudaFuncSetAttribute(mkf_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
-    mkf_build_kernel<false><<<grid, BT, smem, st>>>(c->g, c->p, a);
-  }
+  // four instances: with / without the work counters, hits from the packed index / gathered by id
+  void (*kern)(GeomDev, ParamsDev, BuildArgs) =
+      a.counters ? (a.packed ? mkf_build_kernel<true, true> : mkf_build_kernel<true, false>)
+                 : (a.packed ? mkf_build_kernel<false, true> : mkf_build_kernel<false, false>);
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_tracks: shared memory attribute");
+  kern<<<grid, BT, smem, st>>>(c->g, c->p, a);
   MKF_LAUNCHED(c, "mkf_build_kernel");
   return MKF_OK;
 }
