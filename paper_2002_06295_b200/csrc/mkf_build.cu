@@ -241,6 +241,7 @@ constexpr unsigned long long KEY_NONE = ~0ull;
 __device__ __forceinline__ void accept_hit(Smem& sm, int slot, int nk, float c2, unsigned t) {
   unsigned long long key = ((unsigned long long)__float_as_uint(fmaxf(c2, 0.f)) << 32) | t;
   if (key >= sm.lkey[nk - 1][slot]) return;
+#pragma unroll 1
   for (int k = 0; k < nk; k++) {
     const unsigned long long old = atomicMin(&sm.lkey[k][slot], key);
     if (old == KEY_NONE) break;                                    // took an empty place
@@ -300,6 +301,13 @@ __device__ __noinline__ int overlap_hit(const BuildArgs& a, const ParamsDev& p, 
   if (!(kalman_update(S2, o, c2u) && state_finite(S2) && fabsf(c2u) <= 3.0e38f)) return -2;
   S = S2; chi2_add = c2u;
   return best_id;
+}
+
+// The state of a slot written to the output arrays (offers to `best short`, final readout): one copy of the U D U^T
+// expansion and the rotation to the global frame for its three call sites, out of the layer loop's instruction footprint.
+__device__ __noinline__ void store_slot_state(const float (*M)[SL], int slot, float* par_out, float* cov_out, size_t n, size_t i) {
+  KState S; ld_state(M, slot, S);
+  store_state(S, par_out, cov_out, n, i);
 }
 
 #ifndef MKF_BUILD_MIN_BLOCKS
@@ -370,9 +378,10 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           tb0 = __ldg(row + w0); te0 = __ldg(row + wend);
           if (wrap > 0) { tb1 = __ldg(row); te1 = __ldg(row + wrap); }
         }
-        // a run longer than RUN_MAX hits (never met in practice) goes in as several entries
+        // one entry per non-empty part; a run longer than RUN_MAX hits (never met in practice) goes in as several
         const unsigned n0 = ce0 - cb0, n1 = ce1 > cb1 ? ce1 - cb1 : 0u;
-        const int np = (int)((n0 + RUN_MAX - 1) / RUN_MAX + (n1 + RUN_MAX - 1) / RUN_MAX);
+        const bool lng = n0 > (unsigned)RUN_MAX || n1 > (unsigned)RUN_MAX;
+        const int np = lng ? (int)((n0 + RUN_MAX - 1) / RUN_MAX + (n1 + RUN_MAX - 1) / RUN_MAX) : (n0 ? 1 : 0) + (n1 ? 1 : 0);
         if (np == 0) continue;
         const int k = atomicAdd(&sm.n_rows, np);
         if (COUNT) n_rowt += np;
@@ -382,9 +391,16 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           if (COUNT) n_rowo += np;
           break;
         }
-        int kk = k;
-        for (unsigned o = 0; o < n0; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n0 - o, (unsigned)RUN_MAX) << 8), cb0 + o);
-        for (unsigned o = 0; o < n1; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n1 - o, (unsigned)RUN_MAX) << 8), cb1 + o);
+        if (!lng) {
+          if (n0) sm.rows[k] = make_uint2((unsigned)slot | (n0 << 8), cb0);
+          if (n1) sm.rows[k + (n0 ? 1 : 0)] = make_uint2((unsigned)slot | (n1 << 8), cb1);
+        } else {
+          int kk = k;
+#pragma unroll 1
+          for (unsigned o = 0; o < n0; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n0 - o, (unsigned)RUN_MAX) << 8), cb0 + o);
+#pragma unroll 1
+          for (unsigned o = 0; o < n1; o += RUN_MAX) sm.rows[kk++] = make_uint2((unsigned)slot | (min(n1 - o, (unsigned)RUN_MAX) << 8), cb1 + o);
+        }
       }
       sm.wrow[slot] = ie | (iend << 8);
     };
@@ -440,8 +456,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         sm.tt[slot] = tt; sm.tz[slot] = tz; sm.zz[slot] = zz;
         sm.lim1[slot] = (tt + vxy) * 1.0001f;
         sm.lim2[slot] = (zz + (L.kind == 0 ? vzz : vxy)) * 1.0001f;
-        sm.wrow[slot] = e0 | ((e1 + 1) << 8); sm.wphi[slot] = w0 | (wn << 8);
-        push_rows(slot);
+        sm.wrow[slot] = e0 | ((e1 + 1) << 8); sm.wphi[slot] = w0 | (wn << 8);     // its rows go to the table below
         int fl = FL_SCAN;
         // miss child (C9.5): stopped if it reaches the consecutive-miss limit
         if (consec + 1 >= p.max_consec_miss) { if (nh >= p.min_hits_keep) { fl |= FL_OFFER_MISS; sm.ostat[slot] = 0; } }
@@ -449,13 +464,19 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         sm.flag[slot] = fl;
       }
     }
-    __syncthreads();
 
     // ---- phase S: the hits of all runs of the table as ONE list. Pass A: every thread takes an equal share of it and
     // tests positions (16 B per hit); the survivors go to a queue. Pass B: one thread per queued survivor reads the
     // covariance (32 B) and evaluates chi2; accepted hits sink into their candidate's list. Both passes run with every
     // lane busy whatever the sizes of the windows. Further rounds while windows have rows left. --------------------------
-    for (;;) {
+    for (bool round0 = true;; round0 = false) {
+      if (!round0) {
+        __syncthreads();
+        if (tid == 0) { sm.n_rows = 0; sm.more = 0; }
+        __syncthreads();
+      }
+      if (tid < sm.nP) push_rows(sm.plist[tid]);              // the thread that propagated the slot (no barrier needed before)
+      __syncthreads();
       const int NR = min(sm.n_rows, ROWCAP);
       const int more = sm.more;
       // exclusive prefix of the run lengths
@@ -564,6 +585,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
           }
         };
         if (lane < nproc) fetch(lane);
+#pragma unroll 1
         for (int k = lane; k < nproc; k += 32) {
           const int slot2 = nslot; const unsigned t = nt;
           Hit H2;
@@ -594,11 +616,6 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       }
       __syncthreads();
       if (!more) break;
-      __syncthreads();
-      if (tid == 0) { sm.n_rows = 0; sm.more = 0; }
-      __syncthreads();
-      if (tid < sm.nP) push_rows(sm.plist[tid]);
-      __syncthreads();
     }
 
     // ---- the lists are sorted as they stand: count this slot's entries -----------------------------------------------
@@ -632,7 +649,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         }
         if (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2)) {
           const int src = gbase + ol;
-          if (sub == ol) { KState S; ld_state(ok >= G ? sm.B : sm.A, tid, S); store_state(S, a.par_out, a.cov_out, n, (size_t)i); }
+          if (sub == ol) store_slot_state(ok >= G ? sm.B : sm.A, tid, a.par_out, a.cov_out, n, (size_t)i);
           bs_have = true; bs_score = os; bs_chi2 = oc;
           bs_nh = __shfl_sync(gm, nh, src); bs_nm = __shfl_sync(gm, onm, src);
           bs_stat = __shfl_sync(gm, (fl & (FL_OFFER | FL_OFFER_MISS)) ? sm.ostat[tid] : 0u, src);
@@ -651,6 +668,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
       if (!parent_live) n_hitc = 0;
       int head = 0;
       int my_kind = -1, my_t = 0;
+#pragma unroll 1
       for (int r = 0; r < p.max_cand; r++) {
         // head child of this lane: its next hit or its miss / pass-through child, whichever ranks first (U14)
         unsigned long long k1 = KEY_NONE; int hh = HIT_NONE, hk = 3;
@@ -753,7 +771,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         }
         if (os > -INFINITY && (!bs_have || os > bs_score || (os == bs_score && oc < bs_chi2))) {
           const int src = gbase + ol;
-          if (sub == ol) { KState Sp; ld_state(sm.A, ps, Sp); store_state(Sp, a.par_out, a.cov_out, n, (size_t)i); }
+          if (sub == ol) store_slot_state(sm.A, ps, a.par_out, a.cov_out, n, (size_t)i);
           bs_have = true; bs_score = os; bs_chi2 = oc;
           bs_nh = __shfl_sync(gm, pnh, src); bs_nm = __shfl_sync(gm, pnm, src);
           bs_stat = 0;
@@ -819,7 +837,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
     float o_chi2, o_score; int o_nh, o_nm, bt_step, bt_slot, tail_step = -1, tail_val = -2; unsigned o_stat;
     if (live_wins) {
       const int src = gbase + fl2;
-      if (sub == fl2) { KState Sf; ld_state(sm.A, tid, Sf); store_state(Sf, a.par_out, a.cov_out, n, (size_t)i); }
+      if (sub == fl2) store_slot_state(sm.A, tid, a.par_out, a.cov_out, n, (size_t)i);
       o_chi2 = fc; o_score = fs;
       o_nh = __shfl_sync(gm, nh, src); o_nm = __shfl_sync(gm, nm, src); o_stat = 0;
       bt_step = t_last; bt_slot = fl2;
