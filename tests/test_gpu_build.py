@@ -56,6 +56,25 @@ def test_hit_index_empty_layers_and_crowded_bins():
     check_index(dict(geom=g, hits=hits), datagen.default_params())
 
 
+@pytest.mark.parametrize("n_per_layer", [6001, 12000])
+def test_hit_index_large_segments_odd_and_even_counts(n_per_layer):
+    """Segments beyond 4096 hits on average take the 1024-thread instance of the index kernel; 12000 hits per segment
+    exceed the id list it keeps in shared memory (the rest goes through the workspace). An odd total moves the
+    covariance block of the packed copy by one record (whole-sector records)."""
+    g = datagen.geometry_barrel(3, 10.0, 30.0, 50.0, 0.02)
+    rng = np.random.default_rng(11 + n_per_layer)
+    radii = np.array([l["pos"] for l in g["layers"]])
+    n = 3 * n_per_layer
+    ph = rng.uniform(-np.pi, np.pi, n); r = np.repeat(radii, n_per_layer)
+    x, y, z = r * np.cos(ph), r * np.sin(ph), rng.uniform(-50, 50, n)
+    V = np.zeros((6, n), np.float32); V[0] = rng.uniform(1e-6, 1e-4, n); V[2] = rng.uniform(1e-6, 1e-4, n); V[5] = rng.uniform(1e-5, 1e-3, n)
+    V[1] = 0.3 * np.sqrt(V[0] * V[2])
+    hits = dict(n_events=1, layer_off=(np.arange(4) * n_per_layer).astype(np.int32), x=x.astype(np.float32), y=y.astype(np.float32),
+                z=z.astype(np.float32), V=V)
+    assert (n % 2 == 1) == (n_per_layer % 2 == 1)
+    check_index(dict(geom=g, hits=hits), datagen.default_params())
+
+
 def compare_build(ev, prm, r, h, min_same=0.999):
     n = r["nhits"].shape[0]
     same = np.all(h["hit_ids"] == r["hit_ids"], axis=0)
