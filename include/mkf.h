@@ -126,6 +126,18 @@ int mkf_pack_hits(mkf_ctx*, const mkf_hits*, float* rec_out, void* stream);
  * UNSUPPORTED (n_hits >= 2^28), CUDA_ERROR. */
 int mkf_build_hit_index(mkf_ctx*, const mkf_hits*, mkf_hit_index* out, void* ws, size_t ws_bytes, void* stream);
 
+/* mkf_build_hit_index for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops): same inputs, same outputs (bit-identical), no workspace argument. Its scratch (8 bytes per hit) is a fixed
+ * array of 8 MiB inside the library's device image, held by every GPU that loads the library until exit; the call
+ * makes no cudaMalloc / cudaFree and calls no allocating routine (the first call on a device resolves the array's
+ * address once: make that call outside a capture). Limits: n_hits <= MKF_STATIC_MAX_HITS and at most 16384 bins
+ * per layer, else MKF_UNSUPPORTED with nothing launched; no masked variant. All calls on one device share the
+ * array: two calls that overlap on the GPU (different streams, no dependency between them) race and give undefined
+ * results; calls on one stream, or ordered by events, are safe. The array needs no clearing between calls.
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA_ERROR. */
+#define MKF_STATIC_MAX_HITS (1 << 20)
+int mkf_build_hit_index_static(mkf_ctx*, const mkf_hits*, mkf_hit_index* out, void* stream);
+
 /* a11 / C7 ("Fitting simply applies the KF procedure to all hits identified during building").
  * seeds: n states; plan[n]: plan id per track; track_hits[max_plan_len][n]: global hit id per plan step or <0.
  * For every step with a hit: propagate (C2/C3) -> grazing test (U7) -> covariance transport (C4) -> material

@@ -16,10 +16,11 @@ OK, INVALID_ARG, CUDA_ERROR, WORKSPACE_TOO_SMALL, UNSUPPORTED = 0, -1, -2, -3, -
 PROP_UNREACHABLE, GRAZING, S_NOT_PD, NAN, STOPPED_ELOSS, TRUNCATED = 1, 2, 4, 8, 16, 32
 CALL_BUILD_HIT_INDEX, CALL_FIT, CALL_BUILD_TRACKS, CALL_REMOVE_DUPLICATES = 0, 1, 2, 3
 CALL_FIT_SMOOTH, CALL_BUILD_TRACKS_OVERLAP = 5, 6
+STATIC_MAX_HITS = 1 << 20                      # MKF_STATIC_MAX_HITS of include/mkf.h
 
 EXPORTS = ["mkf_create", "mkf_destroy", "mkf_last_error", "mkf_workspace_bytes", "mkf_launch_count", "mkf_max_plan_len",
            "mkf_build_hit_index", "mkf_fit", "mkf_fit_backward", "mkf_build_tracks", "mkf_remove_duplicates", "mkf_fit_host", "mkf_fit_backward_host", "mkf_build_host",
-           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters", "mkf_fit_smooth", "mkf_build_tracks_overlap"]
+           "mkf_cluster_strips", "mkf_cluster_strips_host", "mkf_mask_hits", "mkf_build_hit_index_masked", "mkf_pack_hits", "mkf_set_build_counters", "mkf_fit_smooth", "mkf_build_tracks_overlap", "mkf_build_hit_index_static"]
 
 
 class Layer(C.Structure):
@@ -92,6 +93,7 @@ def lib():
         vp, sz, i = C.c_void_p, C.c_size_t, C.c_int
         L.mkf_build_hit_index.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), vp, sz, vp]
         L.mkf_build_hit_index_masked.argtypes = [vp, C.POINTER(Hits), vp, C.POINTER(HitIndex), vp, sz, vp]
+        L.mkf_build_hit_index_static.argtypes = [vp, C.POINTER(Hits), C.POINTER(HitIndex), vp]
         L.mkf_mask_hits.argtypes = [vp, i, i, vp, i, vp, vp, vp, i, C.c_float, vp, vp]
         L.mkf_fit.argtypes = [vp, C.POINTER(Hits), C.POINTER(States), vp, vp, i, C.POINTER(States), vp, vp, vp, vp, sz, vp]
         L.mkf_fit_backward.argtypes = L.mkf_fit.argtypes
@@ -217,6 +219,16 @@ class Context:
         self._check(rc, "mkf_build_hit_index")
 
     build_hit_index_masked = build_hit_index
+
+    def build_hit_index_static(self, hits, out):
+        """mkf_build_hit_index_static: the plain hit index with its scratch inside the library (no workspace, no
+        allocation; n_hits <= STATIC_MAX_HITS). hits, out as for build_hit_index."""
+        hs = self.hits_struct(hits, _dev)
+        packed = out.get("packed")
+        idx = HitIndex(_dev(out["bin_off"], torch.int32), _dev(out["sorted_id"], torch.int32), _dev(out["vmax"], torch.float32),
+                       _dev(packed, torch.float32) if packed is not None else None)
+        rc = self.L.mkf_build_hit_index_static(self.h, C.byref(hs), C.byref(idx), _stream())
+        self._check(rc, "mkf_build_hit_index_static")
 
     def mask_hits(self, hit_ids, nhits, chi2, keep, min_hits, max_chi2_ndf, mask):
         """mkf_mask_hits (reading R9): sets mask[h] = 1 for the hits of high-quality tracks; keep may be None."""

@@ -413,3 +413,72 @@ extern "C" int mkf_mask_hits(mkf_ctx* c, int n, int n_hits, const int* hit_ids, 
   MKF_LAUNCHED(c, "mh_mask_kernel");
   return MKF_OK;
 }
+
+// ---- the plain hit index without any caller- or library-allocated scratch ----------------------------------------
+// For callers that cannot allocate (CUDA graph capture, tight serving loops): the scratch of hi_fused_kernel (the
+// key and the scattered id of every hit, 2 x 4 B per hit) lives in a file-scope device array of
+// 2 x MKF_STATIC_MAX_HITS ints = 8 MiB, which every GPU that loads the library holds until exit. All calls on a device
+// share it: calls that overlap on the GPU race. Nothing in it has to start at zero (a call reads only words it has
+// written itself first), so it is not cleared between calls.
+namespace {
+static __device__ __align__(256) int g_hi_static_scratch[2 * (size_t)MKF_STATIC_MAX_HITS];
+
+constexpr int HI_MAX_DEVICES = 64;
+int* g_hi_static_ptr[HI_MAX_DEVICES];        // device address of the array per device (host code sees only a stand-in)
+bool g_hi_static_have[HI_MAX_DEVICES];
+
+// The array's device address on the current device: resolved once per device, with that device current.
+int hi_static_scratch(mkf_ctx* c, int** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_hit_index_static: cudaGetDevice");
+  if (dev < 0 || dev >= HI_MAX_DEVICES) return fail(c, MKF_UNSUPPORTED, "mkf_build_hit_index_static: device ordinal >= 64");
+  if (!g_hi_static_have[dev]) {
+    int* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_hi_static_scratch);
+    if (e != cudaSuccess || !p) return cuda_fail(c, e, "mkf_build_hit_index_static: cudaGetSymbolAddress");
+    g_hi_static_ptr[dev] = p;                // two threads racing here store the same value
+    g_hi_static_have[dev] = true;
+  }
+  *out = g_hi_static_ptr[dev];
+  return MKF_OK;
+}
+}  // namespace
+
+extern "C" int mkf_build_hit_index_static(mkf_ctx* c, const mkf_hits* h, mkf_hit_index* out, void* stream) {
+  if (!c) return MKF_INVALID_ARG;
+  if (!h || !out || !out->bin_off || !out->sorted_id || !out->vmax || !h->layer_off)
+    return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index_static: null argument");
+  if (h->n_events < 1 || h->n_hits < 0) return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index_static: bad sizes");
+  if (h->n_hits > MKF_STATIC_MAX_HITS)
+    return fail(c, MKF_UNSUPPORTED, "mkf_build_hit_index_static: n_hits exceeds MKF_STATIC_MAX_HITS (1048576); use mkf_build_hit_index");
+  if (h->n_hits > 0 && (!h->x || !h->y || !h->z || !h->V)) return fail(c, MKF_INVALID_ARG, "mkf_build_hit_index_static: null hit array");
+  const size_t cnt_smem = (size_t)c->g.n_phi * c->g.n_eta * 4;
+  if (cnt_smem > 64 * 1024)
+    return fail(c, MKF_UNSUPPORTED, "mkf_build_hit_index_static: more than 16384 bins per layer; use mkf_build_hit_index");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nseg = h->n_events * c->g.n_layers;
+  const size_t nbins = (size_t)nseg * c->g.n_phi * c->g.n_eta;
+  if (h->n_hits == 0) {                                        // nothing to place: all offsets are zero
+    cudaError_t e0 = cudaMemsetAsync(out->bin_off, 0, (nbins + 1) * 4, st);
+    if (e0 == cudaSuccess) e0 = cudaMemsetAsync(out->vmax, 0, (size_t)nseg * 8, st);
+    if (e0 != cudaSuccess) return cuda_fail(c, e0, "mkf_build_hit_index_static: memset");
+    return MKF_OK;
+  }
+  int* scratch = nullptr;
+  { const int rc = hi_static_scratch(c, &scratch); if (rc) return rc; }
+  HiArgs a;
+  a.hits = hits_dev(h); a.n_layers = c->g.n_layers; a.n_phi = c->g.n_phi; a.n_eta = c->g.n_eta;
+  a.key = scratch; a.tmp_id = scratch + MKF_STATIC_MAX_HITS; a.cnt = nullptr;
+  a.bin_off = out->bin_off; a.sorted_id = out->sorted_id; a.vmax = out->vmax; a.packed = (float4*)out->packed;
+  a.mask = nullptr; a.n_bins = nbins;
+  const size_t smem_s = cnt_smem + (size_t)HfSmall::tmpcap * 4, smem_l = cnt_smem + (size_t)HfLarge::tmpcap * 4;
+  const bool large = (size_t)h->n_hits > (size_t)nseg * 4096;
+  cudaError_t e1 = large ? cudaFuncSetAttribute(hi_fused_kernel<HfLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l)
+                         : cudaFuncSetAttribute(hi_fused_kernel<HfSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s);
+  if (e1 != cudaSuccess) return cuda_fail(c, e1, "mkf_build_hit_index_static: shared memory attribute");
+  if (large) hi_fused_kernel<HfLarge><<<nseg, HfLarge::block, smem_l, st>>>(c->g, a);
+  else hi_fused_kernel<HfSmall><<<nseg, HfSmall::block, smem_s, st>>>(c->g, a);
+  MKF_LAUNCHED(c, "hi_fused_kernel");
+  return MKF_OK;
+}
