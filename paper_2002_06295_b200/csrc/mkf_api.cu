@@ -78,20 +78,20 @@ constexpr int FIT_BLOCK = MKF_FIT_BLOCK;
 #define MKF_FIT_MIN_BLOCKS 5
 #endif
 
-template <bool STRAG>
+template <bool STRAG, bool PLANES>
 __global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_kernel(const __grid_constant__ GeomDev g,
                                                             const __grid_constant__ ParamsDev p,
                                                             const __grid_constant__ FitArgs a) {
   const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
-  if (i < a.n) fit_one<STRAG>(g, p, a, i);
+  if (i < a.n) fit_one<STRAG, PLANES>(g, p, a, i);
 }
 
-template <bool STRAG>
+template <bool STRAG, bool PLANES>
 __global__ void __launch_bounds__(FIT_BLOCK, MKF_FIT_MIN_BLOCKS) mkf_fit_backward_kernel(const __grid_constant__ GeomDev g,
                                                                         const __grid_constant__ ParamsDev p,
                                                                         const __grid_constant__ FitArgs a) {
   const int i = blockIdx.x * FIT_BLOCK + threadIdx.x;
-  if (i < a.n) fit_one_backward<STRAG>(g, p, a, i);
+  if (i < a.n) fit_one_backward<STRAG, PLANES>(g, p, a, i);
 }
 
 static int fit_common(mkf_ctx* c, bool backward, const mkf_hits* h, const mkf_states* seeds, const signed char* plan,
@@ -119,15 +119,14 @@ int fit_launch(mkf_ctx* c, bool backward, const FitArgs& a, cudaStream_t st) {
   if (a.n <= 0) return MKF_OK;
   const int grid = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
   const bool strag = (c->p.material_flags & 4) != 0;        // R12: its code is only in the kernels that need it
-  if (backward) {
-    if (strag) mkf_fit_backward_kernel<true><<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
-    else mkf_fit_backward_kernel<false><<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
-    MKF_LAUNCHED(c, "mkf_fit_backward_kernel");
-  } else {
-    if (strag) mkf_fit_kernel<true><<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
-    else mkf_fit_kernel<false><<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
-    MKF_LAUNCHED(c, "mkf_fit_kernel");
-  }
+  const bool pl = a.hits.rec == nullptr;                    // hits as planes: instances without the per-hit test of the record pointer
+  void (*kern)(GeomDev, ParamsDev, FitArgs) =
+      backward ? (strag ? (pl ? mkf_fit_backward_kernel<true, true> : mkf_fit_backward_kernel<true, false>)
+                        : (pl ? mkf_fit_backward_kernel<false, true> : mkf_fit_backward_kernel<false, false>))
+               : (strag ? (pl ? mkf_fit_kernel<true, true> : mkf_fit_kernel<true, false>)
+                        : (pl ? mkf_fit_kernel<false, true> : mkf_fit_kernel<false, false>));
+  kern<<<grid, FIT_BLOCK, 0, st>>>(c->g, c->p, a);
+  MKF_LAUNCHED(c, backward ? "mkf_fit_backward_kernel" : "mkf_fit_kernel");
   return MKF_OK;
 }
 }  // namespace mkf
