@@ -215,8 +215,12 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     // no `continue` / `break` out of the layer loop: tracks of one warp meet their first hit at different steps, and
     // threads that ran ahead would never rejoin the others (measured: 3x the instructions); the body is a plain
     // if-region, so the warp reconverges after every layer
+    const int* th = a.track_hits + (size_t)(plen - 1) * n + i;
+    int hid_next = plen - 1 > stop_at ? *th : -1;               // the hit id is fetched one step ahead
     for (int s = plen - 1; s > stop_at; s--) {
-      const int hid = a.track_hits[(size_t)s * n + i];
+      const int hid = hid_next;
+      th -= n;
+      hid_next = s - 1 > stop_at ? *th : -1;
       if (hid >= 0 && !stopped) do {
         if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; break; }
         const int li = g.plan_layers[p0 + s];
