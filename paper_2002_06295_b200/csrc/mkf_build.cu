@@ -526,7 +526,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
         const int qe = min(q + share, c1);
         int j = 0, rb = 0, re = 0, slot = 0, kind = 0;
         float cx = 0.f, cy = 0.f, cz = 0.f, cxl = 0.f, cyl = 0.f, czl = 0.f, cb = 0.f, sb = 0.f, l1 = 0.f, l2 = 0.f;
-        const unsigned* worst = nullptr; const float4* pp = nullptr; float4 qn = make_float4(0.f, 0.f, 0.f, 0.f);
+        const unsigned* worst = nullptr; const float4* pp = nullptr; float4 qn = make_float4(0.f, 0.f, 0.f, 0.f), qn2 = qn;
         if (q < qe) {
           int lo = 0, hi = NR;                                // run of hit q: last j with runpre[j] <= q
           while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sm.runpre[mid] <= q) lo = mid; else hi = mid; }
@@ -548,6 +548,7 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
                 worst = reinterpret_cast<const unsigned*>(&sm.lkey[p.max_cand - 1][slot]) + 1;    // chi2 bits of the list's last hit
                 pp = a.packed + r.y + (q - rb);
                 qn = __ldg(pp);
+                if (q + 1 < min(qe, re)) qn2 = __ldg(pp + 1);
               }
             }
             ent = ((unsigned)j << 22) | (unsigned)(q - rb);
@@ -556,8 +557,9 @@ __global__ void __launch_bounds__(BT, MKF_BUILD_MIN_BLOCKS) mkf_build_kernel(con
               // position first: chi2 >= (e.r)^2 / (e^T S e) for the unit vectors e = w1, w2 (Cauchy-Schwarz, U11); once
               // the candidate's list is full only a hit better than its last one can matter, so the cut follows it
               const float4 q0 = qn;
+              qn = qn2;
               pp++;
-              if (q + 1 < min(qe, re)) qn = __ldg(pp);
+              if (q + 2 < min(qe, re)) qn2 = __ldg(pp + 1);   // the hits two positions ahead of their use
               const float cut = fminf(p.chi2_cut, __uint_as_float(min(*(volatile const unsigned*)worst, 0x7f800000u)));
               const float rx = (q0.x - cx) - cxl, ry = (q0.y - cy) - cyl, rz = (q0.z - cz) - czl;
               const float r1 = kind == 0 ? cb * ry - sb * rx : rx, r2 = kind == 0 ? rz : ry;
