@@ -193,9 +193,12 @@ __global__ void __launch_bounds__(CFG::block, CFG::minb) hi_fused_kernel(const _
   const int seg = blockIdx.x;
   const int nb = a.n_phi * a.n_eta;
   int* s_tmp = reinterpret_cast<int*>(hf_cnt + nb);
+  unsigned short* s_tmp16 = reinterpret_cast<unsigned short*>(s_tmp);     // the same room holds twice as many ids as 16-bit
+                                                                          // offsets from the segment's first hit
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int ev = seg / a.n_layers, l = seg - ev * a.n_layers;
   const int b = a.hits.layer_off[ev * (a.n_layers + 1) + l], e = a.hits.layer_off[ev * (a.n_layers + 1) + l + 1];
+  const bool ids16 = e - b <= 65536;                          // (uniform in the CTA)
   for (int k = tid; k < nb; k += HF_BLOCK) hf_cnt[k] = 0u;
   __syncthreads();
   const float elo = g.layers[l].eta_lo, ehi = g.layers[l].eta_hi;
@@ -261,14 +264,20 @@ __global__ void __launch_bounds__(CFG::block, CFG::minb) hi_fused_kernel(const _
   __syncthreads();
   for (int i = b + tid; i < e; i += HF_BLOCK) {
     const unsigned pos = atomicAdd(&hf_cnt[a.key[i]], 1u);
-    if (pos - (unsigned)b < (unsigned)HF_TMPCAP) s_tmp[pos - b] = i; else a.tmp_id[pos] = i;
+    const unsigned o = pos - (unsigned)b;
+    if (ids16) { if (o < 2u * HF_TMPCAP) s_tmp16[o] = (unsigned short)(i - b); else a.tmp_id[pos] = i; }
+    else { if (o < (unsigned)HF_TMPCAP) s_tmp[o] = i; else a.tmp_id[pos] = i; }
   }
   __syncthreads();                                            // cursor[k] is now the end of bin k
   // rank of id i among the ids of its bin: four independent loads per round (a bin holds a handful of ids)
   auto place = [&](int i, int key) -> unsigned {
     const unsigned kb = key == 0 ? (unsigned)b : hf_cnt[key - 1], ke = hf_cnt[key];
     unsigned rank = 0;
-    auto at = [&](unsigned q) -> int { return q - (unsigned)b < (unsigned)HF_TMPCAP ? s_tmp[q - b] : a.tmp_id[q]; };
+    auto at = [&](unsigned q) -> int {
+      const unsigned o = q - (unsigned)b;
+      if (ids16) return o < 2u * HF_TMPCAP ? b + (int)s_tmp16[o] : a.tmp_id[q];
+      return o < (unsigned)HF_TMPCAP ? s_tmp[o] : a.tmp_id[q];
+    };
     for (unsigned q = kb; q < ke; q += 4) {
       const int v0 = at(q);
       const int v1 = q + 1 < ke ? at(q + 1) : 0x7fffffff;
