@@ -271,19 +271,21 @@ class Runner:
         self.torch, self.a, self.rank, self.local_rank, self.world, self.sampler = torch, a, rank, local_rank, world, sampler
         self.warm = max(a.warmup, 3)
         self.pk = peaks()
+        self.cdev = "cpu" if os.environ.get("MKF_BENCH_BACKEND") == "gloo" else "cuda"     # where the collectives' tensors live
 
-    def barrier(self):
-        if self.world > 1:
+    def barrier(self, ranks=True):
+        if self.world > 1 and ranks:
             import torch.distributed as dist
             dist.barrier()
         self.torch.cuda.synchronize()
 
-    def timed(self, ctx, step, steps=None, warm=None):
+    def timed(self, ctx, step, steps=None, warm=None, ranks=True):
+        """ranks=False: a measurement only rank 0 makes (no barrier between the ranks: the others are not there)."""
         torch = self.torch
         steps = steps or self.a.steps
         for _ in range(self.warm if warm is None else warm):
             step()
-        self.barrier()
+        self.barrier(ranks)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         l0 = ctx.launch_count()
         t0 = time.time()
@@ -291,7 +293,7 @@ class Runner:
         for _ in range(steps):
             step()
         e1.record()
-        self.barrier()
+        self.barrier(ranks)
         t1 = time.time()
         clocks = self.sampler.window(t0, t1) if self.sampler else None
         return e0.elapsed_time(e1), ctx.launch_count() - l0, clocks
@@ -305,7 +307,7 @@ class Runner:
             eu, h2d, d2h = fn()
         self.barrier()
         s = (time.perf_counter() - te) / self.a.e2e_steps
-        s, eu = aggregate(s, eu, self.world, "cuda")
+        s, eu = aggregate(s, eu, self.world, self.cdev)
         return dict(value=eu / s, unit=unit, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h), steps=self.a.e2e_steps,
                     ms_per_step=1e3 * s, host_memory="pinned", h2d_gbs=h2d / s / 1e9,
                     note="H2D of all inputs, kernels and D2H of all outputs inside the timed region (wall clock around the synchronous call)")
@@ -348,7 +350,7 @@ def run_fit(R, w, seed, workload=None):
 
     ms_total, launches, clocks = R.timed(ctx, step)
     u = float(out["nfit"].sum().item())
-    ms_total, u_all = aggregate(ms_total, u, R.world, "cuda")
+    ms_total, u_all = aggregate(ms_total, u, R.world, R.cdev)
     ms_step = ms_total / a.steps
     rec = dict(workload=NAMES[w], metric=METRIC["fit"][0], unit=METRIC["fit"][1], value=u_all / (ms_step * 1e-3), ms_per_step=ms_step,
                steps=a.steps, warmup=R.warm, units_per_step=u_all, gpu_launches=int(launches), clocks=clocks, dtype="f32", **extra)
@@ -456,7 +458,7 @@ def run_build(R, w, seed):
             dd()
 
     ms_total, launches, clocks = R.timed(ctx, step)
-    ms_total, u_all = aggregate(ms_total, float(nev), R.world, "cuda")
+    ms_total, u_all = aggregate(ms_total, float(nev), R.world, R.cdev)
     ms_step = ms_total / a.steps
     rec = dict(workload=NAMES[w], metric=METRIC["build"][0], unit=METRIC["build"][1], value=u_all / (ms_step * 1e-3), ms_per_step=ms_step,
                steps=a.steps, warmup=R.warm, units_per_step=u_all, gpu_launches=int(launches), clocks=clocks, dtype="f32",
@@ -536,7 +538,7 @@ def run_build(R, w, seed):
 
         def fit_step():
             ctx.fit(dh, ds, ds["plan"], th, fo, fo["chi2"], fo["nfit"], fo["status"])
-        ms_f, _, clk = R.timed(ctx, fit_step)
+        ms_f, _, clk = R.timed(ctx, fit_step, ranks=False)
         uf = float(fo["nfit"].sum().item())
         tf = ms_f / a.steps * 1e-3
         rec["chained_fit"] = dict(workload="mkf_fit over the hit lists mkf_build_tracks wrote for configs[3] (PAPER.md:25), hits as 48-byte records",
@@ -572,8 +574,8 @@ def run_overlap(R, seed):
         ctx.build_tracks(dh, idx, ds, ds["event"], ds["hits"], ds["plan"], out, out["chi2"], out["score"], out["nhits"],
                          out["nmiss"], out["hit_ids"], out["status"], ws=wso, hit_ids2=h2)
 
-    ms_o, launches, clk = R.timed(ctx, step)
-    ms_p, _, _ = R.timed(ctx, lambda: step(None), warm=1)
+    ms_o, launches, clk = R.timed(ctx, step, ranks=False)             # rank 0 alone gets here
+    ms_p, _, _ = R.timed(ctx, lambda: step(None), warm=1, ranks=False)
     n2 = int((h2 >= 0).sum().item())
     ctx.close()
     return dict(workload="configs[3] recipe, %d events, overlap_frac 0.25: mkf_build_hit_index + mkf_build_tracks_overlap" % nev,
@@ -600,7 +602,7 @@ def run_strips(R, w, seed):
         ctx.cluster_strips(sd, sp, out, ws)
 
     ms_total, launches, clocks = R.timed(ctx, step)
-    ms_total, u_all = aggregate(ms_total, float(n), R.world, "cuda")
+    ms_total, u_all = aggregate(ms_total, float(n), R.world, R.cdev)
     ms_step = ms_total / a.steps
     rec = dict(workload=NAMES[w], metric=METRIC["strips"][0], unit=METRIC["strips"][1], value=u_all / (ms_step * 1e-3), ms_per_step=ms_step,
                steps=a.steps, warmup=R.warm, units_per_step=u_all, gpu_launches=int(launches), clocks=clocks, dtype="u16/f32")
@@ -661,10 +663,14 @@ def main():
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl mkf needs a CUDA device (there is no CPU fallback)")
+    # MKF_BENCH_BACKEND=gloo with MKF_BENCH_ONE_GPU=1 runs every rank on GPU 0 with host-side collectives: a test of the
+    # ranks' plumbing on a one-GPU box (tests/test_gpu_bench_ranks.py), never a measurement
+    if os.environ.get("MKF_BENCH_ONE_GPU") == "1":
+        local_rank = 0
     torch.cuda.set_device(local_rank)
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl")
+        dist.init_process_group(os.environ.get("MKF_BENCH_BACKEND", "nccl"))
     sampler = ClockSampler(local_rank) if rank == 0 else None
     R = Runner(a, rank, local_rank, world, sampler)
     seed = rank_seed(a.seed, rank)
