@@ -16,6 +16,7 @@
 // an atomic cursor into a scratch list, and every hit then takes as its place in the bin the number of smaller ids it
 // finds there, writing its id and its packed record; the segment is read from HBM once (the later passes hit L2).
 // HBM-bound; algorithmic bytes per hit are listed in DESIGN.md §6.
+#include <atomic>
 #include "mkf_ctx.h"
 #include "mkf_scan.cuh"
 
@@ -433,8 +434,7 @@ namespace {
 static __device__ __align__(256) int g_hi_static_scratch[2 * (size_t)MKF_STATIC_MAX_HITS];
 
 constexpr int HI_MAX_DEVICES = 64;
-int* g_hi_static_ptr[HI_MAX_DEVICES];        // device address of the array per device (host code sees only a stand-in)
-bool g_hi_static_have[HI_MAX_DEVICES];
+std::atomic<int*> g_hi_static_ptr[HI_MAX_DEVICES];   // device address of the array per device (host code sees only a stand-in); null: not resolved yet
 
 // The array's device address on the current device: resolved once per device, with that device current.
 int hi_static_scratch(mkf_ctx* c, int** out) {
@@ -442,14 +442,13 @@ int hi_static_scratch(mkf_ctx* c, int** out) {
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return cuda_fail(c, e, "mkf_build_hit_index_static: cudaGetDevice");
   if (dev < 0 || dev >= HI_MAX_DEVICES) return fail(c, MKF_UNSUPPORTED, "mkf_build_hit_index_static: device ordinal >= 64");
-  if (!g_hi_static_have[dev]) {
-    int* p = nullptr;
+  int* p = g_hi_static_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {
     e = cudaGetSymbolAddress((void**)&p, g_hi_static_scratch);
     if (e != cudaSuccess || !p) return cuda_fail(c, e, "mkf_build_hit_index_static: cudaGetSymbolAddress");
-    g_hi_static_ptr[dev] = p;                // two threads racing here store the same value
-    g_hi_static_have[dev] = true;
+    g_hi_static_ptr[dev].store(p, std::memory_order_release);      // threads racing here store the same value
   }
-  *out = g_hi_static_ptr[dev];
+  *out = p;
   return MKF_OK;
 }
 }  // namespace
