@@ -189,6 +189,9 @@ MKF_HD void fit_one(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int 
 // material of the layer being left, propagate backward (s <= 0), transport, update. After the innermost hit that
 // layer's material is given back too (done on the covariance at the output boundary), so the result is the state
 // before it. A failing step stops the track, which keeps the state after its last good update.
+struct TagTrue { static constexpr bool value = true; };
+struct TagFalse { static constexpr bool value = false; };
+
 template <bool STRAG, bool PLANES>
 MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs& a, int i) {
   const int mflags = STRAG ? p.material_flags : (p.material_flags & 3);
@@ -212,38 +215,48 @@ MKF_HD void fit_one_backward(const GeomDev& g, const ParamsDev& p, const FitArgs
     load_params(S, a.par, n, (size_t)i);
     c2tot = 0.f; nf = 0; prev = -1;
     bool redo = false, stopped = false;
-    // no `continue` / `break` out of the layer loop: tracks of one warp meet their first hit at different steps, and
-    // threads that ran ahead would never rejoin the others (measured: 3x the instructions); the body is a plain
-    // if-region, so the warp reconverges after every layer
+    // One step: the hit `hid` of plan step s. FIRST: the track's first hit of this pass (6x6 transport of the seed
+    // covariance and its factorisation) -- a separate instance, run by all lanes of the warp together before the loop
+    // (each at its own step): 10 % of the helices of configs[1] curl before the outer layers, the tracks of a warp met
+    // their first hit at 3.3 different steps of the loop, and the warp ran that long branch as often at a third of its lanes.
+    auto step = [&](int s, int hid, auto first_tag) {
+      constexpr bool FIRST = decltype(first_tag)::value;
+      if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; return; }
+      const int li = g.plan_layers[p0 + s];
+      const LayerDev& L = g.layers[li];
+      Hit H; load_hit_t<PLANES>(H, a.hits, hid);
+      Prop P;
+      float J = 1.f, th02 = 0.f, q4 = 0.f, ipt_old = S.ipt;
+      if (!FIRST) {                                            // give back the material of the layer being left
+        const LayerDev& Lp = g.layers[prev];
+        float rp;
+        material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, mflags, rp, J, th02, q4);
+        S.ipt = ipt_old * rp;                                  // the geometry uses the momentum after the give-back
+      }
+      const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[FIRST ? li : prev], p.graze_cos_min, 0, false, P);     // R13: back along the arc of the layer being left
+      if (rc) { S.ipt = ipt_old; stat |= rc; stopped = true; return; }
+      if (FIRST) { float c[21]; load_cov(c, a.cov, n, (size_t)i); commit_first(S, c, P, 0); }
+      else commit_step_backward(S, P, J, th02, q4, mflags);
+      SInv o; float c2;
+      hit_to_local(S, H, o);
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; return; }
+      if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; return; }
+      c2tot += c2; nf++; prev = li;
+    };
+    const int* th0 = a.track_hits + i;
+    const int lo = stop_at;                                      // (stop_at changes when a step fails)
+    int sf = lo;                                                 // the track's last hit above lo (independent loads)
+    for (int t = lo + 1; t < plen; t++) if (th0[(size_t)t * n] >= 0) sf = t;
+    if (sf > lo) step(sf, th0[(size_t)sf * n], TagTrue());
+    // no `continue` / `break` out of the layer loop: threads that ran ahead would never rejoin the others (measured: 3x
+    // the instructions); the body is a plain if-region, so the warp reconverges after every layer
     const int* th = a.track_hits + (size_t)(plen - 1) * n + i;
-    int hid_next = plen - 1 > stop_at ? *th : -1;               // the hit id is fetched one step ahead
-    for (int s = plen - 1; s > stop_at; s--) {
+    int hid_next = plen - 1 > lo ? *th : -1;                    // the hit id is fetched one step ahead
+    for (int s = plen - 1; s > lo; s--) {
       const int hid = hid_next;
       th -= n;
-      hid_next = s - 1 > stop_at ? *th : -1;
-      if (hid >= 0 && !stopped) do {
-        if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; break; }
-        const int li = g.plan_layers[p0 + s];
-        const LayerDev& L = g.layers[li];
-        Hit H; load_hit_t<PLANES>(H, a.hits, hid);
-        Prop P;
-        float J = 1.f, th02 = 0.f, q4 = 0.f, ipt_old = S.ipt;
-        if (nf > 0) {                                            // give back the material of the layer being left
-          const LayerDev& Lp = g.layers[prev];
-          float rp;
-          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, mflags, rp, J, th02, q4);
-          S.ipt = ipt_old * rp;                                  // the geometry uses the momentum after the give-back
-        }
-        const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[nf > 0 ? prev : li], p.graze_cos_min, 0, false, P);     // R13: back along the arc of the layer being left
-        if (rc) { S.ipt = ipt_old; stat |= rc; stopped = true; break; }
-        if (nf == 0) { float c[21]; load_cov(c, a.cov, n, (size_t)i); commit_first(S, c, P, 0); }
-        else commit_step_backward(S, P, J, th02, q4, mflags);
-        SInv o; float c2;
-        hit_to_local(S, H, o);
-        if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; stop_at = s; redo = true; stopped = true; break; }
-        if (check && (!state_finite(S) || !(fabsf(c2) <= 3.0e38f))) { stat |= ST_NAN; stop_at = s; redo = true; stopped = true; break; }
-        c2tot += c2; nf++; prev = li;
-      } while (0);
+      hid_next = s - 1 > lo ? *th : -1;
+      if (hid >= 0 && s < sf && !stopped) step(s, hid, TagFalse());
     }
     if (redo) continue;
     if (pass == 0 && nf > 0 && (!state_finite(S) || !(fabsf(c2tot) <= 3.0e38f))) continue;
