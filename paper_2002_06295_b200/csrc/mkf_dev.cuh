@@ -424,74 +424,80 @@ MKF_HD void fit_smooth_one(const GeomDev& g, const ParamsDev& p, const SmoothArg
   KState S;
   load_params(S, a.par, n, (size_t)i);
   float c2tot = 0.f; int nf = 0, last_s = -1; bool smoothable = true;
+  // Both layer loops run over the plan steps for the whole warp, their bodies plain if-regions (no `continue` / `break`:
+  // a thread that leaves a loop early runs ahead of its warp, alone, and the warp does the rest of its work twice).
+  bool stopped = false;
   int hid_next = plen > 0 ? a.track_hits[i] : -1;                // ids one step ahead, the hit before the propagation:
   for (int s = 0; s < plen; s++) {                               // their latency overlaps the arithmetic
     const int hid = hid_next;
     hid_next = s + 1 < plen ? a.track_hits[(size_t)(s + 1) * n + i] : -1;
-    if (hid < 0) continue;
-    if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; break; }
-    Hit H; load_hit(H, a.hits, hid);
-    const int li = g.plan_layers[p0 + s];
-    const LayerDev& L = g.layers[li];
-    const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
-    if (rc) { stat |= rc; break; }
-    float* w = sa.ws + (size_t)s * n + i;
-    const size_t st = (size_t)mpl * n;
-    w[0] = S.x; w[st] = S.y; w[2 * st] = S.z; w[3 * st] = S.xl; w[4 * st] = S.yl; w[5 * st] = S.zl;
-    w[6 * st] = S.ipt; w[7 * st] = S.phi; w[8 * st] = S.th;
-#pragma unroll
-    for (int k = 0; k < 10; k++) w[(9 + k) * st] = S.u[k];
-#pragma unroll
-    for (int k = 0; k < 5; k++) w[(19 + k) * st] = S.d[k];
-    SInv o; float c2;
-    hit_to_local(S, H, o);
-    if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; smoothable = false; break; }
-    if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; smoothable = false; break; }
-    c2tot += c2; nf++; last_s = s;
-  }
-  a.chi2[i] = c2tot; a.nfit[i] = nf;
-  bool ok = smoothable && nf > 0;
-  if (ok) {
-#pragma unroll
-    for (int k = 0; k < 5; k++) S.d[k] *= 1e4f;                  // the backward filter starts from a weak prior
-    int prev = -1;
-    hid_next = a.track_hits[(size_t)last_s * n + i];
-    for (int s = last_s; s >= 0 && ok; s--) {
-      const int hid = hid_next;
-      hid_next = s > 0 ? a.track_hits[(size_t)(s - 1) * n + i] : -1;
-      if (hid < 0) continue;
+    if (hid >= 0 && !stopped) do {
+      if (hid >= a.hits.n_hits) { stat |= ST_TRUNC; stopped = true; break; }
       Hit H; load_hit(H, a.hits, hid);
       const int li = g.plan_layers[p0 + s];
       const LayerDev& L = g.layers[li];
-      float J = 1.f, th02 = 0.f, q4 = 0.f;
-      if (prev >= 0) {
-        const LayerDev& Lp = g.layers[prev];
-        float rp;
-        material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
-        S.ipt *= rp;
-      }
-      Prop P;
-      const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[prev >= 0 ? prev : li], p.graze_cos_min, 0, false, P);
-      if (rc) { stat |= rc; ok = false; break; }
-      commit_step_backward(S, P, J, th02, q4, p.material_flags);
+      const unsigned rc = step_to_layer(S, nf == 0, a.cov, n, (size_t)i, L, qk * g.bz_layer[li], p.graze_cos_min, p.material_flags, false);
+      if (rc) { stat |= rc; stopped = true; break; }
+      float* w = sa.ws + (size_t)s * n + i;
+      const size_t st = (size_t)mpl * n;
+      w[0] = S.x; w[st] = S.y; w[2 * st] = S.z; w[3 * st] = S.xl; w[4 * st] = S.yl; w[5 * st] = S.zl;
+      w[6 * st] = S.ipt; w[7 * st] = S.phi; w[8 * st] = S.th;
+#pragma unroll
+      for (int k = 0; k < 10; k++) w[(9 + k) * st] = S.u[k];
+#pragma unroll
+      for (int k = 0; k < 5; k++) w[(19 + k) * st] = S.d[k];
       SInv o; float c2;
       hit_to_local(S, H, o);
-      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
-      if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; ok = false; break; }
-      float fw[SM_NF];
-      const size_t st = (size_t)mpl * n;
-      const float* w = sa.ws + (size_t)s * n + i;
+      if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; smoothable = false; stopped = true; break; }
+      if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; smoothable = false; stopped = true; break; }
+      c2tot += c2; nf++; last_s = s;
+    } while (0);
+  }
+  a.chi2[i] = c2tot; a.nfit[i] = nf;
+  bool ok = smoothable && nf > 0;
+  const bool had = ok;
+  {
 #pragma unroll
-      for (int k = 0; k < SM_NF; k++) fw[k] = w[k * st];
-      float par6[6], c21[21];
-      if (!smooth_combine_dev(fw, L.kind, S, par6, c21)) { stat |= ST_S_NOT_PD; ok = false; break; }
+    for (int k = 0; k < 5; k++) S.d[k] *= 1e4f;                  // the backward filter starts from a weak prior
+    int prev = -1;
+    hid_next = plen > 0 ? a.track_hits[(size_t)(plen - 1) * n + i] : -1;
+    for (int s = plen - 1; s >= 0; s--) {
+      const int hid = hid_next;
+      hid_next = s > 0 ? a.track_hits[(size_t)(s - 1) * n + i] : -1;
+      if (ok && s <= last_s && hid >= 0) do {
+        Hit H; load_hit(H, a.hits, hid);
+        const int li = g.plan_layers[p0 + s];
+        const LayerDev& L = g.layers[li];
+        float J = 1.f, th02 = 0.f, q4 = 0.f;
+        if (prev >= 0) {
+          const LayerDev& Lp = g.layers[prev];
+          float rp;
+          material_scalars<-1>(Lp.xx0, incidence_of(S), S.ipt, S.sth, p.material_flags, rp, J, th02, q4);
+          S.ipt *= rp;
+        }
+        Prop P;
+        const unsigned rc = propagate_geom<-1>(S, L, qk * g.bz_layer[prev >= 0 ? prev : li], p.graze_cos_min, 0, false, P);
+        if (rc) { stat |= rc; ok = false; break; }
+        commit_step_backward(S, P, J, th02, q4, p.material_flags);
+        SInv o; float c2;
+        hit_to_local(S, H, o);
+        if (!kalman_update(S, o, c2)) { stat |= ST_S_NOT_PD; ok = false; break; }
+        if (!state_finite(S) || !(fabsf(c2) <= 3.0e38f)) { stat |= ST_NAN; ok = false; break; }
+        float fw[SM_NF];
+        const size_t st = (size_t)mpl * n;
+        const float* w = sa.ws + (size_t)s * n + i;
 #pragma unroll
-      for (int k = 0; k < 6; k++) sa.par_s[((size_t)s * 6 + k) * n + i] = par6[k];
+        for (int k = 0; k < SM_NF; k++) fw[k] = w[k * st];
+        float par6[6], c21[21];
+        if (!smooth_combine_dev(fw, L.kind, S, par6, c21)) { stat |= ST_S_NOT_PD; ok = false; break; }
 #pragma unroll
-      for (int k = 0; k < 21; k++) sa.cov_s[((size_t)s * 21 + k) * n + i] = c21[k];
-      prev = li;
+        for (int k = 0; k < 6; k++) sa.par_s[((size_t)s * 6 + k) * n + i] = par6[k];
+#pragma unroll
+        for (int k = 0; k < 21; k++) sa.cov_s[((size_t)s * 21 + k) * n + i] = c21[k];
+        prev = li;
+      } while (0);
     }
-    if (!ok)                                                     // not smoothed: every state of the track is zero
+    if (had && !ok)                                              // not smoothed: every state of the track is zero
       for (int s = 0; s < mpl; s++) {
         for (int k = 0; k < 6; k++) sa.par_s[((size_t)s * 6 + k) * n + i] = 0.f;
         for (int k = 0; k < 21; k++) sa.cov_s[((size_t)s * 21 + k) * n + i] = 0.f;
