@@ -95,7 +95,7 @@ class ClockSampler:
         self.samples, self.proc = [], None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=subprocess.PIPE,
+                                          "--format=csv,noheader,nounits", "-lms", "10"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
@@ -112,7 +112,7 @@ class ClockSampler:
             for _ in range(10):
                 if any(t > t1 for t, _ in self.samples):
                     break
-                time.sleep(0.05)
+                time.sleep(0.02)
             near = sorted(self.samples, key=lambda ts: abs(ts[0] - 0.5 * (t0 + t1)))[:3]
             inside = [s for _, s in near]
         mhz, mx, reasons = [], 0.0, set()
